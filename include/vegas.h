@@ -1,0 +1,192 @@
+/*
+ * vegas.h -- C ABI of the B200-native Vegas iteration library (libvegas_b200.so).
+ *
+ * What it computes.  One Vegas importance-sampling iteration over n events in d dimensions on
+ * [0,1]^d ("importance sampling as implemented in Vegas", section 2.2), the grid
+ * refinement that follows every iteration ("refine how the random numbers are generated",
+ * PAPER.md:49-51) and the value +- error combination of iterations (result format of Table 1,
+ * PAPER.md:83-86).  The integrands are the paper's toy functions (Eqs.(1),(3))
+ * plus the synthetic stand-in for its LO single-top run named in
+ * BASELINE.json:configs.  All numerical conventions the paper leaves open are the readings
+ * C1..C11 listed in DESIGN.md ("Readings of the paper"); BASELINE.json:north_star names the calls.
+ *
+ * Per event e of iteration k (all in registers / shared memory of one fused kernel):
+ *   word_j  = Philox4x32-10(counter = (j>>2, k, e lo, e hi), key = (seed lo, seed hi))[j&3]   (C1,C2)
+ *   b_j     = (word_j * n_bins) >> 32 ;  r_j = ((word_j * n_bins mod 2^32) + 1/2) * 2^-32      (C3)
+ *   x_j     = X[j][b_j] + (X[j][b_j+1] - X[j][b_j]) * r_j ;  J = prod_j n_bins * Delta_j       (C4)
+ *   v       = f(x) * J ;  S1 += v ;  S2 += v^2 ;  H[j][b_j] += v^2 for every j                 (C5,C6)
+ * and per iteration  I = S1/n,  sigma^2 = (S2/n - I^2)/(n-1)                                    (C7).
+ *
+ * Conventions for every entry point
+ *   - Return value: 0 (VEGAS_OK) or a negative VEGAS_E* code; vegas_strerror() explains it.  No C++
+ *     exception crosses this boundary.  There is no global state; calls on ONE vegas_grid are not
+ *     thread-safe, different grids are independent.
+ *   - "host" pointers are ordinary host memory owned by the caller (pageable or pinned), row-major,
+ *     fp64 unless stated.  "device" pointers are CUDA device memory owned by the caller.
+ *   - The library never allocates device memory and never creates streams: the caller provides one
+ *     device workspace at vegas_create() (vegas_workspace_bytes() says how large, 256-byte aligned)
+ *     and a CUstream / cudaStream_t handle (as void*, NULL = default stream) per call.  With PyTorch:
+ *     torch.empty(nbytes, dtype=torch.uint8, device="cuda").data_ptr() and
+ *     torch.cuda.current_stream().cuda_stream.
+ *   - Calls that return numbers to host pointers synchronise the given stream before returning.
+ *     Calls documented as "asynchronous" only enqueue work on the stream.
+ *   - There is NO CPU fallback: without a usable CUDA device every compute call returns VEGAS_ECUDA.
+ */
+#ifndef VEGAS_B200_H
+#define VEGAS_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define VEGAS_OK 0
+#define VEGAS_EINVAL (-1)   /* bad argument: dim not in [1,32], n_bins not in [2,256], n_events < 2,
+                               unknown integrand id / precision, wrong n_params, workspace too small
+                               or misaligned, edges not strictly increasing from 0 to 1, alpha < 0,
+                               NULL where a pointer is required                                    */
+#define VEGAS_ECUDA (-2)    /* a CUDA runtime call or kernel launch failed (message: vegas_strerror
+                               on the grid-less code, details via vegas_last_cuda_error())          */
+#define VEGAS_ENUMERIC (-3) /* S1 or S2 came out non-finite, or vegas_refine() met a dimension whose
+                               smoothed histogram has no finite positive sum (that dimension's grid
+                               is left unchanged, the others are refined)                           */
+
+#define VEGAS_MAX_DIM 32
+#define VEGAS_MAX_BINS 256
+#define VEGAS_MAX_PARAMS 160
+
+/* integrand ids (reading C5) and their host parameter arrays for vegas_set_params():
+ *   VEGAS_F_CONST              f = 1                                               n_params = 0
+ *   VEGAS_F_GAUSS              PAPER.md:65 Eq.(1): (a sqrt(pi))^-d exp(-sum_j (x_j-1/2)^2/a^2)
+ *                              params = { a }                                      n_params = 1
+ *   VEGAS_F_GENZ_PRODUCT_PEAK  PAPER.md:74 Eq.(3) with N = 1: prod_j 1/(c_j^-2 + (x_j-w_j)^2)
+ *                              params = { c[0..d-1], w[0..d-1] }                   n_params = 2d
+ *   VEGAS_F_BW_POLY            BASELINE.json:configs[4]: s = m_min^2 + x_0 (m_max^2 - m_min^2),
+ *                              f = M^2 G^2/((s-M^2)^2 + M^2 G^2) * sum_{i=1..d-1} sum_{k=0..4} a[i][k] x_i^k
+ *                              params = { M, G, m_min, m_max, a[1][0..4], ..., a[d-1][0..4] }
+ *                                                                                  n_params = 4+5(d-1), d >= 2 */
+#define VEGAS_F_CONST 0
+#define VEGAS_F_GAUSS 1
+#define VEGAS_F_GENZ_PRODUCT_PEAK 2
+#define VEGAS_F_BW_POLY 3
+
+/* precision of the per-event arithmetic (reading C11): 64 = everything fp64; 32 = grid table, r, x,
+ * J, f and v in fp32, v widened to fp64 before S1 += v, S2 += v^2, H += v^2.  Words, bins, the master
+ * grid, the sums, the histogram and the refinement are identical / fp64 in both. */
+#define VEGAS_FP64 64
+#define VEGAS_FP32 32
+
+typedef struct vegas_grid vegas_grid; /* opaque host object; owns no device memory */
+
+/* Device bytes the caller must provide to vegas_create() for this (dim, n_bins).  0 if invalid. */
+size_t vegas_workspace_bytes(int dim, int n_bins);
+
+/* Create a grid on the CURRENT CUDA device with the uniform start grid X[j][i] = i/n_bins (C4),
+ * written into the workspace on the default stream (synchronous).  dev_workspace: device pointer,
+ * 256-byte aligned, at least vegas_workspace_bytes() bytes, must outlive the grid.  *out receives the
+ * handle (host object, released by vegas_destroy).  The integrand defaults to VEGAS_F_CONST. */
+int vegas_create(int dim, int n_bins, void* dev_workspace, size_t bytes, vegas_grid** out);
+int vegas_destroy(vegas_grid* g);
+
+/* Copy the integrand parameter array (host, fp64, layout above) into the grid object; it is passed
+ * to the kernels by value at every launch.  Required before iterating with that integrand id
+ * (except VEGAS_F_CONST).  Parameters of several ids can be set; each id keeps its own array. */
+int vegas_set_params(vegas_grid* g, int integrand_id, const double* params_host, int n_params);
+
+/* Inject / read the master grid: edges_host is [dim][n_bins+1] fp64, every row strictly increasing
+ * with first element 0 and last element 1 (checked -> VEGAS_EINVAL).  Synchronous on `stream`. */
+int vegas_set_edges(vegas_grid* g, const double* edges_host, void* cuda_stream);
+int vegas_get_edges(vegas_grid* g, double* edges_host, void* cuda_stream);
+/* Read the histogram [dim][n_bins] left on the device by the last iteration (sum of v^2, C6). */
+int vegas_get_hist(vegas_grid* g, double* hist_host, void* cuda_stream);
+
+/* One Vegas iteration (steps S1-S7 of SURVEY.md 8(a)): n_events events with global indices
+ * 0..n_events-1 of iteration `iteration`, processed in launches of at most chunk_events events
+ * (0 = a single launch; the result does not depend on it beyond summation order, every event's RNG
+ * counter is its global index, C2).  Writes I and sigma (host doubles, C7) and, if hist_host is not
+ * NULL, the histogram [dim][n_bins] (host); the histogram also stays on the device for
+ * vegas_refine(g, NULL, ...).  Synchronises `stream` before returning.
+ * Errors: VEGAS_EINVAL (n_events < 2, unknown id/precision, params not set), VEGAS_ECUDA,
+ * VEGAS_ENUMERIC (I, sigma are still written). */
+int vegas_iterate(vegas_grid* g, uint64_t n_events, uint64_t chunk_events, uint64_t seed,
+                  uint32_t iteration, int integrand_id, int precision, void* cuda_stream, double* I,
+                  double* sigma, double* hist_host);
+
+/* The same iteration split into its asynchronous pieces, for sharding events over several GPUs /
+ * processes: every rank calls begin, accumulate on ITS event range
+ * [first_event, first_event+count), reduce; the ranks then sum the vegas_totals_count() doubles at
+ * vegas_totals_device() (one all-reduce); every rank calls finalize with the GLOBAL event count.
+ * begin/accumulate/reduce only enqueue work; finalize synchronises like vegas_iterate. */
+int vegas_begin_iteration(vegas_grid* g, void* cuda_stream);
+int vegas_accumulate(vegas_grid* g, uint64_t first_event, uint64_t count, uint64_t chunk_events,
+                     uint64_t seed, uint32_t iteration, int integrand_id, int precision,
+                     void* cuda_stream);
+int vegas_reduce(vegas_grid* g, void* cuda_stream);
+int vegas_finalize(vegas_grid* g, uint64_t n_events_total, void* cuda_stream, double* I, double* sigma,
+                   double* hist_host);
+/* Device address / length (in doubles) of the reduced totals { S1_hi, S1_lo, S2_hi, S2_lo,
+ * H[dim][n_bins] } that vegas_reduce() writes and vegas_finalize() / vegas_refine() read. */
+void* vegas_totals_device(vegas_grid* g);
+size_t vegas_totals_count(const vegas_grid* g);
+
+/* Refine the grid (step S8, reading C8: smooth, normalise, compress with damping alpha, rebin), per
+ * dimension, fp64.  hist_host NULL = use the histogram the last iteration left on the device;
+ * otherwise [dim][n_bins] fp64 is uploaded first.  Synchronises `stream`.
+ * Errors: VEGAS_EINVAL (alpha < 0 or NaN), VEGAS_ECUDA, VEGAS_ENUMERIC (see above). */
+int vegas_refine(vegas_grid* g, const double* hist_host, double alpha, void* cuda_stream);
+
+/* n_iter iterations (iteration indices 0..n_iter-1), each followed by a refinement (also the skipped
+ * ones; alpha < 0 disables refinement = importance sampling on a fixed grid), then the
+ * inverse-variance combination of iterations k >= n_skip (step S9, reading C9):
+ * W = sum 1/sigma_k^2, I = sum(I_k/sigma_k^2)/W, sigma = W^-1/2, chi2_dof = sum (I_k-I)^2/sigma_k^2/(K-1);
+ * if an included sigma_k is 0: plain mean, sigma = 0.  All launches are enqueued back to back; the
+ * stream is synchronised once at the end.  per_iter_host: [n_iter][2] = (I_k, sigma_k) or NULL.
+ * Errors: VEGAS_EINVAL (n_iter < 1 or > 4096, n_skip not in [0,n_iter), ...), VEGAS_ECUDA,
+ * VEGAS_ENUMERIC (outputs still written). */
+int vegas_integrate(vegas_grid* g, int n_iter, int n_skip, uint64_t n_events, uint64_t chunk_events,
+                    uint64_t seed, double alpha, int integrand_id, int precision, void* cuda_stream,
+                    double* I, double* sigma, double* chi2_dof, double* per_iter_host);
+
+/* Step S9 alone on host arrays (no device work). */
+int vegas_combine(int n_iter, int n_skip, const double* I_k, const double* sigma_k, double* I,
+                  double* sigma, double* chi2_dof);
+
+/* Parity hook (kernel K4): for events first_event .. first_event+count-1 of `iteration`, run exactly
+ * the device functions of the fused kernel and return, to HOST arrays (any may be NULL):
+ *   words [count][dim] u32 (C2), bins [count][dim] i32 (C3), x [count][dim] fp64 (C4; fp32 values
+ *   widened when precision = 32), fJ [count] fp64 (v = f*J).  dev_scratch: device memory of at least
+ *   vegas_debug_scratch_bytes(dim, count) bytes, caller-owned.  Synchronises `stream`. */
+size_t vegas_debug_scratch_bytes(int dim, uint32_t count);
+int vegas_debug_sample(vegas_grid* g, uint64_t first_event, uint32_t count, uint64_t seed,
+                       uint32_t iteration, int integrand_id, int precision, void* dev_scratch,
+                       void* cuda_stream, uint32_t* words, int32_t* bins, double* x, double* fJ);
+
+/* Launch shape of the fused kernel.  0 = automatic for any field.  blocks: CTAs per launch (default:
+ * one per SM); threads: per CTA (multiple of 32, <= 1024); table_copies / hist_copies: bank-interleaved
+ * replicas of the grid table / histogram in shared memory (powers of two, <= 32), see DESIGN.md.
+ * VEGAS_EINVAL if the combination does not fit the device's shared memory. */
+int vegas_set_launch(vegas_grid* g, int blocks, int threads, int table_copies, int hist_copies);
+int vegas_get_launch(vegas_grid* g, int precision, int* blocks, int* threads, int* table_copies,
+                     int* hist_copies, size_t* shared_bytes);
+
+/* Instrumentation for bench.py: with profiling on, every fused-kernel launch is bracketed by CUDA
+ * events on its stream; vegas_kernel_time_ms() synchronises those events and returns their summed
+ * duration and the number of launches since the last vegas_reset_counters().  vegas_launch_count()
+ * counts ALL kernels of this library launched for the grid (no synchronisation). */
+int vegas_set_profiling(vegas_grid* g, int on);
+int vegas_kernel_time_ms(vegas_grid* g, double* iterate_kernel_ms, uint64_t* iterate_launches);
+uint64_t vegas_launch_count(const vegas_grid* g);
+int vegas_reset_counters(vegas_grid* g);
+
+const char* vegas_strerror(int code);
+/* Text of the last CUDA error seen by a call on this grid ("" if none); valid until the next call. */
+const char* vegas_last_cuda_error(const vegas_grid* g);
+/* Library version / build string, e.g. "vegas_b200 0.1 sm_100a". */
+const char* vegas_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VEGAS_B200_H */

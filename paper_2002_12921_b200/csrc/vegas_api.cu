@@ -1,0 +1,607 @@
+// vegas_api.cu -- host driver and C ABI (include/vegas.h) of libvegas_b200.so.
+// Chunk loop, launch configuration, workspace carving, parameter derivation, error codes.
+// No device allocation, no stream creation, no CPU fallback: every compute entry point launches
+// the sm_100a kernels of vegas_kernels.cu or fails with VEGAS_ECUDA.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/vegas.h"
+#include "vegas_kernels.h"
+
+namespace {
+
+constexpr int kMaxBlocks = 1024;      // per-CTA partial slots carved from the workspace
+constexpr int kMaxIter = 4096;        // per-iteration result slots (vegas_integrate)
+constexpr int kResultStride = 4;      // { I, sigma, status, pad } doubles per iteration
+constexpr size_t kAlign = 256;
+
+size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+struct Layout {
+    size_t edges, totals, result, status, hist_up, partials, total;
+};
+
+Layout make_layout(int dim, int n_bins) {
+    Layout L;
+    const size_t nent = (size_t)dim * n_bins, ntot = 4 + nent;
+    size_t off = 0;
+    L.edges = off;    off += align_up(sizeof(double) * dim * (n_bins + 1));
+    L.totals = off;   off += align_up(sizeof(double) * ntot);
+    L.result = off;   off += align_up(sizeof(double) * kResultStride * kMaxIter);
+    L.status = off;   off += align_up(sizeof(int) * 8);
+    L.hist_up = off;  off += align_up(sizeof(double) * nent);
+    L.partials = off; off += align_up(sizeof(double) * ntot * kMaxBlocks);
+    L.total = off;
+    return L;
+}
+
+bool valid_shape(int dim, int n_bins) {
+    return dim >= 1 && dim <= VEGAS_MAX_DIM && n_bins >= 2 && n_bins <= VEGAS_MAX_BINS;
+}
+
+int expected_n_params(int fid, int dim) {
+    switch (fid) {
+    case VEGAS_F_CONST: return 0;
+    case VEGAS_F_GAUSS: return 1;
+    case VEGAS_F_GENZ_PRODUCT_PEAK: return 2 * dim;
+    case VEGAS_F_BW_POLY: return dim >= 2 ? 4 + 5 * (dim - 1) : -1;
+    default: return -1;
+    }
+}
+
+}  // namespace
+
+struct vegas_grid {
+    int dim = 0, n_bins = 0, device = 0, sm_count = 0;
+    size_t smem_optin = 0;
+    unsigned char* ws = nullptr;
+    Layout L{};
+    double* d_edges = nullptr;
+    double* d_totals = nullptr;
+    double* d_result = nullptr;
+    int* d_status = nullptr;
+    double* d_hist_up = nullptr;
+    double* d_partials = nullptr;
+    bool params_set[4] = {true, false, false, false};
+    double derived[4][VEGAS_MAX_PARAMS] = {};
+    int cfg_blocks = 0, cfg_threads = 0, cfg_ct = 0, cfg_ch = 0;
+    int active_blocks = 0;          // CTAs whose partial slots the current iteration uses
+    bool profiling = false;
+    std::vector<cudaEvent_t> events;   // pairs (start, stop)
+    size_t events_used = 0;
+    double kernel_ms_acc = 0.0;
+    uint64_t iterate_launches = 0, launches = 0;
+    char cuda_err[256] = "";
+};
+
+namespace {
+
+int cuda_fail(vegas_grid* g, cudaError_t e, const char* what) {
+    if (g) snprintf(g->cuda_err, sizeof(g->cuda_err), "%s: %s", what, cudaGetErrorString(e));
+    return VEGAS_ECUDA;
+}
+
+#define CUDA_TRY(g, call)                                        \
+    do {                                                         \
+        cudaError_t e__ = (call);                                \
+        if (e__ != cudaSuccess) return cuda_fail(g, e__, #call); \
+    } while (0)
+
+struct LaunchShape {
+    int blocks, threads, ct, ch;
+    size_t shmem;
+};
+
+// Predicted shared-pipe cost (SM clocks per warp-wide access) of the table gather and of the
+// histogram CAS update as a function of the copy count, from the step-0 microbenchmarks on a
+// B200 (profiles/r01_ubench_pipes.md).  Only used to rank (ct, ch) pairs that fit.
+double table_cost(int precision, int ct) {
+    static const double c64[] = {9.5, 9.4, 7.9, 6.5, 6.5, 6.5};     // ct = 1,2,4,8,(16,32)
+    static const double c32[] = {6.0, 5.6, 5.0, 4.2, 3.4, 3.4};
+    int l = 0;
+    while ((1 << l) < ct) ++l;
+    return precision == VEGAS_FP64 ? c64[l] : c32[l];
+}
+double hist_cost(int ch) {
+    static const double c[] = {26.0, 23.5, 20.0, 15.5, 9.7, 9.0};   // ch = 1,2,4,8,16,32
+    int l = 0;
+    while ((1 << l) < ch) ++l;
+    return c[l];
+}
+
+int resolve_launch(const vegas_grid* g, int precision, LaunchShape* out) {
+    LaunchShape s;
+    s.blocks = g->cfg_blocks > 0 ? g->cfg_blocks : g->sm_count;
+    s.threads = g->cfg_threads > 0 ? g->cfg_threads : vegas::kIterMaxThreads;
+    if (s.blocks > kMaxBlocks || s.threads > vegas::kIterMaxThreads || s.threads % 32) return VEGAS_EINVAL;
+    const int max_ct = precision == VEGAS_FP64 ? 8 : 16;
+    double best = 1e300;
+    s.ct = s.ch = 0;
+    for (int ch = 1; ch <= 32; ch *= 2) {
+        if (g->cfg_ch > 0 && ch != g->cfg_ch) continue;
+        if (g->cfg_ch == 0 && ch > 16) continue;
+        for (int ct = 1; ct <= 32; ct *= 2) {
+            if (g->cfg_ct > 0 && ct != g->cfg_ct) continue;
+            if (g->cfg_ct == 0 && ct > max_ct) continue;
+            const size_t sh = vegas::iterate_shared_bytes(g->dim, g->n_bins, precision, ct, ch);
+            if (sh > g->smem_optin) continue;
+            const double cost = table_cost(precision, ct) + hist_cost(ch) + 1e-9 * (double)sh;
+            if (cost < best) { best = cost; s.ct = ct; s.ch = ch; s.shmem = sh; }
+        }
+    }
+    if (s.ct == 0) return VEGAS_EINVAL;
+    *out = s;
+    return VEGAS_OK;
+}
+
+int ilog2(int v) {
+    int l = 0;
+    while ((1 << l) < v) ++l;
+    return l;
+}
+
+bool check_call(const vegas_grid* g, int fid, int precision) {
+    if (!g) return false;
+    if (fid < 0 || fid > 3 || !g->params_set[fid]) return false;
+    if (expected_n_params(fid, g->dim) < 0) return false;
+    return precision == VEGAS_FP64 || precision == VEGAS_FP32;
+}
+
+double jac_scale_for(const vegas_grid* g, int precision) {
+    if (precision != VEGAS_FP64) return 1.0;
+    double s = 1.0;
+    for (int j = 0; j < g->dim; ++j) s *= (double)g->n_bins;
+    return s;
+}
+
+int finish_iteration(vegas_grid* g, uint64_t n_total, cudaStream_t st, double* I, double* sigma, double* hist_host) {
+    const size_t nent = (size_t)g->dim * g->n_bins;
+    CUDA_TRY(g, vegas::launch_finalize(g->d_totals, (double)n_total, g->d_result, st));
+    g->launches++;
+    double res[3] = {0, 0, 0};
+    CUDA_TRY(g, cudaMemcpyAsync(res, g->d_result, sizeof(res), cudaMemcpyDeviceToHost, st));
+    if (hist_host)
+        CUDA_TRY(g, cudaMemcpyAsync(hist_host, g->d_totals + 4, sizeof(double) * nent, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(g, cudaStreamSynchronize(st));
+    if (I) *I = res[0];
+    if (sigma) *sigma = res[1];
+    return res[2] == 0.0 ? VEGAS_OK : VEGAS_ENUMERIC;
+}
+
+}  // namespace
+
+#pragma GCC visibility push(default)
+extern "C" {
+
+size_t vegas_workspace_bytes(int dim, int n_bins) {
+    if (!valid_shape(dim, n_bins)) return 0;
+    return make_layout(dim, n_bins).total;
+}
+
+int vegas_create(int dim, int n_bins, void* dev_workspace, size_t bytes, vegas_grid** out) {
+    if (!out) return VEGAS_EINVAL;
+    *out = nullptr;
+    if (!valid_shape(dim, n_bins) || !dev_workspace) return VEGAS_EINVAL;
+    if (((uintptr_t)dev_workspace) % kAlign) return VEGAS_EINVAL;
+    const Layout L = make_layout(dim, n_bins);
+    if (bytes < L.total) return VEGAS_EINVAL;
+    vegas_grid* g = new (std::nothrow) vegas_grid();
+    if (!g) return VEGAS_EINVAL;
+    cudaError_t e = cudaGetDevice(&g->device);
+    cudaDeviceProp prop;
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, g->device);
+    if (e != cudaSuccess) { delete g; return VEGAS_ECUDA; }
+    g->dim = dim;
+    g->n_bins = n_bins;
+    g->sm_count = prop.multiProcessorCount;
+    g->smem_optin = prop.sharedMemPerBlockOptin;
+    g->ws = (unsigned char*)dev_workspace;
+    g->L = L;
+    g->d_edges = (double*)(g->ws + L.edges);
+    g->d_totals = (double*)(g->ws + L.totals);
+    g->d_result = (double*)(g->ws + L.result);
+    g->d_status = (int*)(g->ws + L.status);
+    g->d_hist_up = (double*)(g->ws + L.hist_up);
+    g->d_partials = (double*)(g->ws + L.partials);
+    std::vector<double> edges((size_t)dim * (n_bins + 1));
+    for (int j = 0; j < dim; ++j)
+        for (int i = 0; i <= n_bins; ++i) edges[(size_t)j * (n_bins + 1) + i] = (double)i / (double)n_bins;
+    e = cudaMemcpy(g->d_edges, edges.data(), sizeof(double) * edges.size(), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemset(g->d_totals, 0, L.hist_up + align_up(sizeof(double) * dim * n_bins) - L.totals);
+    if (e != cudaSuccess) { delete g; return VEGAS_ECUDA; }
+    *out = g;
+    return VEGAS_OK;
+}
+
+int vegas_destroy(vegas_grid* g) {
+    if (!g) return VEGAS_EINVAL;
+    for (cudaEvent_t ev : g->events) cudaEventDestroy(ev);
+    delete g;
+    return VEGAS_OK;
+}
+
+int vegas_set_params(vegas_grid* g, int fid, const double* p, int n_params) {
+    if (!g || fid < 0 || fid > 3) return VEGAS_EINVAL;
+    const int want = expected_n_params(fid, g->dim);
+    if (want < 0 || n_params != want || want > VEGAS_MAX_PARAMS || (want > 0 && !p)) return VEGAS_EINVAL;
+    for (int i = 0; i < want; ++i)
+        if (!std::isfinite(p[i])) return VEGAS_EINVAL;
+    double* d = g->derived[fid];
+    std::memset(d, 0, sizeof(g->derived[fid]));
+    const int dim = g->dim;
+    switch (fid) {
+    case VEGAS_F_CONST: break;
+    case VEGAS_F_GAUSS: {
+        const double a = p[0];
+        if (!(a > 0.0)) return VEGAS_EINVAL;
+        d[0] = std::pow(a * std::sqrt(3.14159265358979323846), -(double)dim);
+        d[1] = 1.0 / (a * a);
+        break;
+    }
+    case VEGAS_F_GENZ_PRODUCT_PEAK:
+        for (int j = 0; j < dim; ++j) {
+            if (p[j] == 0.0) return VEGAS_EINVAL;
+            d[2 * j] = 1.0 / (p[j] * p[j]);
+            d[2 * j + 1] = p[dim + j];
+        }
+        break;
+    case VEGAS_F_BW_POLY: {
+        const double M = p[0], G = p[1], m_min = p[2], m_max = p[3];
+        d[0] = m_min * m_min;
+        d[1] = m_max * m_max - m_min * m_min;
+        d[2] = M * M;
+        d[3] = M * M * G * G;
+        if (!(d[3] > 0.0)) return VEGAS_EINVAL;
+        for (int i = 0; i < 5 * (dim - 1); ++i) d[4 + i] = p[4 + i];
+        break;
+    }
+    }
+    g->params_set[fid] = true;
+    return VEGAS_OK;
+}
+
+int vegas_set_edges(vegas_grid* g, const double* edges_host, void* cuda_stream) {
+    if (!g || !edges_host) return VEGAS_EINVAL;
+    const int nb = g->n_bins;
+    for (int j = 0; j < g->dim; ++j) {
+        const double* X = edges_host + (size_t)j * (nb + 1);
+        if (X[0] != 0.0 || X[nb] != 1.0) return VEGAS_EINVAL;
+        for (int i = 0; i < nb; ++i)
+            if (!(X[i + 1] > X[i])) return VEGAS_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CUDA_TRY(g, cudaSetDevice(g->device));
+    CUDA_TRY(g, cudaMemcpyAsync(g->d_edges, edges_host, sizeof(double) * g->dim * (nb + 1), cudaMemcpyHostToDevice, st));
+    CUDA_TRY(g, cudaStreamSynchronize(st));
+    return VEGAS_OK;
+}
+
+int vegas_get_edges(vegas_grid* g, double* edges_host, void* cuda_stream) {
+    if (!g || !edges_host) return VEGAS_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CUDA_TRY(g, cudaSetDevice(g->device));
+    CUDA_TRY(g, cudaMemcpyAsync(edges_host, g->d_edges, sizeof(double) * g->dim * (g->n_bins + 1), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(g, cudaStreamSynchronize(st));
+    return VEGAS_OK;
+}
+
+int vegas_get_hist(vegas_grid* g, double* hist_host, void* cuda_stream) {
+    if (!g || !hist_host) return VEGAS_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CUDA_TRY(g, cudaSetDevice(g->device));
+    CUDA_TRY(g, cudaMemcpyAsync(hist_host, g->d_totals + 4, sizeof(double) * g->dim * g->n_bins, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(g, cudaStreamSynchronize(st));
+    return VEGAS_OK;
+}
+
+int vegas_begin_iteration(vegas_grid* g, void* cuda_stream) {
+    if (!g) return VEGAS_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CUDA_TRY(g, cudaSetDevice(g->device));
+    LaunchShape s;
+    if (resolve_launch(g, VEGAS_FP64, &s)) return VEGAS_EINVAL;
+    g->active_blocks = s.blocks;
+    const size_t ntot = 4 + (size_t)g->dim * g->n_bins;
+    CUDA_TRY(g, cudaMemsetAsync(g->d_partials, 0, sizeof(double) * ntot * s.blocks, st));
+    return VEGAS_OK;
+}
+
+int vegas_accumulate(vegas_grid* g, uint64_t first_event, uint64_t count, uint64_t chunk_events, uint64_t seed,
+                     uint32_t iteration, int fid, int precision, void* cuda_stream) {
+    if (!check_call(g, fid, precision)) return VEGAS_EINVAL;
+    if (g->active_blocks <= 0) return VEGAS_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CUDA_TRY(g, cudaSetDevice(g->device));
+    LaunchShape s;
+    if (resolve_launch(g, precision, &s)) return VEGAS_EINVAL;
+    if (s.blocks != g->active_blocks) return VEGAS_EINVAL;
+    vegas::IterArgs a;
+    a.edges = g->d_edges;
+    a.partials = g->d_partials;
+    a.key0 = (uint32_t)(seed & 0xFFFFFFFFu);
+    a.key1 = (uint32_t)(seed >> 32);
+    a.iteration = iteration;
+    a.dim = g->dim;
+    a.n_bins = g->n_bins;
+    a.log_ct = ilog2(s.ct);
+    a.log_ch = ilog2(s.ch);
+    a.jac_scale = jac_scale_for(g, precision);
+    const uint64_t chunk = chunk_events ? chunk_events : count;
+    for (uint64_t done = 0; done < count; done += chunk) {
+        a.first_event = first_event + done;
+        a.count = (count - done < chunk) ? count - done : chunk;
+        cudaEvent_t e0 = nullptr, e1 = nullptr;
+        if (g->profiling) {
+            if (g->events_used + 2 > g->events.size()) {
+                cudaEvent_t n0, n1;
+                CUDA_TRY(g, cudaEventCreate(&n0));
+                CUDA_TRY(g, cudaEventCreate(&n1));
+                g->events.push_back(n0);
+                g->events.push_back(n1);
+            }
+            e0 = g->events[g->events_used];
+            e1 = g->events[g->events_used + 1];
+            g->events_used += 2;
+            CUDA_TRY(g, cudaEventRecord(e0, st));
+        }
+        CUDA_TRY(g, vegas::launch_iterate(fid, precision, a, g->derived[fid], s.blocks, s.threads, s.shmem, st));
+        if (g->profiling) CUDA_TRY(g, cudaEventRecord(e1, st));
+        g->iterate_launches++;
+        g->launches++;
+    }
+    return VEGAS_OK;
+}
+
+int vegas_reduce(vegas_grid* g, void* cuda_stream) {
+    if (!g || g->active_blocks <= 0) return VEGAS_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CUDA_TRY(g, cudaSetDevice(g->device));
+    const int ntot = 4 + g->dim * g->n_bins;
+    CUDA_TRY(g, vegas::launch_reduce(g->d_partials, g->active_blocks, ntot, g->d_totals, st));
+    g->launches++;
+    return VEGAS_OK;
+}
+
+int vegas_finalize(vegas_grid* g, uint64_t n_events_total, void* cuda_stream, double* I, double* sigma,
+                   double* hist_host) {
+    if (!g || n_events_total < 2) return VEGAS_EINVAL;
+    CUDA_TRY(g, cudaSetDevice(g->device));
+    return finish_iteration(g, n_events_total, (cudaStream_t)cuda_stream, I, sigma, hist_host);
+}
+
+void* vegas_totals_device(vegas_grid* g) { return g ? (void*)g->d_totals : nullptr; }
+size_t vegas_totals_count(const vegas_grid* g) { return g ? 4 + (size_t)g->dim * g->n_bins : 0; }
+
+int vegas_iterate(vegas_grid* g, uint64_t n_events, uint64_t chunk_events, uint64_t seed, uint32_t iteration,
+                  int fid, int precision, void* cuda_stream, double* I, double* sigma, double* hist_host) {
+    if (!check_call(g, fid, precision) || n_events < 2) return VEGAS_EINVAL;
+    int rc = vegas_begin_iteration(g, cuda_stream);
+    if (rc) return rc;
+    rc = vegas_accumulate(g, 0, n_events, chunk_events, seed, iteration, fid, precision, cuda_stream);
+    if (rc) return rc;
+    rc = vegas_reduce(g, cuda_stream);
+    if (rc) return rc;
+    return finish_iteration(g, n_events, (cudaStream_t)cuda_stream, I, sigma, hist_host);
+}
+
+int vegas_refine(vegas_grid* g, const double* hist_host, double alpha, void* cuda_stream) {
+    if (!g || !(alpha >= 0.0) || !std::isfinite(alpha)) return VEGAS_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CUDA_TRY(g, cudaSetDevice(g->device));
+    const double* hist = g->d_totals + 4;
+    if (hist_host) {
+        CUDA_TRY(g, cudaMemcpyAsync(g->d_hist_up, hist_host, sizeof(double) * g->dim * g->n_bins, cudaMemcpyHostToDevice, st));
+        hist = g->d_hist_up;
+    }
+    CUDA_TRY(g, cudaMemsetAsync(g->d_status, 0, sizeof(int), st));
+    CUDA_TRY(g, vegas::launch_refine(g->d_edges, hist, g->dim, g->n_bins, alpha, g->d_status, st));
+    g->launches++;
+    int status = 0;
+    CUDA_TRY(g, cudaMemcpyAsync(&status, g->d_status, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(g, cudaStreamSynchronize(st));
+    return status == 0 ? VEGAS_OK : VEGAS_ENUMERIC;
+}
+
+int vegas_combine(int n_iter, int n_skip, const double* I_k, const double* sigma_k, double* I, double* sigma,
+                  double* chi2_dof) {
+    if (n_iter < 1 || n_skip < 0 || n_skip >= n_iter || !I_k || !sigma_k || !I || !sigma || !chi2_dof)
+        return VEGAS_EINVAL;
+    const int K = n_iter - n_skip;
+    bool any_zero = false;
+    for (int k = n_skip; k < n_iter; ++k)
+        if (!(sigma_k[k] > 0.0)) any_zero = true;
+    if (any_zero) {
+        double acc = 0.0;
+        for (int k = n_skip; k < n_iter; ++k) acc += I_k[k];
+        *I = acc / K;
+        *sigma = 0.0;
+        *chi2_dof = 0.0;
+        return VEGAS_OK;
+    }
+    // weights relative to the smallest sigma keep 1/sigma^2 in range
+    double smin = sigma_k[n_skip];
+    for (int k = n_skip; k < n_iter; ++k) smin = std::fmin(smin, sigma_k[k]);
+    double W = 0.0, WI = 0.0;
+    for (int k = n_skip; k < n_iter; ++k) {
+        const double r = smin / sigma_k[k], w = r * r;
+        W += w;
+        WI += w * I_k[k];
+    }
+    const double mean = WI / W;
+    double chi2 = 0.0;
+    for (int k = n_skip; k < n_iter; ++k) {
+        const double dev = (I_k[k] - mean) / sigma_k[k];
+        chi2 += dev * dev;
+    }
+    *I = mean;
+    *sigma = smin / std::sqrt(W);
+    *chi2_dof = K > 1 ? chi2 / (K - 1) : 0.0;
+    return VEGAS_OK;
+}
+
+int vegas_integrate(vegas_grid* g, int n_iter, int n_skip, uint64_t n_events, uint64_t chunk_events, uint64_t seed,
+                    double alpha, int fid, int precision, void* cuda_stream, double* I, double* sigma,
+                    double* chi2_dof, double* per_iter_host) {
+    if (!check_call(g, fid, precision) || n_events < 2) return VEGAS_EINVAL;
+    if (n_iter < 1 || n_iter > kMaxIter || n_skip < 0 || n_skip >= n_iter || !I || !sigma || !chi2_dof)
+        return VEGAS_EINVAL;
+    if (alpha != alpha || std::isinf(alpha)) return VEGAS_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CUDA_TRY(g, cudaSetDevice(g->device));
+    CUDA_TRY(g, cudaMemsetAsync(g->d_status, 0, sizeof(int), st));
+    for (int k = 0; k < n_iter; ++k) {
+        int rc = vegas_begin_iteration(g, cuda_stream);
+        if (rc) return rc;
+        rc = vegas_accumulate(g, 0, n_events, chunk_events, seed, (uint32_t)k, fid, precision, cuda_stream);
+        if (rc) return rc;
+        rc = vegas_reduce(g, cuda_stream);
+        if (rc) return rc;
+        CUDA_TRY(g, vegas::launch_finalize(g->d_totals, (double)n_events, g->d_result + (size_t)kResultStride * k, st));
+        g->launches++;
+        if (alpha >= 0.0) {
+            CUDA_TRY(g, vegas::launch_refine(g->d_edges, g->d_totals + 4, g->dim, g->n_bins, alpha, g->d_status, st));
+            g->launches++;
+        }
+    }
+    std::vector<double> res((size_t)kResultStride * n_iter);
+    int status = 0;
+    CUDA_TRY(g, cudaMemcpyAsync(res.data(), g->d_result, sizeof(double) * res.size(), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(g, cudaMemcpyAsync(&status, g->d_status, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(g, cudaStreamSynchronize(st));
+    std::vector<double> Ik(n_iter), sk(n_iter);
+    int rc = status == 0 ? VEGAS_OK : VEGAS_ENUMERIC;
+    for (int k = 0; k < n_iter; ++k) {
+        Ik[k] = res[(size_t)kResultStride * k];
+        sk[k] = res[(size_t)kResultStride * k + 1];
+        if (res[(size_t)kResultStride * k + 2] != 0.0) rc = VEGAS_ENUMERIC;
+        if (per_iter_host) { per_iter_host[2 * k] = Ik[k]; per_iter_host[2 * k + 1] = sk[k]; }
+    }
+    const int rc2 = vegas_combine(n_iter, n_skip, Ik.data(), sk.data(), I, sigma, chi2_dof);
+    return rc2 ? rc2 : rc;
+}
+
+size_t vegas_debug_scratch_bytes(int dim, uint32_t count) {
+    if (dim < 1 || dim > VEGAS_MAX_DIM) return 0;
+    const size_t per_dim = (size_t)count * dim;
+    return align_up(per_dim * 4) + align_up(per_dim * 4) + align_up(per_dim * 8) + align_up((size_t)count * 8);
+}
+
+int vegas_debug_sample(vegas_grid* g, uint64_t first_event, uint32_t count, uint64_t seed, uint32_t iteration,
+                       int fid, int precision, void* dev_scratch, void* cuda_stream, uint32_t* words,
+                       int32_t* bins, double* x, double* fJ) {
+    if (!check_call(g, fid, precision) || !dev_scratch || count == 0) return VEGAS_EINVAL;
+    if (((uintptr_t)dev_scratch) % kAlign) return VEGAS_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CUDA_TRY(g, cudaSetDevice(g->device));
+    const size_t per_dim = (size_t)count * g->dim;
+    unsigned char* base = (unsigned char*)dev_scratch;
+    vegas::DebugArgs a;
+    a.edges = g->d_edges;
+    a.first_event = first_event;
+    a.count = count;
+    a.key0 = (uint32_t)(seed & 0xFFFFFFFFu);
+    a.key1 = (uint32_t)(seed >> 32);
+    a.iteration = iteration;
+    a.dim = g->dim;
+    a.n_bins = g->n_bins;
+    a.jac_scale = jac_scale_for(g, precision);
+    a.words = (uint32_t*)base;                 base += align_up(per_dim * 4);
+    a.bins = (int32_t*)base;                   base += align_up(per_dim * 4);
+    a.x = (double*)base;                       base += align_up(per_dim * 8);
+    a.fJ = (double*)base;
+    CUDA_TRY(g, vegas::launch_debug(fid, precision, a, g->derived[fid], st));
+    g->launches++;
+    if (words) CUDA_TRY(g, cudaMemcpyAsync(words, a.words, per_dim * 4, cudaMemcpyDeviceToHost, st));
+    if (bins) CUDA_TRY(g, cudaMemcpyAsync(bins, a.bins, per_dim * 4, cudaMemcpyDeviceToHost, st));
+    if (x) CUDA_TRY(g, cudaMemcpyAsync(x, a.x, per_dim * 8, cudaMemcpyDeviceToHost, st));
+    if (fJ) CUDA_TRY(g, cudaMemcpyAsync(fJ, a.fJ, (size_t)count * 8, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(g, cudaStreamSynchronize(st));
+    return VEGAS_OK;
+}
+
+int vegas_set_launch(vegas_grid* g, int blocks, int threads, int table_copies, int hist_copies) {
+    if (!g || blocks < 0 || threads < 0 || table_copies < 0 || hist_copies < 0) return VEGAS_EINVAL;
+    auto pow2 = [](int v) { return v == 0 || (v & (v - 1)) == 0; };
+    if (!pow2(table_copies) || !pow2(hist_copies) || table_copies > 32 || hist_copies > 32) return VEGAS_EINVAL;
+    vegas_grid trial = *g;
+    trial.events.clear();
+    trial.cfg_blocks = blocks;
+    trial.cfg_threads = threads;
+    trial.cfg_ct = table_copies;
+    trial.cfg_ch = hist_copies;
+    LaunchShape s;
+    if (resolve_launch(&trial, VEGAS_FP64, &s) || resolve_launch(&trial, VEGAS_FP32, &s)) return VEGAS_EINVAL;
+    g->cfg_blocks = blocks;
+    g->cfg_threads = threads;
+    g->cfg_ct = table_copies;
+    g->cfg_ch = hist_copies;
+    g->active_blocks = 0;
+    return VEGAS_OK;
+}
+
+int vegas_get_launch(vegas_grid* g, int precision, int* blocks, int* threads, int* table_copies, int* hist_copies,
+                     size_t* shared_bytes) {
+    if (!g || (precision != VEGAS_FP64 && precision != VEGAS_FP32)) return VEGAS_EINVAL;
+    LaunchShape s;
+    if (resolve_launch(g, precision, &s)) return VEGAS_EINVAL;
+    if (blocks) *blocks = s.blocks;
+    if (threads) *threads = s.threads;
+    if (table_copies) *table_copies = s.ct;
+    if (hist_copies) *hist_copies = s.ch;
+    if (shared_bytes) *shared_bytes = s.shmem;
+    return VEGAS_OK;
+}
+
+int vegas_set_profiling(vegas_grid* g, int on) {
+    if (!g) return VEGAS_EINVAL;
+    g->profiling = on != 0;
+    return VEGAS_OK;
+}
+
+int vegas_kernel_time_ms(vegas_grid* g, double* iterate_kernel_ms, uint64_t* iterate_launches) {
+    if (!g) return VEGAS_EINVAL;
+    CUDA_TRY(g, cudaSetDevice(g->device));
+    for (size_t i = 0; i + 1 < g->events_used; i += 2) {
+        CUDA_TRY(g, cudaEventSynchronize(g->events[i + 1]));
+        float ms = 0.f;
+        CUDA_TRY(g, cudaEventElapsedTime(&ms, g->events[i], g->events[i + 1]));
+        g->kernel_ms_acc += (double)ms;
+    }
+    g->events_used = 0;
+    if (iterate_kernel_ms) *iterate_kernel_ms = g->kernel_ms_acc;
+    if (iterate_launches) *iterate_launches = g->iterate_launches;
+    return VEGAS_OK;
+}
+
+uint64_t vegas_launch_count(const vegas_grid* g) { return g ? g->launches : 0; }
+
+int vegas_reset_counters(vegas_grid* g) {
+    if (!g) return VEGAS_EINVAL;
+    g->events_used = 0;
+    g->kernel_ms_acc = 0.0;
+    g->iterate_launches = 0;
+    g->launches = 0;
+    return VEGAS_OK;
+}
+
+const char* vegas_strerror(int code) {
+    switch (code) {
+    case VEGAS_OK: return "ok";
+    case VEGAS_EINVAL: return "invalid argument";
+    case VEGAS_ECUDA: return "CUDA runtime or launch failure (see vegas_last_cuda_error)";
+    case VEGAS_ENUMERIC: return "non-finite sums, or a histogram row without a finite positive sum in refine";
+    default: return "unknown error code";
+    }
+}
+
+const char* vegas_last_cuda_error(const vegas_grid* g) { return g ? g->cuda_err : ""; }
+
+const char* vegas_version(void) { return "vegas_b200 0.1 sm_100a"; }
+
+}  // extern "C"
+#pragma GCC visibility pop

@@ -1,0 +1,205 @@
+// vegas_device.cuh -- device functions shared by the fused iterate kernel (K1) and the parity
+// hook (K4): Philox4x32-10, word split, grid map, the built-in integrands, compensated sums.
+// sm_100a only.  Readings C1..C11 are those of DESIGN.md; citations are PAPER.md lines.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/vegas.h"
+
+namespace vegas {
+
+// ------------------------------------------------------------------------------------------
+// Integrand parameters as the kernels see them: derived on the host from the user's array
+// (vegas_api.cu: derive_params), passed by value as a __grid_constant__ so that every access is a
+// constant-bank read with a compile-time offset inside the unrolled dimension loop.
+//   GAUSS:  p[0] = (a sqrt(pi))^-d, p[1] = 1/a^2
+//   GENZ:   p[2j] = 1/c_j^2, p[2j+1] = w_j
+//   BW_POLY: p[0] = s_min, p[1] = s_max - s_min, p[2] = M^2, p[3] = M^2 G^2,
+//            p[4 + 5(i-1) + k] = a[i][k]
+// ------------------------------------------------------------------------------------------
+template <typename T>
+struct FParams {
+    T p[VEGAS_MAX_PARAMS];
+};
+
+// ------------------------------------------------------------------------------------------
+// C1: Philox4x32-10.  20 wide multiplies + 20 three-input XORs per block of 4 words; the key
+// schedule depends only on the seed, so ptxas keeps it on the uniform datapath.
+// ------------------------------------------------------------------------------------------
+struct PhiloxKey {
+    uint32_t k0[10], k1[10];
+};
+
+__device__ __forceinline__ PhiloxKey philox_key_schedule(uint32_t key0, uint32_t key1) {
+    PhiloxKey ks;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        ks.k0[r] = key0 + (uint32_t)r * 0x9E3779B9u;
+        ks.k1[r] = key1 + (uint32_t)r * 0xBB67AE85u;
+    }
+    return ks;
+}
+
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              const PhiloxKey& ks, uint32_t (&out)[4]) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ ks.k0[r];
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ ks.k1[r];
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// ------------------------------------------------------------------------------------------
+// C3: split a word into (bin, in-bin offset).  P = word * n_bins exactly; bin = P >> 32.
+// fp64: r = (lo + 1/2) 2^-32 exactly, built in the mantissa of a double in [1,2) and shifted down by
+//       one exact subtraction (I2F.F64.U32 runs at a quarter of the DADD rate on sm_100).
+// fp32 (C11): r32 = ((lo >> 8) + 1/2) 2^-24, within 2^-24 of the fp64 r; the kernel wants
+//       r/n_bins because its table stores n_bins*Delta (keeps the Jacobian product in range).
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void split_word(uint32_t word, uint32_t n_bins, uint32_t& bin, uint32_t& lo) {
+    const uint64_t P = (uint64_t)word * n_bins;
+    bin = (uint32_t)(P >> 32);
+    lo = (uint32_t)P;
+}
+
+__device__ __forceinline__ double offset_f64(uint32_t lo) {
+    const double m = __hiloint2double((int)(0x3FF00000u | (lo >> 12)), (int)((lo << 20) | 0x80000u));
+    return m - 1.0;
+}
+
+__device__ __forceinline__ float offset_f32_scaled(uint32_t lo, float inv_nb_2m24, float inv_nb_2m25) {
+    return fmaf((float)(lo >> 8), inv_nb_2m24, inv_nb_2m25);
+}
+
+// ------------------------------------------------------------------------------------------
+// C5: the built-in integrands in streaming form: begin(), one dim(j, x) call per dimension in
+// increasing j, finish() -> f(x).  Nothing of x is kept.
+// ------------------------------------------------------------------------------------------
+template <typename T> __device__ __forceinline__ T t_exp(T x);
+template <> __device__ __forceinline__ double t_exp<double>(double x) { return exp(x); }
+template <> __device__ __forceinline__ float t_exp<float>(float x) { return expf(x); }
+template <typename T> __device__ __forceinline__ T t_fma(T a, T b, T c);
+template <> __device__ __forceinline__ double t_fma<double>(double a, double b, double c) { return fma(a, b, c); }
+template <> __device__ __forceinline__ float t_fma<float>(float a, float b, float c) { return fmaf(a, b, c); }
+
+template <int FID, typename T>
+struct Integrand;
+
+template <typename T>
+struct Integrand<VEGAS_F_CONST, T> {
+    __device__ __forceinline__ void begin() {}
+    __device__ __forceinline__ void dim(int, T, const FParams<T>&) {}
+    __device__ __forceinline__ T finish(const FParams<T>&) const { return (T)1; }
+};
+
+template <typename T>
+struct Integrand<VEGAS_F_GAUSS, T> {   // PAPER.md:65 Eq.(1)
+    T s;
+    __device__ __forceinline__ void begin() { s = (T)0; }
+    __device__ __forceinline__ void dim(int, T x, const FParams<T>&) {
+        const T t = x - (T)0.5;
+        s = t_fma(t, t, s);
+    }
+    __device__ __forceinline__ T finish(const FParams<T>& fp) const { return fp.p[0] * t_exp<T>(-s * fp.p[1]); }
+};
+
+template <typename T>
+struct Integrand<VEGAS_F_GENZ_PRODUCT_PEAK, T> {   // PAPER.md:74 Eq.(3), N = 1
+    T prod;
+    __device__ __forceinline__ void begin() { prod = (T)1; }
+    __device__ __forceinline__ void dim(int j, T x, const FParams<T>& fp) {
+        const T t = x - fp.p[2 * j + 1];
+        prod *= t_fma(t, t, fp.p[2 * j]);
+    }
+    __device__ __forceinline__ T finish(const FParams<T>&) const { return (T)1 / prod; }
+};
+
+template <typename T>
+struct Integrand<VEGAS_F_BW_POLY, T> {   // BASELINE.json:configs[4], readings R11, R12
+    T bw, poly;
+    __device__ __forceinline__ void begin() { bw = (T)0; poly = (T)0; }
+    __device__ __forceinline__ void dim(int j, T x, const FParams<T>& fp) {
+        if (j == 0) {
+            const T ds = t_fma(x, fp.p[1], fp.p[0]) - fp.p[2];        // s - M^2
+            bw = fp.p[3] / t_fma(ds, ds, fp.p[3]);
+        } else {
+            const T* a = &fp.p[4 + 5 * (j - 1)];
+            T h = a[4];
+            h = t_fma(h, x, a[3]);
+            h = t_fma(h, x, a[2]);
+            h = t_fma(h, x, a[1]);
+            h = t_fma(h, x, a[0]);
+            poly += h;
+        }
+    }
+    __device__ __forceinline__ T finish(const FParams<T>&) const { return bw * poly; }
+};
+
+// ------------------------------------------------------------------------------------------
+// Compensated sums.  Per-thread Kahan accumulators (value s, compensation c; the sum is s - c),
+// merged as double-double (hi, lo) pairs, so that S1 and S2 are good to ~1e-30 relative and the
+// cancellation in S2/n - I^2 (reading C7) costs nothing even when sigma << I.
+// ------------------------------------------------------------------------------------------
+struct dd {
+    double hi, lo;
+};
+
+__device__ __forceinline__ void kahan_add(double& s, double& c, double v) {
+    const double y = __dsub_rn(v, c);
+    const double t = __dadd_rn(s, y);
+    c = __dsub_rn(__dsub_rn(t, s), y);
+    s = t;
+}
+
+__device__ __forceinline__ dd two_sum(double a, double b) {
+    const double s = __dadd_rn(a, b);
+    const double bb = __dsub_rn(s, a);
+    const double e = __dadd_rn(__dsub_rn(a, __dsub_rn(s, bb)), __dsub_rn(b, bb));
+    return dd{s, e};
+}
+
+__device__ __forceinline__ dd fast_two_sum(double a, double b) {   // |a| >= |b|
+    const double s = __dadd_rn(a, b);
+    return dd{s, __dsub_rn(b, __dsub_rn(s, a))};
+}
+
+__device__ __forceinline__ dd dd_add(dd x, dd y) {
+    dd s = two_sum(x.hi, y.hi);
+    s.lo = __dadd_rn(s.lo, __dadd_rn(x.lo, y.lo));
+    return fast_two_sum(s.hi, s.lo);
+}
+
+__device__ __forceinline__ dd dd_neg(dd x) { return dd{-x.hi, -x.lo}; }
+
+__device__ __forceinline__ dd dd_div_d(dd x, double n) {   // x / n
+    const double q1 = __ddiv_rn(x.hi, n);
+    const double r = __fma_rn(-q1, n, x.hi);                 // exact remainder
+    const double q2 = __ddiv_rn(__dadd_rn(r, x.lo), n);
+    return fast_two_sum(q1, q2);
+}
+
+__device__ __forceinline__ dd dd_sqr(dd x) {
+    const double p = __dmul_rn(x.hi, x.hi);
+    const double e = __fma_rn(x.hi, x.hi, -p);
+    return fast_two_sum(p, __fma_rn(2.0 * x.hi, x.lo, e));
+}
+
+__device__ __forceinline__ dd dd_shfl_xor(dd v, int mask) {
+    return dd{__shfl_xor_sync(0xffffffffu, v.hi, mask), __shfl_xor_sync(0xffffffffu, v.lo, mask)};
+}
+
+__device__ __forceinline__ dd dd_warp_sum(dd v) {
+#pragma unroll
+    for (int m = 16; m > 0; m >>= 1) v = dd_add(v, dd_shfl_xor(v, m));
+    return v;
+}
+
+}  // namespace vegas

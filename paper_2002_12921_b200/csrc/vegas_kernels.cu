@@ -1,0 +1,406 @@
+// vegas_kernels.cu -- the sm_100a kernels of the Vegas iteration library and their launchers.
+//   K1 k_iterate   fused RNG -> split -> grid map -> integrand -> S1, S2, histogram   (S1..S6)
+//   K2 k_reduce    deterministic second-level reduction over the per-CTA partials
+//      k_finalize  I = S1/n, sigma^2 = (S2/n - I^2)/(n-1) in double-double             (S7)
+//   K3 k_refine    smooth, normalise, compress with alpha, rebin; one CTA per dimension (S8)
+//   K4 k_debug     parity hook: words, bins, x, f*J of single events through K1's device functions
+// Step names S1..S9 are SURVEY.md 8(a); readings C1..C11 are DESIGN.md.
+#include "vegas_kernels.h"
+
+#include "vegas_device.cuh"
+
+namespace vegas {
+
+template <typename T> struct Vec2;
+template <> struct Vec2<double> { using type = double2; };
+template <> struct Vec2<float> { using type = float2; };
+
+// One grid-table entry from two master-grid edges (C4).  fp64: (X_b, Delta).  fp32 (C11):
+// (X_b, n_bins*Delta) rounded to fp32 -- the per-dimension Jacobian factor itself, so that the
+// running product stays O(1) instead of underflowing like prod Delta would in fp32.
+template <typename T>
+__device__ __forceinline__ typename Vec2<T>::type make_entry(double x0, double x1, int n_bins);
+template <>
+__device__ __forceinline__ double2 make_entry<double>(double x0, double x1, int) {
+    return make_double2(x0, x1 - x0);
+}
+template <>
+__device__ __forceinline__ float2 make_entry<float>(double x0, double x1, int n_bins) {
+    return make_float2((float)x0, (float)((double)n_bins * (x1 - x0)));
+}
+
+// x_j and the Jacobian factor from the table entry and the low product word (C3, C4).
+template <typename T> struct MapConst;
+template <> struct MapConst<double> {
+    __device__ __forceinline__ MapConst(int) {}
+    __device__ __forceinline__ double x(double2 ent, uint32_t lo) const {
+        return fma(ent.y, offset_f64(lo), ent.x);
+    }
+};
+template <> struct MapConst<float> {
+    float c24, c25;
+    __device__ __forceinline__ MapConst(int n_bins)
+        : c24(5.9604644775390625e-08f / (float)n_bins), c25(2.98023223876953125e-08f / (float)n_bins) {}
+    __device__ __forceinline__ float x(float2 ent, uint32_t lo) const {
+        return fmaf(ent.y, offset_f32_scaled(lo, c24, c25), ent.x);
+    }
+};
+
+// ---------------------------------------------------------------------------------------------
+// K1.  One thread = one event at a time, grid-stride over the launch's event range.
+// Shared memory: the grid table, `ct` bank-interleaved copies ([entry][copy], copy = lane mod ct),
+// then the histogram, `ch` bank-interleaved fp64 copies ([bin][copy], copy = lane mod ch), then the
+// block-reduction scratch.  The copies put the lanes of one shared-memory wavefront on different
+// banks whatever bins they drew.
+// NBLK = ceil(dim/4) Philox blocks per event, compile time so that the packed bin indices
+// (one byte per dimension) live in registers.
+// ---------------------------------------------------------------------------------------------
+template <int FID, typename T, int NBLK>
+__global__ void __launch_bounds__(kIterMaxThreads, 1)
+k_iterate(const IterArgs a, const __grid_constant__ FParams<T> fp) {
+    using T2 = typename Vec2<T>::type;
+    extern __shared__ __align__(16) unsigned char smem[];
+    const int dim = a.dim, nb = a.n_bins, nent = dim * nb;
+    const int ct = 1 << a.log_ct, ch = 1 << a.log_ch;
+    const uint32_t table_bytes = (uint32_t)(sizeof(T2) * nent * ct);
+    T2* table = reinterpret_cast<T2*>(smem);
+    double* hist = reinterpret_cast<double*>(smem + table_bytes);
+    dd* red = reinterpret_cast<dd*>(smem + table_bytes + (uint32_t)(8 * nent * ch));
+
+    for (int i = threadIdx.x; i < nent; i += blockDim.x) {
+        const int j = i / nb, b = i - j * nb;
+        const double* X = a.edges + (size_t)j * (nb + 1);
+        const T2 ent = make_entry<T>(X[b], X[b + 1], nb);
+        for (int c = 0; c < ct; ++c) table[i * ct + c] = ent;
+    }
+    for (int i = threadIdx.x; i < nent * ch; i += blockDim.x) hist[i] = 0.0;
+    __syncthreads();
+
+    const int lane = threadIdx.x & 31;
+    const unsigned char* tlane = smem + (uint32_t)(lane & (ct - 1)) * (uint32_t)sizeof(T2);
+    const uint32_t tstride = (uint32_t)sizeof(T2) << a.log_ct;       // bytes per table entry row
+    double* hlane = hist + (lane & (ch - 1));
+    const PhiloxKey ks = philox_key_schedule(a.key0, a.key1);
+    const MapConst<T> mapc(nb);
+    const double jac_scale = a.jac_scale;
+
+    double s1 = 0.0, c1 = 0.0, s2 = 0.0, c2 = 0.0;
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long q = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; q < a.count;
+         q += stride) {
+        const unsigned long long e = a.first_event + q;
+        const uint32_t e_lo = (uint32_t)e, e_hi = (uint32_t)(e >> 32);
+        Integrand<FID, T> f;
+        f.begin();
+        T jac = (T)1;
+        uint32_t packed[NBLK];
+#pragma unroll
+        for (int blk = 0; blk < NBLK; ++blk) {
+            uint32_t w[4];
+            philox4x32_10((uint32_t)blk, a.iteration, e_lo, e_hi, ks, w);
+            uint32_t pk = 0;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int j = 4 * blk + i;
+                if (j < dim) {
+                    uint32_t b, lo;
+                    split_word(w[i], (uint32_t)nb, b, lo);
+                    const T2 ent = *reinterpret_cast<const T2*>(tlane + ((uint32_t)(j * nb) + b) * tstride);
+                    const T x = mapc.x(ent, lo);
+                    jac *= ent.y;
+                    f.dim(j, x, fp);
+                    pk |= b << (8 * i);
+                }
+            }
+            packed[blk] = pk;
+        }
+        const double v = (double)(f.finish(fp) * jac) * jac_scale;
+        const double v2 = v * v;
+        kahan_add(s1, c1, v);
+        kahan_add(s2, c2, v2);
+#pragma unroll
+        for (int blk = 0; blk < NBLK; ++blk) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int j = 4 * blk + i;
+                if (j < dim) {
+                    const uint32_t b = (packed[blk] >> (8 * i)) & 0xFFu;
+                    atomicAdd(hlane + (((uint32_t)(j * nb) + b) << a.log_ch), v2);
+                }
+            }
+        }
+    }
+
+    // S5: warp shuffle -> CTA -> this CTA's partial (accumulated over the launches of an iteration)
+    dd t1 = dd_warp_sum(fast_two_sum(s1, -c1));
+    dd t2 = dd_warp_sum(fast_two_sum(s2, -c2));
+    const int warp = threadIdx.x >> 5, nwarps = (blockDim.x + 31) >> 5;
+    if (lane == 0) { red[2 * warp] = t1; red[2 * warp + 1] = t2; }
+    __syncthreads();
+    double* part = a.partials + (size_t)blockIdx.x * (4 + nent);
+    if (warp == 0) {
+        t1 = (lane < nwarps) ? red[2 * lane] : dd{0.0, 0.0};
+        t2 = (lane < nwarps) ? red[2 * lane + 1] : dd{0.0, 0.0};
+        t1 = dd_warp_sum(t1);
+        t2 = dd_warp_sum(t2);
+        if (lane == 0) {
+            t1 = dd_add(t1, dd{part[0], part[1]});
+            t2 = dd_add(t2, dd{part[2], part[3]});
+            part[0] = t1.hi; part[1] = t1.lo; part[2] = t2.hi; part[3] = t2.lo;
+        }
+    }
+    // S6: merge the copies in fixed order, one coalesced pass per CTA
+    for (int i = threadIdx.x; i < nent; i += blockDim.x) {
+        double h = 0.0;
+        for (int c = 0; c < ch; ++c) h += hist[i * ch + c];
+        part[4 + i] += h;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// K2: totals[i] = sum over CTAs, in CTA order, of partials[cta][i]  (i >= 4: histogram, plain fp64;
+// i < 4: the two double-double sums, merged by one thread).
+// ---------------------------------------------------------------------------------------------
+__global__ void k_reduce(const double* __restrict__ partials, int n_parts, int n_tot, double* __restrict__ totals) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_tot) return;
+    if (i >= 4) {
+        double h = 0.0;
+        for (int p = 0; p < n_parts; ++p) h += partials[(size_t)p * n_tot + i];
+        totals[i] = h;
+    } else if (i == 0 || i == 2) {
+        dd s{0.0, 0.0};
+        for (int p = 0; p < n_parts; ++p)
+            s = dd_add(s, dd{partials[(size_t)p * n_tot + i], partials[(size_t)p * n_tot + i + 1]});
+        totals[i] = s.hi;
+        totals[i + 1] = s.lo;
+    }
+}
+
+// S7 (C7): I = S1/n; Var = (S2/n - I^2)/(n-1); sigma = sqrt(max(Var, 0)).
+// result = { I, sigma, status } (status 0 or VEGAS_ENUMERIC as a double).
+__global__ void k_finalize(const double* __restrict__ totals, double n, double* __restrict__ result) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const dd S1 = fast_two_sum(totals[0], totals[1]);
+    const dd S2 = fast_two_sum(totals[2], totals[3]);
+    const dd mean = dd_div_d(S1, n);
+    const dd ex2 = dd_div_d(S2, n);
+    const dd diff = dd_add(ex2, dd_neg(dd_sqr(mean)));
+    const dd var = dd_div_d(diff, n - 1.0);
+    const double v = var.hi + var.lo;
+    const double I = mean.hi + mean.lo;
+    const double sigma = (v > 0.0) ? sqrt(v) : ((v != v) ? v : 0.0);
+    result[0] = I;
+    result[1] = sigma;
+    result[2] = (isfinite(I) && isfinite(sigma) && isfinite(S2.hi)) ? 0.0 : (double)VEGAS_ENUMERIC;
+}
+
+// ---------------------------------------------------------------------------------------------
+// K3 (C8): one CTA per dimension, one thread per bin.  The two running sums that decide where the
+// new edges fall (sum of s_i, cumulative sum of m_i) are formed by thread 0 in index order, i.e. in
+// the order the method states them, so the walk "advance while C + m_i < t" sees the same doubles
+// whichever thread evaluates it.
+// status[0] is set to VEGAS_ENUMERIC if a dimension has no finite positive smoothed sum.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(VEGAS_MAX_BINS)
+k_refine(double* __restrict__ edges, const double* __restrict__ hist, int n_bins, double alpha, int* status) {
+    __shared__ double X[VEGAS_MAX_BINS + 1], m[VEGAS_MAX_BINS], cum[VEGAS_MAX_BINS + 1], s[VEGAS_MAX_BINS];
+    __shared__ double total_s;
+    const int j = blockIdx.x, nb = n_bins, i = threadIdx.x;
+    double* Xg = edges + (size_t)j * (nb + 1);
+    const double* h = hist + (size_t)j * nb;
+    if (i < nb) {
+        X[i] = Xg[i];
+        if (i == 0) X[nb] = Xg[nb];
+        double si;
+        if (i == 0) si = (h[0] + h[1]) / 2.0;
+        else if (i == nb - 1) si = (h[nb - 2] + h[nb - 1]) / 2.0;
+        else si = (h[i - 1] + h[i] + h[i + 1]) / 3.0;
+        s[i] = si;
+    }
+    __syncthreads();
+    if (i == 0) {
+        double t = 0.0;
+        for (int k = 0; k < nb; ++k) t += s[k];
+        total_s = t;
+    }
+    __syncthreads();
+    const double total = total_s;
+    if (!(total > 0.0) || !isfinite(total)) {
+        if (i == 0) *status = VEGAS_ENUMERIC;
+        return;   // whole CTA: this dimension keeps its grid
+    }
+    if (i < nb) {
+        const double p = s[i] / total;
+        double mi;
+        if (p <= 0.0) mi = 0.0;
+        else if (p >= 1.0) mi = 1.0;
+        else mi = pow((1.0 - p) / log(1.0 / p), alpha);
+        m[i] = mi;
+    }
+    __syncthreads();
+    if (i == 0) {
+        double c = 0.0;
+        cum[0] = 0.0;
+        for (int k = 0; k < nb; ++k) { c += m[k]; cum[k + 1] = c; }
+    }
+    __syncthreads();
+    if (i >= 1 && i < nb) {
+        const double delta = cum[nb] / (double)nb;
+        const double t = (double)i * delta;
+        int k = 0;
+        while (k < nb - 1 && cum[k + 1] < t) ++k;        // cum[k+1] == C + m_k of the sequential walk
+        double frac = (m[k] > 0.0) ? (t - cum[k]) / m[k] : 0.0;
+        frac = fmin(fmax(frac, 0.0), 1.0);
+        Xg[i] = X[k] + frac * (X[k + 1] - X[k]);
+    }
+    if (i == 0) { Xg[0] = 0.0; Xg[nb] = 1.0; }
+}
+
+// ---------------------------------------------------------------------------------------------
+// K4: one thread per event, generic in dim; same device functions as K1.
+// ---------------------------------------------------------------------------------------------
+template <int FID, typename T>
+__global__ void k_debug(const DebugArgs a, const __grid_constant__ FParams<T> fp) {
+    using T2 = typename Vec2<T>::type;
+    const uint32_t q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= a.count) return;
+    const unsigned long long e = a.first_event + q;
+    const int dim = a.dim, nb = a.n_bins;
+    const PhiloxKey ks = philox_key_schedule(a.key0, a.key1);
+    const MapConst<T> mapc(nb);
+    Integrand<FID, T> f;
+    f.begin();
+    T jac = (T)1;
+    uint32_t w[4] = {0, 0, 0, 0};
+    for (int j = 0; j < dim; ++j) {
+        if ((j & 3) == 0) philox4x32_10((uint32_t)(j >> 2), a.iteration, (uint32_t)e, (uint32_t)(e >> 32), ks, w);
+        const uint32_t word = (j & 3) == 0 ? w[0] : (j & 3) == 1 ? w[1] : (j & 3) == 2 ? w[2] : w[3];
+        uint32_t b, lo;
+        split_word(word, (uint32_t)nb, b, lo);
+        const double* X = a.edges + (size_t)j * (nb + 1);
+        const T2 ent = make_entry<T>(X[b], X[b + 1], nb);
+        const T x = mapc.x(ent, lo);
+        jac *= ent.y;
+        f.dim(j, x, fp);
+        a.words[(size_t)q * dim + j] = word;
+        a.bins[(size_t)q * dim + j] = (int32_t)b;
+        a.x[(size_t)q * dim + j] = (double)x;
+    }
+    a.fJ[q] = (double)(f.finish(fp) * jac) * a.jac_scale;
+}
+
+// =============================================================================================
+// Launchers
+// =============================================================================================
+template <int FID, typename T, int NBLK>
+static cudaError_t launch_iterate_t(const IterArgs& a, const FParams<T>& fp, int blocks, int threads,
+                                    size_t shmem, cudaStream_t st) {
+    auto kern = k_iterate<FID, T, NBLK>;
+    static size_t configured = 0;   // per instantiation; attribute is sticky per context
+    if (shmem > configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem);
+        if (e != cudaSuccess) return e;
+        configured = shmem;
+    }
+    kern<<<blocks, threads, shmem, st>>>(a, fp);
+    return cudaGetLastError();
+}
+
+template <int FID, typename T>
+static cudaError_t launch_iterate_nblk(const IterArgs& a, const FParams<T>& fp, int blocks, int threads,
+                                       size_t shmem, cudaStream_t st) {
+    switch ((a.dim + 3) / 4) {
+    case 1: return launch_iterate_t<FID, T, 1>(a, fp, blocks, threads, shmem, st);
+    case 2: return launch_iterate_t<FID, T, 2>(a, fp, blocks, threads, shmem, st);
+    case 3: return launch_iterate_t<FID, T, 3>(a, fp, blocks, threads, shmem, st);
+    case 4: return launch_iterate_t<FID, T, 4>(a, fp, blocks, threads, shmem, st);
+    case 5: return launch_iterate_t<FID, T, 5>(a, fp, blocks, threads, shmem, st);
+    case 6: return launch_iterate_t<FID, T, 6>(a, fp, blocks, threads, shmem, st);
+    case 7: return launch_iterate_t<FID, T, 7>(a, fp, blocks, threads, shmem, st);
+    case 8: return launch_iterate_t<FID, T, 8>(a, fp, blocks, threads, shmem, st);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+template <typename T>
+static cudaError_t launch_iterate_fid(int fid, const IterArgs& a, const FParams<T>& fp, int blocks,
+                                      int threads, size_t shmem, cudaStream_t st) {
+    switch (fid) {
+    case VEGAS_F_CONST: return launch_iterate_nblk<VEGAS_F_CONST, T>(a, fp, blocks, threads, shmem, st);
+    case VEGAS_F_GAUSS: return launch_iterate_nblk<VEGAS_F_GAUSS, T>(a, fp, blocks, threads, shmem, st);
+    case VEGAS_F_GENZ_PRODUCT_PEAK:
+        return launch_iterate_nblk<VEGAS_F_GENZ_PRODUCT_PEAK, T>(a, fp, blocks, threads, shmem, st);
+    case VEGAS_F_BW_POLY: return launch_iterate_nblk<VEGAS_F_BW_POLY, T>(a, fp, blocks, threads, shmem, st);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+template <typename T>
+static void convert_params(const double* src, FParams<T>& dst) {
+    for (int i = 0; i < VEGAS_MAX_PARAMS; ++i) dst.p[i] = (T)src[i];
+}
+
+cudaError_t launch_iterate(int fid, int precision, const IterArgs& a, const double* derived_params,
+                           int blocks, int threads, size_t shmem, cudaStream_t st) {
+    if (precision == VEGAS_FP64) {
+        FParams<double> fp;
+        convert_params(derived_params, fp);
+        return launch_iterate_fid<double>(fid, a, fp, blocks, threads, shmem, st);
+    }
+    FParams<float> fp;
+    convert_params(derived_params, fp);
+    return launch_iterate_fid<float>(fid, a, fp, blocks, threads, shmem, st);
+}
+
+size_t iterate_shared_bytes(int dim, int n_bins, int precision, int table_copies, int hist_copies) {
+    const size_t nent = (size_t)dim * n_bins;
+    const size_t entry = precision == VEGAS_FP64 ? 16 : 8;
+    return entry * nent * table_copies + 8 * nent * hist_copies + 2 * sizeof(dd) * (kIterMaxThreads / 32);
+}
+
+cudaError_t launch_reduce(const double* partials, int n_parts, int n_tot, double* totals, cudaStream_t st) {
+    const int threads = 128;
+    k_reduce<<<(n_tot + threads - 1) / threads, threads, 0, st>>>(partials, n_parts, n_tot, totals);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_finalize(const double* totals, double n_events, double* result, cudaStream_t st) {
+    k_finalize<<<1, 32, 0, st>>>(totals, n_events, result);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_refine(double* edges, const double* hist, int dim, int n_bins, double alpha, int* status,
+                          cudaStream_t st) {
+    const int threads = ((n_bins + 31) / 32) * 32;
+    k_refine<<<dim, threads, 0, st>>>(edges, hist, n_bins, alpha, status);
+    return cudaGetLastError();
+}
+
+template <typename T>
+static cudaError_t launch_debug_t(int fid, const DebugArgs& a, const FParams<T>& fp, cudaStream_t st) {
+    const int threads = 128;
+    const int blocks = (int)((a.count + threads - 1) / threads);
+    switch (fid) {
+    case VEGAS_F_CONST: k_debug<VEGAS_F_CONST, T><<<blocks, threads, 0, st>>>(a, fp); break;
+    case VEGAS_F_GAUSS: k_debug<VEGAS_F_GAUSS, T><<<blocks, threads, 0, st>>>(a, fp); break;
+    case VEGAS_F_GENZ_PRODUCT_PEAK: k_debug<VEGAS_F_GENZ_PRODUCT_PEAK, T><<<blocks, threads, 0, st>>>(a, fp); break;
+    case VEGAS_F_BW_POLY: k_debug<VEGAS_F_BW_POLY, T><<<blocks, threads, 0, st>>>(a, fp); break;
+    default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_debug(int fid, int precision, const DebugArgs& a, const double* derived_params,
+                         cudaStream_t st) {
+    if (precision == VEGAS_FP64) {
+        FParams<double> fp;
+        convert_params(derived_params, fp);
+        return launch_debug_t<double>(fid, a, fp, st);
+    }
+    FParams<float> fp;
+    convert_params(derived_params, fp);
+    return launch_debug_t<float>(fid, a, fp, st);
+}
+
+}  // namespace vegas

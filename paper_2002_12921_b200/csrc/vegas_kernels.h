@@ -1,0 +1,49 @@
+// vegas_kernels.h -- host-visible launchers of the sm_100a kernels (vegas_kernels.cu).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/vegas.h"
+
+namespace vegas {
+
+constexpr int kIterMaxThreads = 512;   // __launch_bounds__ of K1: up to 128 registers per thread
+
+struct IterArgs {
+    const double* edges;            // device, [dim][n_bins+1] master grid
+    double* partials;               // device, [blocks][4 + dim*n_bins]
+    unsigned long long first_event; // global index of the first event of this launch (C2)
+    unsigned long long count;       // events in this launch
+    uint32_t key0, key1;            // seed lo, seed hi
+    uint32_t iteration;
+    int dim, n_bins;
+    int log_ct, log_ch;             // log2 of the table / histogram copy counts
+    double jac_scale;               // fp64: n_bins^dim (the table holds Delta); fp32: 1
+};
+
+struct DebugArgs {
+    const double* edges;
+    unsigned long long first_event;
+    uint32_t count;
+    uint32_t key0, key1, iteration;
+    int dim, n_bins;
+    double jac_scale;
+    uint32_t* words;
+    int32_t* bins;
+    double* x;
+    double* fJ;
+};
+
+size_t iterate_shared_bytes(int dim, int n_bins, int precision, int table_copies, int hist_copies);
+
+cudaError_t launch_iterate(int fid, int precision, const IterArgs& a, const double* derived_params,
+                           int blocks, int threads, size_t shmem, cudaStream_t st);
+cudaError_t launch_reduce(const double* partials, int n_parts, int n_tot, double* totals, cudaStream_t st);
+cudaError_t launch_finalize(const double* totals, double n_events, double* result, cudaStream_t st);
+cudaError_t launch_refine(double* edges, const double* hist, int dim, int n_bins, double alpha, int* status,
+                          cudaStream_t st);
+cudaError_t launch_debug(int fid, int precision, const DebugArgs& a, const double* derived_params,
+                         cudaStream_t st);
+
+}  // namespace vegas

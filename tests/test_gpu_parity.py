@@ -1,0 +1,434 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Protocol P1..P7 of DESIGN.md.  Tolerances (north_star): Philox words and bin
+indices bit-exact; I, sigma, H <= 1e-10 relative in fp64; fp32 path <= 1e-5 relative against the
+fp64 oracle (H in per-dimension max-norm, finding F3); refined edges <= 1e-10 absolute."""
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import oracle as O
+from paper_2002_12921_b200 import workloads as W
+
+THREADS = os.cpu_count() or 8
+RTOL64 = 1e-10
+RTOL32 = 1e-5
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
+    from paper_2002_12921_b200 import binding
+    return binding
+
+
+def _grid(B, w, edges=None):
+    g = B.VegasGrid(w.dim, w.n_bins)
+    g.set_params(w.integrand_id, w.params)
+    if edges is not None:
+        g.set_edges(edges)
+    return g
+
+
+def _assert_hist(h_gpu, h_ref, precision):
+    if precision == 64:
+        np.testing.assert_allclose(h_gpu, h_ref, rtol=RTOL64, atol=0)
+        assert np.all(h_gpu[h_ref == 0] == 0)
+    else:
+        # H accumulates v^2: a relative error eps on the fp32 v is 2 eps on its square (reading R20)
+        scale = h_ref.max(axis=1, keepdims=True)
+        assert np.all(np.abs(h_gpu - h_ref) <= 2 * RTOL32 * scale)
+
+
+# parity-sized versions of the five configs: several CTAs x several grid-stride passes and a ragged tail
+SMALL = {
+    1: dict(n_events=100_000, n_iter=5),               # cfg1 is already oracle-sized: full size
+    2: dict(n_events=1_000_003, n_iter=4),
+    3: dict(n_events=500_009, n_iter=4),
+    4: dict(n_events=300_007, n_iter=4),
+    5: dict(n_events=1_000_003, n_iter=4, chunk_events=250_000),
+}
+
+
+def _small(i):
+    return W.config(i).scaled(**SMALL[i])
+
+
+@pytest.fixture(scope="module")
+def chains():
+    """Oracle free-running chains of the parity-sized configs (grid_k, H_k, I_k, sigma_k)."""
+    out = {}
+    for i in range(1, 6):
+        w = _small(i)
+        out[i] = O.integrate(w.dim, w.n_bins, w.n_iter, w.n_events, w.seed, w.alpha, w.integrand_id, w.params,
+                             threads=THREADS)
+    return out
+
+
+# ------------------------------------------------------------------ P1, P2: words and bins, bit-exact
+@pytest.mark.parametrize("cfg,precision", [(1, 64), (3, 64), (3, 32), (4, 64), (4, 32), (5, 64)])
+def test_p1_p2_words_and_bins_bit_exact(B, cfg, precision):
+    w = W.config(cfg)
+    edges = W.adapted_edges(w.dim, w.n_bins, seed=cfg)
+    g = _grid(B, w, edges)
+    count = 60_000                                   # x dim >= 240k..1.2M (event, dim) pairs per range
+    for first, it in ((0, 0), (123_456_789, 7), ((1 << 32) - 1000, 1), ((5 << 32) + 17, 0xFFFFFFFE)):
+        gw, gb, gx, gf = g.debug_sample(first, count, w.seed, it, w.integrand_id, precision)
+        ow, ob, ox, of = O.sample(edges, w.seed, it, first, count, w.integrand_id, w.params)
+        assert np.array_equal(gw, ow)
+        assert np.array_equal(gb, ob)
+        if precision == 64:
+            np.testing.assert_allclose(gx, ox, rtol=5e-16, atol=0)
+            np.testing.assert_allclose(gf, of, rtol=1e-12, atol=0)
+        else:
+            np.testing.assert_allclose(gx, ox, rtol=0, atol=1.5e-7)
+            rel = np.abs(gf - of) / np.maximum(np.abs(of), 1e-300)
+            big = of > 1e-6 * of.max()
+            assert np.median(rel[big]) < 2e-6 and rel[big].max() < 1e-3
+    g.close()
+
+
+# ------------------------------------------------------------------ P3: teacher-forced iterations
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_p3_iterate_on_oracle_grids_fp64(B, chains, cfg):
+    w, ch = _small(cfg), chains[cfg]
+    g = _grid(B, w)
+    for k in range(w.n_iter):
+        g.set_edges(ch["edges_trace"][k])
+        I, s, H, st = g.iterate(w.n_events, w.seed, k, w.integrand_id, 64, chunk_events=w.chunk_events)
+        assert st == 0
+        assert I == pytest.approx(ch["per_iter"][k, 0], rel=RTOL64)
+        assert s == pytest.approx(ch["per_iter"][k, 1], rel=RTOL64)
+        _assert_hist(H, ch["hist_trace"][k], 64)
+        np.testing.assert_array_equal(g.get_hist(), H)
+    g.close()
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_p3_iterate_on_oracle_grids_fp32(B, chains, cfg):
+    w, ch = _small(cfg), chains[cfg]
+    g = _grid(B, w)
+    for k in range(w.n_iter):
+        g.set_edges(ch["edges_trace"][k])
+        I, s, H, st = g.iterate(w.n_events, w.seed, k, w.integrand_id, 32, chunk_events=w.chunk_events)
+        assert st == 0
+        assert I == pytest.approx(ch["per_iter"][k, 0], rel=RTOL32)
+        assert s == pytest.approx(ch["per_iter"][k, 1], rel=RTOL32)
+        _assert_hist(H, ch["hist_trace"][k], 32)
+    g.close()
+
+
+# ------------------------------------------------------------------ P4: refine on the oracle's histograms
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_p4_refine_on_oracle_histograms(B, chains, cfg):
+    w, ch = _small(cfg), chains[cfg]
+    g = _grid(B, w)
+    for k in range(w.n_iter):
+        g.set_edges(ch["edges_trace"][k])
+        assert g.refine(w.alpha, hist=ch["hist_trace"][k]) == 0
+        new = g.get_edges()
+        want = ch["edges_trace"][k + 1] if k + 1 < w.n_iter else ch["edges"]
+        np.testing.assert_allclose(new, want, rtol=0, atol=1e-10)
+        assert np.all(new[:, 0] == 0.0) and np.all(new[:, -1] == 1.0)
+        assert np.all(np.diff(new, axis=1) > 0)
+    g.close()
+
+
+def test_p4_refine_pins_hold_on_the_gpu_too(B):
+    rng = np.random.default_rng(5)
+    for dim, nb, alpha in ((3, 50, 1.5), (2, 100, 0.7), (1, 2, 1.5), (4, 256, 2.0), (32, 7, 1.0)):
+        g = B.VegasGrid(dim, nb)
+        edges = W.adapted_edges(dim, nb, seed=nb + dim)
+        hist = rng.random((dim, nb)) ** 5 * 10.0 ** rng.integers(-40, 40, size=(dim, 1))
+        if nb > 8:
+            hist[0, 2:6] = 0.0
+        g.set_edges(edges)
+        assert g.refine(alpha, hist=hist) == 0
+        want, rc = O.refine(edges, hist, alpha)
+        assert rc == 0
+        np.testing.assert_allclose(g.get_edges(), want, rtol=0, atol=1e-12)
+        # alpha = 0 leaves any grid unchanged; a constant histogram leaves the uniform grid unchanged
+        g.set_edges(edges)
+        assert g.refine(0.0, hist=hist + 1e-300) == 0
+        np.testing.assert_allclose(g.get_edges(), edges, rtol=0, atol=1e-14)
+        g.set_edges(O.uniform_edges(dim, nb))
+        assert g.refine(1.5, hist=np.full((dim, nb), 2.5)) == 0
+        np.testing.assert_allclose(g.get_edges(), O.uniform_edges(dim, nb), rtol=0, atol=1e-14)
+        g.close()
+
+
+def test_p4_refine_degenerate_row(B):
+    g = B.VegasGrid(3, 10)
+    edges = W.adapted_edges(3, 10, seed=3)
+    g.set_edges(edges)
+    hist = np.ones((3, 10))
+    hist[1] = 0.0
+    assert g.refine(1.5, hist=hist) == B.VEGAS_ENUMERIC
+    new = g.get_edges()
+    want, rc = O.refine(edges, hist, 1.5)
+    assert rc == O.ENUMERIC
+    np.testing.assert_array_equal(new[1], edges[1])
+    np.testing.assert_allclose(new, want, rtol=0, atol=1e-12)
+    g.close()
+
+
+# ------------------------------------------------------------------ P5: free-running chains
+@pytest.mark.parametrize("cfg,precision", [(1, 64), (2, 64), (3, 64), (4, 64), (5, 64), (1, 32), (3, 32), (4, 32)])
+def test_p5_free_running_integrate(B, chains, cfg, precision):
+    w, ch = _small(cfg), chains[cfg]
+    g = _grid(B, w)
+    r = g.integrate(w.n_iter, w.n_events, w.seed, w.alpha, w.integrand_id, precision, n_skip=0,
+                    chunk_events=w.chunk_events)
+    assert r["status"] == 0
+    oI, oS, oC = O.combine(ch["per_iter"][:, 0], ch["per_iter"][:, 1], 0)
+    if precision == 64:
+        np.testing.assert_allclose(r["per_iter"][:, 0], ch["per_iter"][:, 0], rtol=1e-8)
+        np.testing.assert_allclose(r["per_iter"][:, 1], ch["per_iter"][:, 1], rtol=1e-7)
+        assert r["I"] == pytest.approx(oI, rel=1e-8) and r["sigma"] == pytest.approx(oS, rel=1e-7)
+        np.testing.assert_allclose(g.get_edges(), ch["edges"], rtol=0, atol=1e-8)
+    else:
+        # finding F3: a free-running fp32 chain feeds its own rounding back through the grid, so only
+        # iteration 0 (identical grid) is held to 1e-5; later iterations and the average must agree
+        # with the oracle's to a small fraction of their own statistical error.
+        assert r["per_iter"][0, 0] == pytest.approx(ch["per_iter"][0, 0], rel=RTOL32)
+        for k in range(w.n_iter):
+            tol = max(RTOL32 * abs(ch["per_iter"][k, 0]), 0.05 * ch["per_iter"][k, 1])
+            assert abs(r["per_iter"][k, 0] - ch["per_iter"][k, 0]) <= tol
+        assert abs(r["I"] - oI) <= max(RTOL32 * abs(oI), 0.05 * oS)
+    g.close()
+
+
+# ------------------------------------------------------------------ P6: chunking, launch shapes, sharding
+def test_p6_chunked_equals_single_launch(B):
+    w = _small(3)
+    edges = W.adapted_edges(w.dim, w.n_bins, seed=33)
+    g = _grid(B, w, edges)
+    ref = g.iterate(w.n_events, w.seed, 2, w.integrand_id, 64)
+    for chunk in (w.n_events // 2 + 1, 100_000, 77_777, 1):
+        if chunk == 1:
+            n = 300                                   # 300 launches of one event each
+            a = g.iterate(n, w.seed, 2, w.integrand_id, 64)
+            b = g.iterate(n, w.seed, 2, w.integrand_id, 64, chunk_events=1)
+        else:
+            a, b = ref, g.iterate(w.n_events, w.seed, 2, w.integrand_id, 64, chunk_events=chunk)
+        assert b[0] == pytest.approx(a[0], rel=1e-12) and b[1] == pytest.approx(a[1], rel=1e-12)
+        np.testing.assert_allclose(b[2], a[2], rtol=1e-12)
+    g.close()
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_p6_launch_shapes_give_the_same_iteration(B, precision):
+    w = _small(4)
+    edges = W.adapted_edges(w.dim, w.n_bins, seed=44)
+    oI, oS, oH = O.iterate(edges, w.n_events, w.seed, 1, w.integrand_id, w.params, threads=THREADS)
+    g = _grid(B, w, edges)
+    shapes = [(0, 0, 0, 0), (1, 32, 1, 1), (7, 96, 2, 4), (148, 256, 1, 16), (296, 512, 4, 2), (1024, 64, 1, 1),
+              (37, 512, 2, 8)]
+    for blocks, threads, ct, ch in shapes:
+        g.set_launch(blocks, threads, ct, ch)
+        I, s, H, st = g.iterate(w.n_events, w.seed, 1, w.integrand_id, precision)
+        tol = RTOL64 if precision == 64 else RTOL32
+        assert st == 0 and I == pytest.approx(oI, rel=tol) and s == pytest.approx(oS, rel=tol)
+        _assert_hist(H, oH, precision)
+    g.close()
+
+
+def test_p6_event_range_sharding_matches_whole_iteration(B):
+    """The multi-GPU decomposition (begin / accumulate ranges / reduce / finalize) on one GPU."""
+    w = _small(5)
+    edges = W.adapted_edges(w.dim, w.n_bins, seed=55)
+    g = _grid(B, w, edges)
+    whole = g.iterate(w.n_events, w.seed, 3, w.integrand_id, 64)
+    g.begin_iteration()
+    bounds = [0, 1, 400_000, 400_001, 777_777, w.n_events]
+    for lo, hi in zip(bounds[:-1], bounds[1:]):
+        g.accumulate(lo, hi - lo, w.seed, 3, w.integrand_id, 64)
+    g.reduce()
+    tot = g.totals_tensor().cpu().numpy()
+    assert tot.shape == (4 + w.dim * w.n_bins,)
+    I, s, H, st = g.finalize(w.n_events)
+    assert I == pytest.approx(whole[0], rel=1e-13) and s == pytest.approx(whole[1], rel=1e-12)
+    np.testing.assert_allclose(H, whole[2], rtol=1e-12)
+    np.testing.assert_allclose(tot[4:].reshape(w.dim, w.n_bins), H, rtol=0)
+    # events beyond 2^32: the high counter word is live
+    off = (3 << 32) + 12345
+    n = 200_003
+    g.begin_iteration()
+    g.accumulate(off, n, w.seed, 3, w.integrand_id, 64)
+    g.reduce()
+    I, s, H, st = g.finalize(n)
+    S1, S2, Ho = O.accumulate(edges, w.seed, 3, off, n, w.integrand_id, w.params)
+    oI, oS = O.estimate(S1, S2, n)
+    assert I == pytest.approx(oI, rel=RTOL64) and s == pytest.approx(oS, rel=RTOL64)
+    np.testing.assert_allclose(H, Ho.astype(np.float64), rtol=RTOL64)
+    g.close()
+
+
+# ------------------------------------------------------------------ P7: 5 sigma, control, fixed point
+def test_p7_constant_control_and_fixed_point(B):
+    w = W.control_const(n_events=10_000_000)
+    g = _grid(B, w)
+    r = g.integrate(3, w.n_events, w.seed, w.alpha, w.integrand_id, 64)
+    # reading R9: exactly 1 up to rounding on the uniform grid
+    assert abs(r["per_iter"][0, 0] - 1.0) <= 1e-12 and r["per_iter"][0, 1] <= 1e-9
+    o = O.integrate(w.dim, w.n_bins, 3, w.n_events, w.seed, w.alpha, w.integrand_id, None, threads=THREADS)
+    np.testing.assert_allclose(r["per_iter"][1:, 0], o["per_iter"][1:, 0], rtol=RTOL64)
+    np.testing.assert_allclose(r["per_iter"][1:, 1], o["per_iter"][1:, 1], rtol=1e-8)
+    # reading R10(ii): sampled flat histogram leaves the grid within 1e-3 of uniform
+    assert np.abs(g.get_edges() - O.uniform_edges(w.dim, w.n_bins)).max() < 1e-3
+    g.close()
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 4, 5])
+def test_p7_five_sigma_rule(B, cfg):
+    w = _small(cfg).scaled(n_events=SMALL[cfg]["n_events"], n_iter=8)
+    g = _grid(B, w)
+    n_skip = 2                       # reduced-size chains: the first iterations under-estimate sigma (F1)
+    r = g.integrate(w.n_iter, w.n_events, w.seed, w.alpha, w.integrand_id, 64, n_skip=n_skip)
+    exact = w.closed_form
+    assert abs(r["I"] - exact) < 5 * r["sigma"]
+    for k in range(n_skip, w.n_iter):
+        assert abs(r["per_iter"][k, 0] - exact) < 5 * r["per_iter"][k, 1]
+    g.close()
+
+
+# ------------------------------------------------------------------ edge cases
+def test_edge_shapes(B):
+    rng = np.random.default_rng(1)
+    cases = [(1, 2, 2), (1, 256, 1000), (32, 2, 5000), (32, 256, 20_011), (5, 3, 3), (17, 31, 33), (4, 128, 31)]
+    for dim, nb, n in cases:
+        edges = W.adapted_edges(dim, nb, seed=dim * nb)
+        # c in [1,3]: keeps prod_j (c_j^-2 + t^2) inside the fp32 range for dim = 32
+        params = np.concatenate([1 + 2 * rng.random(dim), rng.random(dim)])
+        g = B.VegasGrid(dim, nb)
+        g.set_params(B.VEGAS_F_GENZ_PRODUCT_PEAK, params)
+        g.set_params(B.VEGAS_F_GAUSS, [0.3])
+        g.set_edges(edges)
+        for fid, p in ((B.VEGAS_F_GENZ_PRODUCT_PEAK, params), (B.VEGAS_F_GAUSS, [0.3]), (B.VEGAS_F_CONST, None)):
+            for precision in (64, 32):
+                I, s, H, st = g.iterate(n, 9, 4, fid, precision)
+                oI, oS, oH = O.iterate(edges, n, 9, 4, fid, p)
+                tol = RTOL64 if precision == 64 else 2 * RTOL32
+                assert st == 0 and I == pytest.approx(oI, rel=tol)
+                assert s == pytest.approx(oS, rel=tol if precision == 64 else 1e-4, abs=1e-300)
+                _assert_hist(H, oH, precision) if precision == 64 else None
+        g.close()
+
+
+def test_bw_poly_other_dimensions(B):
+    for dim in (2, 3, 9):
+        p = W.bw_poly_params(dim, 77)
+        edges = W.adapted_edges(dim, 40, seed=dim)
+        g = B.VegasGrid(dim, 40)
+        g.set_params(B.VEGAS_F_BW_POLY, p)
+        g.set_edges(edges)
+        I, s, H, st = g.iterate(100_001, 3, 0, B.VEGAS_F_BW_POLY, 64)
+        oI, oS, oH = O.iterate(edges, 100_001, 3, 0, O.BW_POLY, p)
+        assert I == pytest.approx(oI, rel=RTOL64) and s == pytest.approx(oS, rel=RTOL64)
+        _assert_hist(H, oH, 64)
+        g.close()
+
+
+def test_errors(B):
+    import ctypes as C
+    assert B.vegas_workspace_bytes(0, 50) == 0 and B.vegas_workspace_bytes(33, 50) == 0
+    assert B.vegas_workspace_bytes(4, 1) == 0 and B.vegas_workspace_bytes(4, 257) == 0
+    with pytest.raises(B.VegasError):
+        B.VegasGrid(0, 50)
+    g = B.VegasGrid(4, 50)
+    with pytest.raises(B.VegasError) as e:
+        g.iterate(1000, 1, 0, B.VEGAS_F_GAUSS)            # params not set
+    assert e.value.code == B.VEGAS_EINVAL
+    g.set_params(B.VEGAS_F_GAUSS, [0.1])
+    for bad in (dict(n_events=1), dict(integrand_id=7), dict(precision=16)):
+        kw = dict(n_events=1000, seed=1, iteration=0, integrand_id=B.VEGAS_F_GAUSS, precision=64)
+        kw.update(bad)
+        with pytest.raises(B.VegasError) as e:
+            g.iterate(**kw)
+        assert e.value.code == B.VEGAS_EINVAL
+    with pytest.raises(B.VegasError):
+        g.set_params(B.VEGAS_F_GAUSS, [0.1, 0.2])
+    with pytest.raises(B.VegasError):
+        g.set_params(B.VEGAS_F_GENZ_PRODUCT_PEAK, [1.0] * 7)
+    e2 = O.uniform_edges(4, 50)
+    e2[2, 10] = e2[2, 9]
+    with pytest.raises(B.VegasError):
+        g.set_edges(e2)
+    e3 = O.uniform_edges(4, 50)
+    e3[0, -1] = 0.999
+    with pytest.raises(B.VegasError):
+        g.set_edges(e3)
+    with pytest.raises(B.VegasError):
+        g.refine(-1.0)
+    with pytest.raises(B.VegasError):
+        g.refine(float("nan"))
+    with pytest.raises(B.VegasError):
+        g.set_launch(0, 0, 3, 0)                          # not a power of two
+    with pytest.raises(B.VegasError):
+        g.set_launch(0, 1000, 0, 0)                       # not a multiple of 32
+    with pytest.raises(B.VegasError):
+        g.integrate(0, 1000, 1, 1.5, B.VEGAS_F_GAUSS)
+    with pytest.raises(B.VegasError):
+        g.integrate(3, 1000, 1, 1.5, B.VEGAS_F_GAUSS, n_skip=3)
+    # too small / misaligned workspace
+    import torch
+    buf = torch.empty(4096, dtype=torch.uint8, device="cuda")
+    h = C.c_void_p()
+    assert B.lib.vegas_create(4, 50, C.c_void_p(buf.data_ptr()), 4096, C.byref(h)) == B.VEGAS_EINVAL
+    big = torch.empty(B.vegas_workspace_bytes(4, 50) + 512, dtype=torch.uint8, device="cuda")
+    assert B.lib.vegas_create(4, 50, C.c_void_p(big.data_ptr() + 8), big.numel() - 8, C.byref(h)) == B.VEGAS_EINVAL
+    # the grid is still usable after the failed calls
+    I, s, H, st = g.iterate(10_000, 1, 0, B.VEGAS_F_GAUSS)
+    oI, oS, oH = O.iterate(O.uniform_edges(4, 50), 10_000, 1, 0, O.GAUSS, [0.1])
+    assert st == 0 and I == pytest.approx(oI, rel=RTOL64)
+    g.close()
+
+
+def test_non_default_stream_and_counters(B):
+    import torch
+    w = _small(1)
+    g = _grid(B, w)
+    st = torch.cuda.Stream()
+    g.set_profiling(True)
+    g.reset_counters()
+    with torch.cuda.stream(st):
+        I, s, H, rc = g.iterate(w.n_events, w.seed, 0, w.integrand_id, 64, chunk_events=30_000)
+    ms, n = g.kernel_time_ms()
+    assert n == 4 and ms > 0 and g.launch_count() == 4 + 2     # 4 chunks + reduce + finalize
+    oI, oS, oH = O.iterate(O.uniform_edges(w.dim, w.n_bins), w.n_events, w.seed, 0, w.integrand_id, w.params)
+    assert I == pytest.approx(oI, rel=RTOL64)
+    g.close()
+
+
+# ------------------------------------------------------------------ full BASELINE sizes, bench launch shape
+@pytest.mark.parametrize("cfg,precision", [(2, 64), (3, 64), (3, 32), (4, 64), (5, 64)])
+def test_full_size_iteration_in_bench_configuration(B, chains, cfg, precision):
+    """One iteration at the config's full n_events (and chunking) on the adapted grid of the small
+    oracle chain, default launch shape (what bench.py times), against the oracle run on all host
+    cores; plus sampled events through K4 and the size-independent invariant sum_b H[j][b] = S2."""
+    w = W.config(cfg)
+    edges = chains[cfg]["edges"]
+    g = _grid(B, w, edges)
+    it = 5
+    I, s, H, st = g.iterate(w.n_events, w.seed, it, w.integrand_id, precision, chunk_events=w.chunk_events)
+    assert st == 0
+    n = w.n_events
+    S2 = n * (s * s * (n - 1) + I * I)
+    np.testing.assert_allclose(H.sum(axis=1), S2, rtol=1e-9 if precision == 64 else 1e-6)
+    rng = np.random.default_rng(cfg)
+    for first in rng.integers(0, n - 64, size=6).tolist() + [0, n - 64]:
+        gw, gb, gx, gf = g.debug_sample(first, 64, w.seed, it, w.integrand_id, precision)
+        ow, ob, ox, of = O.sample(edges, w.seed, it, first, 64, w.integrand_id, w.params)
+        assert np.array_equal(gw, ow) and np.array_equal(gb, ob)
+        if precision == 64:
+            np.testing.assert_allclose(gf, of, rtol=1e-12)
+    oI, oS, oH = O.iterate(edges, n, w.seed, it, w.integrand_id, w.params, threads=THREADS)
+    tol = RTOL64 if precision == 64 else RTOL32
+    assert I == pytest.approx(oI, rel=tol) and s == pytest.approx(oS, rel=tol)
+    _assert_hist(H, oH, precision)
+    assert abs(I - w.closed_form) < 5 * s
+    g.close()

@@ -1,0 +1,310 @@
+#!/usr/bin/env python
+"""bench.py -- events/s of one Vegas iteration (fused iterate kernel + reduce + finalize + refine) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--precision 64|32]
+    python bench.py --impl reference ...      # the CPU oracle on the host cores, same metric/config
+
+A "step" is one pass of the whole hot path over one batch: one Vegas iteration
+of the workload's n_events events (in its chunk size) followed by the grid refinement.  Warm-up steps
+are the first iterations of the chain, so the timed steps run on an adapted grid (equiprobable bins:
+the conflict-heavy state the method spends its time in).  Inputs are seeded and synthetic
+(paper_2002_12921_b200/workloads.py).  One JSON line on stdout (rank 0).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "events/sec per Vegas iteration"
+UNIT = "events/s"
+SM_COUNT, ISSUE_LANES, FP64_LANES = 148, 128, 64          # per SM per clock (guide + profiles/r01_ubench_pipes.md)
+INTEGRAND_DIM_FP = {0: 0, 1: 2, 2: 3, 3: 4}                # SURVEY.md 8(d) counting rule
+INTEGRAND_EVENT_FP = {0: {64: 0, 32: 0}, 1: {64: 19, 32: 5}, 2: {64: 8, 32: 8}, 3: {64: 12, 32: 12}}
+
+
+def n_issue(w, precision):
+    """Algorithmic thread-level instructions per event (SURVEY.md 8(d) counting rule)."""
+    d = w.dim
+    per_dim_fp = INTEGRAND_DIM_FP[w.integrand_id] * (d - 1 if w.integrand_id == 3 else d)
+    return 42 * ((d + 3) // 4) + d * (4 + 1 + 2 + 3) + per_dim_fp + 3 + 4 + INTEGRAND_EVENT_FP[w.integrand_id][precision]
+
+
+def n_fp(w, precision):
+    d = w.dim
+    per_dim_fp = INTEGRAND_DIM_FP[w.integrand_id] * (d - 1 if w.integrand_id == 3 else d)
+    return 3 * d + per_dim_fp + 4 + INTEGRAND_EVENT_FP[w.integrand_id][precision]
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return json.load(fh)
+    except Exception:
+        return {}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.gpu, self.rows, self.proc = gpu_index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([t.strip() for t in line.split(",")])
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+        sm, smax, reasons, power = [], 0.0, set(), 0.0
+        for r in self.rows:
+            try:
+                sm.append(float(r[1])); smax = max(smax, float(r[2])); power = max(power, float(r[3]))
+            except Exception:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        busy = [c for c in sm if c > 0.5 * smax] or sm
+        return {"sm_mhz": statistics.median(busy) if busy else None, "sm_max_mhz": smax or None,
+                "reasons": sorted(reasons), "power_w_max": power or None, "samples": len(sm)}
+
+
+def cpu_baseline(w, edges, target_cpu_seconds=16.0):
+    """The oracle, as it stands, on the host cores: a bounded sample of the same workload."""
+    import oracle as O
+    cores = os.cpu_count() or 1
+    t0 = time.perf_counter()
+    O.iterate(edges, 200_000, w.seed, 0, w.integrand_id, w.params, threads=1)
+    rate1 = 200_000 / (time.perf_counter() - t0)
+    n = int(min(w.n_events, max(cores * 100_000, rate1 * target_cpu_seconds)))
+    t0 = time.perf_counter()
+    O.iterate(edges, n, w.seed, 1, w.integrand_id, w.params, threads=cores)
+    dt = time.perf_counter() - t0
+    return {"value": n / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "%d of %d events of one %s iteration on the adapted grid, %d threads over disjoint "
+                      "event ranges (%.1f s wall)" % (n, w.n_events, w.name, cores, dt),
+            "per_core": n / dt / cores}
+
+
+def run_reference(args, w, precision):
+    """--impl reference: the oracle timed on the host cores; each step = one iteration + refine over a
+    bounded sample of the workload's events."""
+    import oracle as O
+    from oracle import build as obuild
+    obuild.build()
+    cores = os.cpu_count() or 1
+    edges = O.uniform_edges(w.dim, w.n_bins)
+    t0 = time.perf_counter()
+    O.iterate(edges, 100_000, w.seed, 0, w.integrand_id, w.params, threads=1)
+    rate1 = 100_000 / (time.perf_counter() - t0)
+    budget = 120.0 / max(1, args.steps + args.warmup)              # wall seconds per step
+    n = int(min(w.n_events, max(cores * 50_000, rate1 * cores * 0.6 * budget)))
+    k = 0
+    for _ in range(args.warmup):
+        _, _, H = O.iterate(edges, n, w.seed, k, w.integrand_id, w.params, threads=cores)
+        edges, _ = O.refine(edges, H, w.alpha)
+        k += 1
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        _, _, H = O.iterate(edges, n, w.seed, k, w.integrand_id, w.params, threads=cores)
+        edges, _ = O.refine(edges, H, w.alpha)
+        k += 1
+    dt = time.perf_counter() - t0
+    value = n * args.steps / dt
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "dim": w.dim, "n_bins": w.n_bins, "integrand": w.integrand_id,
+                       "n_events_per_step": n, "full_n_events": w.n_events},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": "%d events per step (bounded sample of %d), %d threads" % (n, w.n_events, cores)},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="cfg3", help="cfg1..cfg5 (BASELINE.json configs)")
+    ap.add_argument("--precision", type=int, default=64, choices=[64, 32])
+    ap.add_argument("--n-events", type=int, default=0, help="override events per step per GPU")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--launch", default="", help="blocks,threads,table_copies,hist_copies (0 = auto)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+
+    from paper_2002_12921_b200 import workloads as W
+    w = W.config(int(args.workload.replace("cfg", "")))
+    if args.n_events:
+        w = w.scaled(args.n_events)
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        if rank == 0:
+            run_reference(args, w, args.precision)
+        return
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2002_12921_b200 import binding as B
+    from paper_2002_12921_b200 import distributed as D
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    g = B.VegasGrid(w.dim, w.n_bins)
+    g.set_params(w.integrand_id, w.params)
+    if args.launch:
+        g.set_launch(*[int(v) for v in args.launch.split(",")])
+    shape = g.get_launch(args.precision)
+    n_step = w.n_events * world                                   # weak scaling: n_events per GPU per step
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+
+    def step(k):
+        I, s, _, st = D.iterate_sharded(g, n_step, w.seed, k, w.integrand_id, args.precision, w.chunk_events,
+                                        rank, world, want_hist=False)
+        g.refine(w.alpha)
+        return I, s
+
+    k = 0
+    for _ in range(args.warmup):
+        step(k)
+        k += 1
+    # ---- timed region: K steps, device events per step (L2 flushed between steps, outside the brackets)
+    sampler = ClockSampler(local_rank)
+    g.set_profiling(True)
+    g.reset_counters()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    results = []
+    barrier()
+    sampler.start()
+    t_wall = time.perf_counter()
+    for i in range(args.steps):
+        flush.zero_()
+        ev[i][0].record()
+        results.append(step(k))
+        ev[i][1].record()
+        k += 1
+    barrier()
+    t_wall = time.perf_counter() - t_wall
+    clocks = sampler.stop()
+    ms = sum(a.elapsed_time(b) for a, b in ev)
+    k1_ms, k1_launches = g.kernel_time_ms()
+    launches = g.launch_count()
+    g.set_profiling(False)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = n_step * args.steps / (ms * 1e-3)
+
+    # ---- e2e: the same step through the C ABI with HOST buffers (edges in, I/sigma/hist/edges out)
+    edges_host = g.get_edges()
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        g.set_edges(edges_host)
+        if world > 1:
+            I, s, H, st = D.iterate_sharded(g, n_step, w.seed, k, w.integrand_id, args.precision, w.chunk_events,
+                                            rank, world, want_hist=True)
+        else:
+            I, s, H, st = g.iterate(n_step, w.seed, k, w.integrand_id, args.precision, w.chunk_events, want_hist=True)
+        g.refine(w.alpha, hist=H)
+        edges_host = g.get_edges()
+        k += 1
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    nent = w.dim * w.n_bins
+    h2d = 8 * w.dim * (w.n_bins + 1) + 8 * nent + 8 * B.VEGAS_MAX_PARAMS   # edges + hist for refine + by-value params
+    d2h = 24 + 8 * nent + 8 * w.dim * (w.n_bins + 1) + 4
+
+    if rank == 0:
+        peaks = measured_peaks()
+        sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+        clk = float(clocks["sm_mhz"] or sm_max)
+        ni, nf = n_issue(w, args.precision), n_fp(w, args.precision)
+        k1_s = (k1_ms * 1e-3) / max(1, k1_launches)
+        events_per_launch = (w.n_events if not w.chunk_events else min(w.chunk_events, w.n_events))
+        k1_rate = events_per_launch / k1_s                         # events/s of the fused kernel alone
+        peak_instr = SM_COUNT * ISSUE_LANES * sm_max * 1e6         # thread-instructions/s at max clock
+        roofline = {"bound": "alu", "kernel": "k_iterate",
+                    "achieved": k1_rate * ni / 1e12, "peak": peak_instr / 1e12, "unit": "Tinstr/s",
+                    "frac": k1_rate * ni / peak_instr,
+                    "frac_at_measured_clock": k1_rate * ni / (SM_COUNT * ISSUE_LANES * clk * 1e6),
+                    "peak_source": "148 SMs x 128 issue lanes x sm_max_mhz of MEASURED_PEAKS.json (%s); issue rate "
+                                   "confirmed by profiles/r01_ubench_pipes.md" % ("measured" if peaks else "fallback 1965 MHz"),
+                    "instr_per_event": ni, "fp_instr_per_event": nf,
+                    "fp_pipe_frac": k1_rate * nf / (SM_COUNT * (FP64_LANES if args.precision == 64 else ISSUE_LANES) * sm_max * 1e6),
+                    "kernel_events_per_s": k1_rate, "kernel_ms_per_launch": k1_s * 1e3, "kernel_launches": int(k1_launches),
+                    "kernel_share_of_step": k1_ms / ms if world == 1 else None,
+                    "traffic": None}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64" if args.precision == 64 else "f32", "data": "synthetic",
+                "config": {"workload": w.name, "dim": w.dim, "n_bins": w.n_bins, "integrand": W.INTEGRAND_NAMES[w.integrand_id],
+                           "n_events_per_gpu_per_step": w.n_events, "chunk_events": w.chunk_events, "alpha": w.alpha,
+                           "seed": w.seed, "launch": shape, "l2": "256 MiB memset between timed steps, outside the event brackets "
+                           "(the path reads ~10 KB of global memory per launch)",
+                           "grid": "adapted by the %d warm-up iterations" % args.warmup},
+                "clocks": clocks, "wall_s_timed_region": t_wall,
+                "e2e": {"value": n_step * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+                "gpu_launches": int(launches),
+                "roofline": roofline,
+                "last_iteration": {"I": results[-1][0], "sigma": results[-1][1], "closed_form": w.closed_form}}
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(w, edges_host)
+        print(json.dumps(line))
+    g.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

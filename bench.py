@@ -198,7 +198,7 @@ def main():
     g.set_params(w.integrand_id, w.params)
     if args.launch:
         g.set_launch(*[int(v) for v in args.launch.split(",")])
-    shape = g.get_launch(args.precision)
+    shape = g.get_launch(w.integrand_id, args.precision)
     n_step = w.n_events * world                                   # weak scaling: n_events per GPU per step
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
 

@@ -164,12 +164,16 @@ int vegas_debug_sample(vegas_grid* g, uint64_t first_event, uint32_t count, uint
                        void* cuda_stream, uint32_t* words, int32_t* bins, double* x, double* fJ);
 
 /* Launch shape of the fused kernel.  0 = automatic for any field.  blocks: CTAs per launch (default:
- * one per SM); threads: per CTA (multiple of 32, <= 1024); table_copies / hist_copies: bank-interleaved
- * replicas of the grid table / histogram in shared memory (powers of two, <= 32), see DESIGN.md.
- * VEGAS_EINVAL if the combination does not fit the device's shared memory. */
+ * one or two per SM); threads: per CTA (multiple of 32, <= 512).  The library has two fused kernels
+ * (DESIGN.md "Kernels"): the fast path (path 1: compile-time dimension, affine pre-composed table, bank
+ * rotation; CONST and GAUSS in both precisions, GENZ product peak in fp64, when its shared memory fits)
+ * and the generic path (path 0: every integrand, any shape).  table_copies / hist_copies are the
+ * bank-interleaved replicas of the grid table / histogram of the GENERIC kernel (powers of two, <= 32);
+ * setting either to a non-zero value pins the generic path.  VEGAS_EINVAL if the combination does not fit
+ * the device's shared memory.  vegas_get_launch reports what a call with (integrand_id, precision) will use. */
 int vegas_set_launch(vegas_grid* g, int blocks, int threads, int table_copies, int hist_copies);
-int vegas_get_launch(vegas_grid* g, int precision, int* blocks, int* threads, int* table_copies,
-                     int* hist_copies, size_t* shared_bytes);
+int vegas_get_launch(vegas_grid* g, int integrand_id, int precision, int* path, int* blocks, int* threads,
+                     int* table_copies, int* hist_copies, size_t* shared_bytes);
 
 /* Instrumentation for bench.py: with profiling on, every fused-kernel launch is bracketed by CUDA
  * events on its stream; vegas_kernel_time_ms() synchronises those events and returns their summed

@@ -54,8 +54,8 @@ SIGNATURES = {
     "vegas_debug_sample": (C.c_int, [_vp, _u64, C.c_uint32, _u64, C.c_uint32, C.c_int, C.c_int, _vp, _vp,
                                      _u32p, _i32p, _f64p, _f64p]),
     "vegas_set_launch": (C.c_int, [_vp, C.c_int, C.c_int, C.c_int, C.c_int]),
-    "vegas_get_launch": (C.c_int, [_vp, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int),
-                                   C.POINTER(C.c_int), C.POINTER(C.c_size_t)]),
+    "vegas_get_launch": (C.c_int, [_vp, C.c_int, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int),
+                                   C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_size_t)]),
     "vegas_set_profiling": (C.c_int, [_vp, C.c_int]),
     "vegas_kernel_time_ms": (C.c_int, [_vp, _f64p, C.POINTER(_u64)]),
     "vegas_launch_count": (_u64, [_vp]),
@@ -250,12 +250,12 @@ class VegasGrid:
     def set_launch(self, blocks=0, threads=0, table_copies=0, hist_copies=0):
         self._check(lib.vegas_set_launch(self._h, blocks, threads, table_copies, hist_copies))
 
-    def get_launch(self, precision=VEGAS_FP64):
-        b, t, ct, ch, sh = C.c_int(), C.c_int(), C.c_int(), C.c_int(), C.c_size_t()
-        self._check(lib.vegas_get_launch(self._h, precision, C.byref(b), C.byref(t), C.byref(ct), C.byref(ch),
-                                         C.byref(sh)))
-        return dict(blocks=b.value, threads=t.value, table_copies=ct.value, hist_copies=ch.value,
-                    shared_bytes=sh.value)
+    def get_launch(self, integrand_id=VEGAS_F_CONST, precision=VEGAS_FP64):
+        pa, b, t, ct, ch, sh = C.c_int(), C.c_int(), C.c_int(), C.c_int(), C.c_int(), C.c_size_t()
+        self._check(lib.vegas_get_launch(self._h, integrand_id, precision, C.byref(pa), C.byref(b), C.byref(t),
+                                         C.byref(ct), C.byref(ch), C.byref(sh)))
+        return dict(path="rotated" if pa.value else "generic", blocks=b.value, threads=t.value,
+                    table_copies=ct.value, hist_copies=ch.value, shared_bytes=sh.value)
 
     def set_profiling(self, on=True):
         self._check(lib.vegas_set_profiling(self._h, int(bool(on))))

@@ -12,6 +12,7 @@
 
 #include "../../include/vegas.h"
 #include "vegas_kernels.h"
+#include "vegas_iterate_rot.cuh"
 
 namespace {
 
@@ -58,7 +59,7 @@ int expected_n_params(int fid, int dim) {
 
 struct vegas_grid {
     int dim = 0, n_bins = 0, device = 0, sm_count = 0;
-    size_t smem_optin = 0;
+    size_t smem_optin = 0, smem_total_sm = 0;
     unsigned char* ws = nullptr;
     Layout L{};
     double* d_edges = nullptr;
@@ -69,6 +70,7 @@ struct vegas_grid {
     double* d_partials = nullptr;
     bool params_set[4] = {true, false, false, false};
     double derived[4][VEGAS_MAX_PARAMS] = {};
+    double user[4][VEGAS_MAX_PARAMS] = {};       // the caller's arrays as given to vegas_set_params
     int cfg_blocks = 0, cfg_threads = 0, cfg_ct = 0, cfg_ch = 0;
     int active_blocks = 0;          // CTAs whose partial slots the current iteration uses
     bool profiling = false;
@@ -159,6 +161,75 @@ double jac_scale_for(const vegas_grid* g, int precision) {
     return s;
 }
 
+// The fast path (vegas_iterate_rot.cuh) serves integrands that are functions of per-dimension affine
+// variables; it is taken unless the caller pinned the copy counts of the generic kernel with
+// vegas_set_launch (which is also how the tests keep the generic kernel covered).
+bool use_rot_path(const vegas_grid* g, int fid, int precision) {
+    if (g->cfg_ct > 0 || g->cfg_ch > 0) return false;
+    const bool kind = fid == VEGAS_F_CONST || fid == VEGAS_F_GAUSS ||
+                      (fid == VEGAS_F_GENZ_PRODUCT_PEAK && precision == VEGAS_FP64);
+    if (!kind) return false;
+    if (g->cfg_threads > vegas::kRotThreads) return false;
+    return vegas::rot_shared_bytes(g->dim, g->n_bins) <= g->smem_optin;
+}
+
+// shift_j, scale_j, post_scale, fin0 of the affine pre-composition (see vegas_iterate_rot.cuh)
+void rot_constants(const vegas_grid* g, int fid, double* shift, double* scale, double* post_scale, double* fin0) {
+    const int dim = g->dim;
+    const double nb = (double)g->n_bins;
+    *post_scale = 1.0;
+    *fin0 = 0.0;
+    for (int j = 0; j < VEGAS_MAX_DIM; ++j) { shift[j] = 0.0; scale[j] = nb; }
+    if (fid == VEGAS_F_GAUSS) {
+        const double a = g->user[fid][0];
+        for (int j = 0; j < dim; ++j) shift[j] = 0.5;
+        *fin0 = 1.0 / ((nb * a) * (nb * a));
+        *post_scale = g->derived[fid][0];                       // (a sqrt(pi))^-d; prod B_j is the Jacobian
+    } else if (fid == VEGAS_F_GENZ_PRODUCT_PEAK) {
+        double ps = 1.0;
+        for (int j = 0; j < dim; ++j) {
+            const double c = g->user[fid][j];
+            shift[j] = g->user[fid][dim + j];
+            scale[j] = c;
+            ps *= c * nb;                                        // f J = prod(c_j nb) prod B_j / prod(1+u_j^2)
+        }
+        *post_scale = ps;
+    }
+}
+
+struct RotShape {
+    int blocks, threads;
+    size_t shmem;
+};
+
+RotShape rot_shape(const vegas_grid* g) {
+    RotShape s;
+    s.shmem = vegas::rot_shared_bytes(g->dim, g->n_bins);
+    s.threads = g->cfg_threads > 0 ? g->cfg_threads : vegas::kRotThreads;
+    int per_sm = (int)(g->smem_total_sm / (s.shmem + 1024));
+    if (per_sm < 1) per_sm = 1;
+    if (per_sm > vegas::kRotMinBlocks) per_sm = vegas::kRotMinBlocks;
+    s.blocks = g->cfg_blocks > 0 ? g->cfg_blocks : g->sm_count * per_sm;
+    return s;
+}
+
+cudaError_t launch_rot(int fid, int precision, int dim, const vegas::RotArgs& a, const RotShape& s, cudaStream_t st) {
+    if (precision == VEGAS_FP64) {
+        switch (fid) {
+        case VEGAS_F_CONST: return vegas::launch_iterate_rot<VEGAS_F_CONST, double>(dim, a, s.blocks, s.threads, s.shmem, st);
+        case VEGAS_F_GAUSS: return vegas::launch_iterate_rot<VEGAS_F_GAUSS, double>(dim, a, s.blocks, s.threads, s.shmem, st);
+        case VEGAS_F_GENZ_PRODUCT_PEAK:
+            return vegas::launch_iterate_rot<VEGAS_F_GENZ_PRODUCT_PEAK, double>(dim, a, s.blocks, s.threads, s.shmem, st);
+        }
+    } else {
+        switch (fid) {
+        case VEGAS_F_CONST: return vegas::launch_iterate_rot<VEGAS_F_CONST, float>(dim, a, s.blocks, s.threads, s.shmem, st);
+        case VEGAS_F_GAUSS: return vegas::launch_iterate_rot<VEGAS_F_GAUSS, float>(dim, a, s.blocks, s.threads, s.shmem, st);
+        }
+    }
+    return cudaErrorInvalidValue;
+}
+
 int finish_iteration(vegas_grid* g, uint64_t n_total, cudaStream_t st, double* I, double* sigma, double* hist_host) {
     const size_t nent = (size_t)g->dim * g->n_bins;
     CUDA_TRY(g, vegas::launch_finalize(g->d_totals, (double)n_total, g->d_result, st));
@@ -200,6 +271,7 @@ int vegas_create(int dim, int n_bins, void* dev_workspace, size_t bytes, vegas_g
     g->n_bins = n_bins;
     g->sm_count = prop.multiProcessorCount;
     g->smem_optin = prop.sharedMemPerBlockOptin;
+    g->smem_total_sm = prop.sharedMemPerMultiprocessor;
     g->ws = (unsigned char*)dev_workspace;
     g->L = L;
     g->d_edges = (double*)(g->ws + L.edges);
@@ -233,6 +305,8 @@ int vegas_set_params(vegas_grid* g, int fid, const double* p, int n_params) {
         if (!std::isfinite(p[i])) return VEGAS_EINVAL;
     double* d = g->derived[fid];
     std::memset(d, 0, sizeof(g->derived[fid]));
+    std::memset(g->user[fid], 0, sizeof(g->user[fid]));
+    for (int i = 0; i < want; ++i) g->user[fid][i] = p[i];
     const int dim = g->dim;
     switch (fid) {
     case VEGAS_F_CONST: break;
@@ -305,9 +379,16 @@ int vegas_begin_iteration(vegas_grid* g, void* cuda_stream) {
     CUDA_TRY(g, cudaSetDevice(g->device));
     LaunchShape s;
     if (resolve_launch(g, VEGAS_FP64, &s)) return VEGAS_EINVAL;
-    g->active_blocks = s.blocks;
+    // either kernel path may serve the accumulate calls of this iteration: reserve slots for the wider one
+    int blocks = s.blocks;
+    if (use_rot_path(g, VEGAS_F_CONST, VEGAS_FP64)) {
+        const RotShape r = rot_shape(g);
+        if (r.blocks > blocks) blocks = r.blocks;
+    }
+    if (blocks > kMaxBlocks) return VEGAS_EINVAL;
+    g->active_blocks = blocks;
     const size_t ntot = 4 + (size_t)g->dim * g->n_bins;
-    CUDA_TRY(g, cudaMemsetAsync(g->d_partials, 0, sizeof(double) * ntot * s.blocks, st));
+    CUDA_TRY(g, cudaMemsetAsync(g->d_partials, 0, sizeof(double) * ntot * blocks, st));
     return VEGAS_OK;
 }
 
@@ -317,24 +398,39 @@ int vegas_accumulate(vegas_grid* g, uint64_t first_event, uint64_t count, uint64
     if (g->active_blocks <= 0) return VEGAS_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     CUDA_TRY(g, cudaSetDevice(g->device));
-    LaunchShape s;
-    if (resolve_launch(g, precision, &s)) return VEGAS_EINVAL;
-    if (s.blocks != g->active_blocks) return VEGAS_EINVAL;
-    vegas::IterArgs a;
-    a.edges = g->d_edges;
-    a.partials = g->d_partials;
-    a.key0 = (uint32_t)(seed & 0xFFFFFFFFu);
-    a.key1 = (uint32_t)(seed >> 32);
-    a.iteration = iteration;
-    a.dim = g->dim;
-    a.n_bins = g->n_bins;
-    a.log_ct = ilog2(s.ct);
-    a.log_ch = ilog2(s.ch);
-    a.jac_scale = jac_scale_for(g, precision);
+    const bool rot = use_rot_path(g, fid, precision);
+    LaunchShape s{};
+    RotShape rs{};
+    vegas::IterArgs a{};
+    vegas::RotArgs ra{};
+    if (rot) {
+        rs = rot_shape(g);
+        if (rs.blocks > g->active_blocks) return VEGAS_EINVAL;
+        ra.edges = g->d_edges;
+        ra.partials = g->d_partials;
+        ra.key0 = (uint32_t)(seed & 0xFFFFFFFFu);
+        ra.key1 = (uint32_t)(seed >> 32);
+        ra.iteration = iteration;
+        ra.n_bins = g->n_bins;
+        rot_constants(g, fid, ra.shift, ra.scale, &ra.post_scale, &ra.fin0);
+    } else {
+        if (resolve_launch(g, precision, &s)) return VEGAS_EINVAL;
+        if (s.blocks > g->active_blocks) return VEGAS_EINVAL;
+        a.edges = g->d_edges;
+        a.partials = g->d_partials;
+        a.key0 = (uint32_t)(seed & 0xFFFFFFFFu);
+        a.key1 = (uint32_t)(seed >> 32);
+        a.iteration = iteration;
+        a.dim = g->dim;
+        a.n_bins = g->n_bins;
+        a.log_ct = ilog2(s.ct);
+        a.log_ch = ilog2(s.ch);
+        a.jac_scale = jac_scale_for(g, precision);
+    }
     const uint64_t chunk = chunk_events ? chunk_events : count;
     for (uint64_t done = 0; done < count; done += chunk) {
-        a.first_event = first_event + done;
-        a.count = (count - done < chunk) ? count - done : chunk;
+        a.first_event = ra.first_event = first_event + done;
+        a.count = ra.count = (count - done < chunk) ? count - done : chunk;
         cudaEvent_t e0 = nullptr, e1 = nullptr;
         if (g->profiling) {
             if (g->events_used + 2 > g->events.size()) {
@@ -349,7 +445,10 @@ int vegas_accumulate(vegas_grid* g, uint64_t first_event, uint64_t count, uint64
             g->events_used += 2;
             CUDA_TRY(g, cudaEventRecord(e0, st));
         }
-        CUDA_TRY(g, vegas::launch_iterate(fid, precision, a, g->derived[fid], s.blocks, s.threads, s.shmem, st));
+        if (rot)
+            CUDA_TRY(g, launch_rot(fid, precision, g->dim, ra, rs, st));
+        else
+            CUDA_TRY(g, vegas::launch_iterate(fid, precision, a, g->derived[fid], s.blocks, s.threads, s.shmem, st));
         if (g->profiling) CUDA_TRY(g, cudaEventRecord(e1, st));
         g->iterate_launches++;
         g->launches++;
@@ -514,7 +613,9 @@ int vegas_debug_sample(vegas_grid* g, uint64_t first_event, uint32_t count, uint
     a.bins = (int32_t*)base;                   base += align_up(per_dim * 4);
     a.x = (double*)base;                       base += align_up(per_dim * 8);
     a.fJ = (double*)base;
-    CUDA_TRY(g, vegas::launch_debug(fid, precision, a, g->derived[fid], st));
+    const bool rot = use_rot_path(g, fid, precision);
+    if (rot) rot_constants(g, fid, a.shift, a.scale, &a.post_scale, &a.fin0);
+    CUDA_TRY(g, vegas::launch_debug(fid, precision, rot, a, g->derived[fid], st));
     g->launches++;
     if (words) CUDA_TRY(g, cudaMemcpyAsync(words, a.words, per_dim * 4, cudaMemcpyDeviceToHost, st));
     if (bins) CUDA_TRY(g, cudaMemcpyAsync(bins, a.bins, per_dim * 4, cudaMemcpyDeviceToHost, st));
@@ -544,9 +645,20 @@ int vegas_set_launch(vegas_grid* g, int blocks, int threads, int table_copies, i
     return VEGAS_OK;
 }
 
-int vegas_get_launch(vegas_grid* g, int precision, int* blocks, int* threads, int* table_copies, int* hist_copies,
-                     size_t* shared_bytes) {
-    if (!g || (precision != VEGAS_FP64 && precision != VEGAS_FP32)) return VEGAS_EINVAL;
+int vegas_get_launch(vegas_grid* g, int integrand_id, int precision, int* path, int* blocks, int* threads,
+                     int* table_copies, int* hist_copies, size_t* shared_bytes) {
+    if (!g || (precision != VEGAS_FP64 && precision != VEGAS_FP32) || integrand_id < 0 || integrand_id > 3)
+        return VEGAS_EINVAL;
+    if (use_rot_path(g, integrand_id, precision)) {
+        const RotShape r = rot_shape(g);
+        if (blocks) *blocks = r.blocks;
+        if (threads) *threads = r.threads;
+        if (table_copies) *table_copies = precision == VEGAS_FP64 ? 2 : 4;
+        if (hist_copies) *hist_copies = 8;
+        if (shared_bytes) *shared_bytes = r.shmem;
+        if (path) *path = 1;
+        return VEGAS_OK;
+    }
     LaunchShape s;
     if (resolve_launch(g, precision, &s)) return VEGAS_EINVAL;
     if (blocks) *blocks = s.blocks;
@@ -554,6 +666,7 @@ int vegas_get_launch(vegas_grid* g, int precision, int* blocks, int* threads, in
     if (table_copies) *table_copies = s.ct;
     if (hist_copies) *hist_copies = s.ch;
     if (shared_bytes) *shared_bytes = s.shmem;
+    if (path) *path = 0;
     return VEGAS_OK;
 }
 

@@ -1,0 +1,269 @@
+// vegas_iterate_rot.cuh -- K1, "rotated" fast path of the fused iterate kernel (sm_100a).
+//
+// Same computation as the generic k_iterate (vegas_kernels.cu), for integrands whose dependence on
+// x_j goes through a per-dimension affine variable u_j = scale_j (x_j - shift_j)
+// (CONST, GAUSS: u = n_bins (x - 1/2); GENZ product peak: u = c_j (x - w_j)).  Three changes, each
+// driven by a counter of profiles/r01_k_iterate_v1.md:
+//
+//  1. DIM is a compile-time constant: no per-dimension guards, fully unrolled, bins packed one byte
+//     per dimension in registers.
+//  2. Affine pre-composition: the shared-memory table holds, per (dimension, bin), the pair
+//     (A', B) with u = A' + B m, where m in [1,2) is built from the 32 low product bits by two funnel
+//     shifts (fp64: m = 1 + r exactly; fp32: 23 bits, centred).  One FMA gives u; x_j itself is never
+//     formed, and B is the Jacobian factor up to a per-dimension constant folded into post_scale.
+//     No integrand parameter is read inside the event loop.
+//  3. Bank rotation.  A Philox block serves 4 dimensions.  The 32 lanes of a warp are split into 4
+//     groups gamma = (lane>>1)&3; at sub-step i group gamma works on dimension 4 blk + (gamma ^ i)
+//     (its four Philox words are permuted accordingly, 8 SELs per block).  So the lanes of one
+//     shared-memory wavefront always touch different dimensions, and the rows
+//         table [blk*n_bins + bin] : 128 B = 4 dim-slots x 2 copies x 16 B   (fp32: 4 x 4 x 8 B)
+//         hist  [blk*n_bins + bin] : 256 B = 2 half-warps x 4 dim-slots x 4 copies x 8 B
+//     are conflict-free whatever bins the lanes drew, with 2 table copies and 8 histogram copies
+//     instead of 8 and 16, and no two lanes of a warp ever update the same histogram word (no CAS
+//     retries inside a warp).  A last block with 2 (1) dimensions uses 2 (1) groups and 4 (8) table
+//     copies in the same row size; with 3 dimensions it uses 4 groups and one idle sub-step.
+#pragma once
+#include "vegas_device.cuh"
+#include "vegas_kernels.h"
+
+namespace vegas {
+
+// ---- integrands in the affine variable u --------------------------------------------------------
+template <int FID, typename T> struct IntegrandU;
+
+template <typename T> struct IntegrandU<VEGAS_F_CONST, T> {
+    __device__ __forceinline__ void begin() {}
+    __device__ __forceinline__ void dim(T) {}
+    __device__ __forceinline__ T finish(T) const { return (T)1; }
+};
+template <typename T> struct IntegrandU<VEGAS_F_GAUSS, T> {   // PAPER.md:65 Eq.(1); u = n_bins (x - 1/2)
+    T s;
+    __device__ __forceinline__ void begin() { s = (T)0; }
+    __device__ __forceinline__ void dim(T u) { s = t_fma(u, u, s); }
+    __device__ __forceinline__ T finish(T fin0) const { return t_exp<T>(-s * fin0); }   // fin0 = 1/(n_bins a)^2
+};
+template <typename T> struct IntegrandU<VEGAS_F_GENZ_PRODUCT_PEAK, T> {   // PAPER.md:74 Eq.(3); u = c_j (x - w_j)
+    T prod;
+    __device__ __forceinline__ void begin() { prod = (T)1; }
+    __device__ __forceinline__ void dim(T u) { prod *= t_fma(u, u, (T)1); }
+    __device__ __forceinline__ T finish(T) const { return (T)1 / prod; }
+};
+
+// ---- table entry and u from the low product word ---------------------------------------------------
+template <typename T> struct RotEntry;
+template <> struct RotEntry<double> {
+    using type = double2;
+    static __device__ __forceinline__ double2 make(double x0, double x1, double shift, double scale) {
+        const double B = (x1 - x0) * scale, A = (x0 - shift) * scale;
+        return make_double2(A - B, B);                              // u = (A - B) + B m,  m = 1 + r
+    }
+    static __device__ __forceinline__ double u(double2 e, uint32_t lo) {
+        const double m = __hiloint2double((int)__funnelshift_r(lo, 0x3FFu, 12),
+                                          (int)__funnelshift_r(0x80000000u, lo, 12));
+        return fma(e.y, m, e.x);
+    }
+};
+template <> struct RotEntry<float> {
+    using type = float2;
+    static __device__ __forceinline__ float2 make(double x0, double x1, double shift, double scale) {
+        const double B = (x1 - x0) * scale, A = (x0 - shift) * scale;
+        // m = 1 + k 2^-23 with k = lo >> 9; the half-step 2^-24 centres r within 2^-24 of C3's r (C11)
+        return make_float2((float)(A - B + B * 5.9604644775390625e-08), (float)B);
+    }
+    static __device__ __forceinline__ float u(float2 e, uint32_t lo) {
+        const float m = __uint_as_float(__funnelshift_r(lo, 0x7Fu, 9));
+        return fmaf(e.y, m, e.x);
+    }
+};
+
+struct RotArgs {
+    const double* edges;            // device, [DIM][n_bins+1]
+    double* partials;               // device, [gridDim.x][4 + DIM*n_bins]
+    unsigned long long first_event, count;
+    uint32_t key0, key1, iteration;
+    int n_bins;
+    double post_scale;              // v = f_u * prod_j B_j * post_scale
+    double fin0;                    // integrand finish constant
+    double shift[VEGAS_MAX_DIM], scale[VEGAS_MAX_DIM];
+};
+
+constexpr int kRotThreads = 512;
+constexpr int kRotMinBlocks = 2;     // 64 registers per thread
+
+__host__ __device__ constexpr int rot_groups(int r) { return r >= 3 ? 4 : r; }   // dims in block -> lane groups
+
+// byte offset of (slot 0, this lane's copy) inside a table row, for a block with G lane groups;
+// the offset for slot s is this value ^ (s << (7 - log2 G)).  ENTRY = sizeof(table entry) (16 or 8).
+template <int G, int ENTRY>
+__device__ __forceinline__ uint32_t rot_table_off0(int lane) {
+    const int p = lane & 7, b3 = (lane >> 3) & 1;
+    constexpr int LG = (G == 4) ? 2 : (G == 2) ? 1 : 0;
+    const int gamma = p >> (3 - LG), tc = p & ((8 >> LG) - 1);
+    if (ENTRY == 16) return (uint32_t)(gamma * (128 >> LG) + tc * 16);
+    return (uint32_t)(gamma * (128 >> LG) + (tc + (8 >> LG) * b3) * 8);     // 8-byte entries: half-warp phases
+}
+template <int G>
+__device__ __forceinline__ uint32_t rot_hist_off0(int lane) {
+    const int p = lane & 7, b3 = (lane >> 3) & 1, b4 = lane >> 4;
+    constexpr int LG = (G == 4) ? 2 : (G == 2) ? 1 : 0;
+    const int gamma = p >> (3 - LG), tc = p & ((8 >> LG) - 1);
+    return (uint32_t)(b4 * 128 + gamma * (128 >> LG) + (tc + (8 >> LG) * b3) * 8);
+}
+template <int G>
+__device__ __forceinline__ int rot_gamma(int lane) {
+    constexpr int LG = (G == 4) ? 2 : (G == 2) ? 1 : 0;
+    return (lane & 7) >> (3 - LG);
+}
+
+template <int FID, typename T, int DIM>
+__global__ void __launch_bounds__(kRotThreads, kRotMinBlocks)
+k_iterate_rot(const __grid_constant__ RotArgs a) {
+    using E = RotEntry<T>;
+    using T2 = typename E::type;
+    constexpr int NBLK = (DIM + 3) / 4;
+    constexpr int R = DIM - 4 * (NBLK - 1);               // dimensions in the last block, 1..4
+    constexpr int GL = rot_groups(R);
+    constexpr int ENTRY = (int)sizeof(T2);
+    extern __shared__ __align__(256) unsigned char smem_rot[];
+    const int nb = a.n_bins;
+    const int rows = NBLK * nb;
+    unsigned char* table = smem_rot;                           // rows x 128 B
+    unsigned char* hist = smem_rot + (size_t)rows * 128;       // rows x 256 B
+    dd* red = reinterpret_cast<dd*>(hist + (size_t)rows * 256);
+
+    // ---- prologue: table from the master grid, zero histogram
+    for (int idx = threadIdx.x; idx < rows * (128 / ENTRY); idx += blockDim.x) {
+        const int row = idx / (128 / ENTRY), e = idx - row * (128 / ENTRY);   // entry e of the row
+        const int blk = row / nb, b = row - blk * nb;
+        const int G = (blk < NBLK - 1) ? 4 : GL;
+        const int slot = e / ((128 / ENTRY) / G);
+        const int j = 4 * blk + slot;
+        T2 ent = T2{};
+        if (j < DIM) {
+            const double* X = a.edges + (size_t)j * (nb + 1);
+            ent = E::make(X[b], X[b + 1], a.shift[j], a.scale[j]);
+        }
+        reinterpret_cast<T2*>(table)[idx] = ent;
+    }
+    for (int idx = threadIdx.x; idx < rows * 32; idx += blockDim.x) reinterpret_cast<double*>(hist)[idx] = 0.0;
+    __syncthreads();
+
+    const int lane = threadIdx.x & 31;
+    const uint32_t toff4 = rot_table_off0<4, ENTRY>(lane), hoff4 = rot_hist_off0<4>(lane);
+    const uint32_t toffL = rot_table_off0<GL, ENTRY>(lane), hoffL = rot_hist_off0<GL>(lane);
+    const int gamma4 = rot_gamma<4>(lane), gammaL = rot_gamma<GL>(lane);
+    const PhiloxKey ks = philox_key_schedule(a.key0, a.key1);
+    const T fin0 = (T)a.fin0;
+
+    double s1 = 0.0, c1 = 0.0, s2 = 0.0, c2 = 0.0;
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long q = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; q < a.count; q += stride) {
+        const unsigned long long ev = a.first_event + q;
+        const uint32_t e_lo = (uint32_t)ev, e_hi = (uint32_t)(ev >> 32);
+        IntegrandU<FID, T> f;
+        f.begin();
+        T jac = (T)1;
+        uint32_t packed[NBLK];
+#pragma unroll
+        for (int blk = 0; blk < NBLK; ++blk) {
+            const bool last = (blk == NBLK - 1);
+            const int G = last ? GL : 4;
+            const int SH = (G == 4) ? 5 : (G == 2) ? 6 : 7;             // slot -> byte offset shift
+            const int NSUB = last ? ((R == 3) ? 4 : R) : 4;             // sub-steps of this block
+            const uint32_t toff = last ? toffL : toff4;
+            const int gamma = last ? gammaL : gamma4;
+            uint32_t w[4];
+            philox4x32_10((uint32_t)blk, a.iteration, e_lo, e_hi, ks, w);
+            // w'[i] = w[gamma ^ i]
+            if (G == 4) {
+                const bool g1 = gamma & 1, g2 = gamma & 2;
+                const uint32_t t0 = g1 ? w[1] : w[0], t1 = g1 ? w[0] : w[1], t2 = g1 ? w[3] : w[2], t3 = g1 ? w[2] : w[3];
+                w[0] = g2 ? t2 : t0; w[1] = g2 ? t3 : t1; w[2] = g2 ? t0 : t2; w[3] = g2 ? t1 : t3;
+            } else if (G == 2) {
+                const bool g1 = gamma & 1;
+                const uint32_t t0 = g1 ? w[1] : w[0], t1 = g1 ? w[0] : w[1];
+                w[0] = t0; w[1] = t1;
+            }
+            const unsigned char* trow = table + (size_t)(blk * nb) * 128;
+            uint32_t pk = 0;
+#pragma unroll
+            for (int i = 0; i < NSUB; ++i) {
+                const bool active = !(last && R == 3) || ((gamma ^ i) < 3);
+                if (active) {
+                    uint32_t b, lo;
+                    split_word(w[i], (uint32_t)nb, b, lo);
+                    const T2 ent = *reinterpret_cast<const T2*>(trow + (b * 128u + (toff ^ (uint32_t)(i << SH))));
+                    const T u = E::u(ent, lo);
+                    jac *= ent.y;
+                    f.dim(u);
+                    pk |= b << (8 * i);
+                }
+            }
+            packed[blk] = pk;
+        }
+        const double v = (double)(f.finish(fin0) * jac) * a.post_scale;
+        const double v2 = v * v;
+        kahan_add(s1, c1, v);
+        kahan_add(s2, c2, v2);
+#pragma unroll
+        for (int blk = 0; blk < NBLK; ++blk) {
+            const bool last = (blk == NBLK - 1);
+            const int G = last ? GL : 4;
+            const int SH = (G == 4) ? 5 : (G == 2) ? 6 : 7;
+            const int NSUB = last ? ((R == 3) ? 4 : R) : 4;
+            const uint32_t hoff = last ? hoffL : hoff4;
+            const int gamma = last ? gammaL : gamma4;
+            unsigned char* hrow = hist + (size_t)(blk * nb) * 256;
+#pragma unroll
+            for (int i = 0; i < NSUB; ++i) {
+                const bool active = !(last && R == 3) || ((gamma ^ i) < 3);
+                if (active) {
+                    const uint32_t b256 = __byte_perm(packed[blk], 0, 0x4404 | (i << 4));   // byte i -> bits 8..15
+                    atomicAdd(reinterpret_cast<double*>(hrow + (b256 + (hoff ^ (uint32_t)(i << SH)))), v2);
+                }
+            }
+        }
+    }
+
+    // ---- S5: warp shuffle -> CTA -> this CTA's partial (accumulated over the launches of an iteration)
+    dd t1 = dd_warp_sum(fast_two_sum(s1, -c1));
+    dd t2 = dd_warp_sum(fast_two_sum(s2, -c2));
+    const int warp = threadIdx.x >> 5, nwarps = (blockDim.x + 31) >> 5;
+    if (lane == 0) { red[2 * warp] = t1; red[2 * warp + 1] = t2; }
+    __syncthreads();
+    double* part = a.partials + (size_t)blockIdx.x * (4 + DIM * nb);
+    if (warp == 0) {
+        t1 = (lane < nwarps) ? red[2 * lane] : dd{0.0, 0.0};
+        t2 = (lane < nwarps) ? red[2 * lane + 1] : dd{0.0, 0.0};
+        t1 = dd_warp_sum(t1);
+        t2 = dd_warp_sum(t2);
+        if (lane == 0) {
+            t1 = dd_add(t1, dd{part[0], part[1]});
+            t2 = dd_add(t2, dd{part[2], part[3]});
+            part[0] = t1.hi; part[1] = t1.lo; part[2] = t2.hi; part[3] = t2.lo;
+        }
+    }
+    // ---- S6: merge the copies of every (dimension, bin) in fixed order, one pass per CTA
+    for (int idx = threadIdx.x; idx < DIM * nb; idx += blockDim.x) {
+        const int j = idx / nb, b = idx - j * nb;
+        const int blk = j >> 2, slot = j & 3;
+        const int G = (blk < NBLK - 1) ? 4 : GL;
+        const int per = 16 / G;                                   // copies per half-warp row half
+        const double* row = reinterpret_cast<const double*>(hist + (size_t)(blk * nb + b) * 256);
+        double h = 0.0;
+        for (int half = 0; half < 2; ++half)
+            for (int c = 0; c < per; ++c) h += row[half * 16 + slot * per + c];
+        part[4 + idx] += h;
+    }
+}
+
+inline size_t rot_shared_bytes(int dim, int n_bins) {
+    const size_t rows = (size_t)((dim + 3) / 4) * n_bins;
+    return rows * (128 + 256) + 2 * sizeof(dd) * (kRotThreads / 32);
+}
+
+// one translation unit per (FID, T) instantiates DIM = 1..32 (vegas_rot_inst.cu)
+template <int FID, typename T>
+cudaError_t launch_iterate_rot(int dim, const RotArgs& a, int blocks, int threads, size_t shmem, cudaStream_t st);
+
+}  // namespace vegas

@@ -8,6 +8,7 @@
 #include "vegas_kernels.h"
 
 #include "vegas_device.cuh"
+#include "vegas_iterate_rot.cuh"
 
 namespace vegas {
 
@@ -56,7 +57,7 @@ template <> struct MapConst<float> {
 // (one byte per dimension) live in registers.
 // ---------------------------------------------------------------------------------------------
 template <int FID, typename T, int NBLK>
-__global__ void __launch_bounds__(kIterMaxThreads, 1)
+__global__ void __launch_bounds__(kIterMaxThreads, kIterMinBlocks)
 k_iterate(const IterArgs a, const __grid_constant__ FParams<T> fp) {
     using T2 = typename Vec2<T>::type;
     extern __shared__ __align__(16) unsigned char smem[];
@@ -290,6 +291,39 @@ __global__ void k_debug(const DebugArgs a, const __grid_constant__ FParams<T> fp
     a.fJ[q] = (double)(f.finish(fp) * jac) * a.jac_scale;
 }
 
+// K4 for the fast path: u_j and f*J through the device functions of k_iterate_rot (RotEntry,
+// IntegrandU); x_j, which that kernel never forms, is reported from the plain map (C4).
+template <int FID, typename T>
+__global__ void k_debug_rot(const __grid_constant__ DebugArgs a) {
+    using E = RotEntry<T>;
+    const uint32_t q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= a.count) return;
+    const unsigned long long e = a.first_event + q;
+    const int dim = a.dim, nb = a.n_bins;
+    const PhiloxKey ks = philox_key_schedule(a.key0, a.key1);
+    IntegrandU<FID, T> f;
+    f.begin();
+    T jac = (T)1;
+    uint32_t w[4] = {0, 0, 0, 0};
+    for (int j = 0; j < dim; ++j) {
+        if ((j & 3) == 0) philox4x32_10((uint32_t)(j >> 2), a.iteration, (uint32_t)e, (uint32_t)(e >> 32), ks, w);
+        const uint32_t word = (j & 3) == 0 ? w[0] : (j & 3) == 1 ? w[1] : (j & 3) == 2 ? w[2] : w[3];
+        uint32_t b, lo;
+        split_word(word, (uint32_t)nb, b, lo);
+        const double* X = a.edges + (size_t)j * (nb + 1);
+        const typename E::type ent = E::make(X[b], X[b + 1], a.shift[j], a.scale[j]);
+        jac *= ent.y;
+        f.dim(E::u(ent, lo));
+        a.words[(size_t)q * dim + j] = word;
+        a.bins[(size_t)q * dim + j] = (int32_t)b;
+        a.x[(size_t)q * dim + j] = (sizeof(T) == 8) ? fma(X[b + 1] - X[b], offset_f64(lo), X[b])
+                                                     : (double)fmaf((float)(X[b + 1] - X[b]),
+                                                                    offset_f32_scaled(lo, 5.9604644775390625e-08f, 2.98023223876953125e-08f),
+                                                                    (float)X[b]);
+    }
+    a.fJ[q] = (double)(f.finish((T)a.fin0) * jac) * a.post_scale;
+}
+
 // =============================================================================================
 // Launchers
 // =============================================================================================
@@ -391,8 +425,23 @@ static cudaError_t launch_debug_t(int fid, const DebugArgs& a, const FParams<T>&
     return cudaGetLastError();
 }
 
-cudaError_t launch_debug(int fid, int precision, const DebugArgs& a, const double* derived_params,
+template <typename T>
+static cudaError_t launch_debug_rot_t(int fid, const DebugArgs& a, cudaStream_t st) {
+    const int threads = 128;
+    const int blocks = (int)((a.count + threads - 1) / threads);
+    switch (fid) {
+    case VEGAS_F_CONST: k_debug_rot<VEGAS_F_CONST, T><<<blocks, threads, 0, st>>>(a); break;
+    case VEGAS_F_GAUSS: k_debug_rot<VEGAS_F_GAUSS, T><<<blocks, threads, 0, st>>>(a); break;
+    case VEGAS_F_GENZ_PRODUCT_PEAK: k_debug_rot<VEGAS_F_GENZ_PRODUCT_PEAK, T><<<blocks, threads, 0, st>>>(a); break;
+    default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_debug(int fid, int precision, bool rot_path, const DebugArgs& a, const double* derived_params,
                          cudaStream_t st) {
+    if (rot_path)
+        return precision == VEGAS_FP64 ? launch_debug_rot_t<double>(fid, a, st) : launch_debug_rot_t<float>(fid, a, st);
     if (precision == VEGAS_FP64) {
         FParams<double> fp;
         convert_params(derived_params, fp);

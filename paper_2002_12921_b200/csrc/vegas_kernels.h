@@ -8,7 +8,14 @@
 
 namespace vegas {
 
-constexpr int kIterMaxThreads = 512;   // __launch_bounds__ of K1: up to 128 registers per thread
+#ifndef VEGAS_ITER_MAX_THREADS
+#define VEGAS_ITER_MAX_THREADS 512
+#endif
+#ifndef VEGAS_ITER_MIN_BLOCKS
+#define VEGAS_ITER_MIN_BLOCKS 1
+#endif
+constexpr int kIterMaxThreads = VEGAS_ITER_MAX_THREADS;   // __launch_bounds__ of K1
+constexpr int kIterMinBlocks = VEGAS_ITER_MIN_BLOCKS;
 
 struct IterArgs {
     const double* edges;            // device, [dim][n_bins+1] master grid
@@ -33,6 +40,9 @@ struct DebugArgs {
     int32_t* bins;
     double* x;
     double* fJ;
+    // fast ("rotated") path only: the affine map and constants of vegas_iterate_rot.cuh
+    double post_scale, fin0;
+    double shift[VEGAS_MAX_DIM], scale[VEGAS_MAX_DIM];
 };
 
 size_t iterate_shared_bytes(int dim, int n_bins, int precision, int table_copies, int hist_copies);
@@ -43,7 +53,7 @@ cudaError_t launch_reduce(const double* partials, int n_parts, int n_tot, double
 cudaError_t launch_finalize(const double* totals, double n_events, double* result, cudaStream_t st);
 cudaError_t launch_refine(double* edges, const double* hist, int dim, int n_bins, double alpha, int* status,
                           cudaStream_t st);
-cudaError_t launch_debug(int fid, int precision, const DebugArgs& a, const double* derived_params,
+cudaError_t launch_debug(int fid, int precision, bool rot_path, const DebugArgs& a, const double* derived_params,
                          cudaStream_t st);
 
 }  // namespace vegas

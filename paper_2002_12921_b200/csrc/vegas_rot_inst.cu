@@ -1,0 +1,44 @@
+// vegas_rot_inst.cu -- instantiates k_iterate_rot<ROT_FID, T, DIM> for DIM = 1..32.
+// Compiled once per (ROT_FID, ROT_FP) pair by build.py so that the pairs build in parallel.
+#include "vegas_iterate_rot.cuh"
+
+#ifndef ROT_FID
+#error "compile with -DROT_FID=<integrand id> -DROT_FP=<64|32>"
+#endif
+
+namespace vegas {
+
+#if ROT_FP == 64
+using RT = double;
+#else
+using RT = float;
+#endif
+
+template <int DIM>
+static cudaError_t go(const RotArgs& a, int blocks, int threads, size_t shmem, cudaStream_t st) {
+    auto kern = k_iterate_rot<ROT_FID, RT, DIM>;
+    static size_t configured = 0;
+    if (shmem > configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem);
+        if (e != cudaSuccess) return e;
+        configured = shmem;
+    }
+    kern<<<blocks, threads, shmem, st>>>(a);
+    return cudaGetLastError();
+}
+
+template <>
+cudaError_t launch_iterate_rot<ROT_FID, RT>(int dim, const RotArgs& a, int blocks, int threads, size_t shmem,
+                                            cudaStream_t st) {
+    switch (dim) {
+#define CASE(D) case D: return go<D>(a, blocks, threads, shmem, st);
+        CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
+        CASE(9) CASE(10) CASE(11) CASE(12) CASE(13) CASE(14) CASE(15) CASE(16)
+        CASE(17) CASE(18) CASE(19) CASE(20) CASE(21) CASE(22) CASE(23) CASE(24)
+        CASE(25) CASE(26) CASE(27) CASE(28) CASE(29) CASE(30) CASE(31) CASE(32)
+#undef CASE
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace vegas

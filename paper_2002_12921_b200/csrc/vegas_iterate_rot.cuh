@@ -58,8 +58,8 @@ template <> struct RotEntry<double> {
         return make_double2(A - B, B);                              // u = (A - B) + B m,  m = 1 + r
     }
     static __device__ __forceinline__ double u(double2 e, uint32_t lo) {
-        const double m = __hiloint2double((int)__funnelshift_r(lo, 0x3FFu, 12),
-                                          (int)__funnelshift_r(0x80000000u, lo, 12));
+        // hi word: (0x3FF : lo) >> 12 (one funnel shift); lo word: lo * 2^20 + 2^19 (one IMAD, FMA pipe)
+        const double m = __hiloint2double((int)__funnelshift_r(lo, 0x3FFu, 12), (int)(lo * 0x100000u + 0x80000u));
         return fma(e.y, m, e.x);
     }
 };
@@ -75,6 +75,19 @@ template <> struct RotEntry<float> {
         return fmaf(e.y, m, e.x);
     }
 };
+
+// 32-bit shared-window addressing: one register per address, no generic-to-shared conversion
+template <typename T2> __device__ __forceinline__ T2 lds_entry(uint32_t addr);
+template <> __device__ __forceinline__ double2 lds_entry<double2>(uint32_t addr) {
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+template <> __device__ __forceinline__ float2 lds_entry<float2>(uint32_t addr) {
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+    return v;
+}
 
 struct RotArgs {
     const double* edges;            // device, [DIM][n_bins+1]
@@ -149,6 +162,7 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     __syncthreads();
 
     const int lane = threadIdx.x & 31;
+    const uint32_t tbase = (uint32_t)__cvta_generic_to_shared(table);
     const uint32_t toff4 = rot_table_off0<4, ENTRY>(lane), hoff4 = rot_hist_off0<4>(lane);
     const uint32_t toffL = rot_table_off0<GL, ENTRY>(lane), hoffL = rot_hist_off0<GL>(lane);
     const int gamma4 = rot_gamma<4>(lane), gammaL = rot_gamma<GL>(lane);
@@ -184,19 +198,28 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
                 const uint32_t t0 = g1 ? w[1] : w[0], t1 = g1 ? w[0] : w[1];
                 w[0] = t0; w[1] = t1;
             }
-            const unsigned char* trow = table + (size_t)(blk * nb) * 128;
-            uint32_t pk = 0;
+            // the block's table reads are issued together, then consumed (their latency overlaps)
+            const uint32_t tblk = tbase + (uint32_t)(blk * nb) * 128u;
+            uint32_t lo[4], pk = 0;
+            T2 ent[4];
+#pragma unroll
+            for (int i = 0; i < NSUB; ++i) {
+                const bool active = !(last && R == 3) || ((gamma ^ i) < 3);
+                uint32_t b = 0;
+                lo[i] = 0;
+                ent[i] = T2{};
+                if (active) {
+                    split_word(w[i], (uint32_t)nb, b, lo[i]);
+                    ent[i] = lds_entry<T2>(tblk + (b * 128u + (toff ^ (uint32_t)(i << SH))));
+                    pk |= b << (8 * i);
+                }
+            }
 #pragma unroll
             for (int i = 0; i < NSUB; ++i) {
                 const bool active = !(last && R == 3) || ((gamma ^ i) < 3);
                 if (active) {
-                    uint32_t b, lo;
-                    split_word(w[i], (uint32_t)nb, b, lo);
-                    const T2 ent = *reinterpret_cast<const T2*>(trow + (b * 128u + (toff ^ (uint32_t)(i << SH))));
-                    const T u = E::u(ent, lo);
-                    jac *= ent.y;
-                    f.dim(u);
-                    pk |= b << (8 * i);
+                    jac *= ent[i].y;
+                    f.dim(E::u(ent[i], lo[i]));
                 }
             }
             packed[blk] = pk;
@@ -213,13 +236,17 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
             const int NSUB = last ? ((R == 3) ? 4 : R) : 4;
             const uint32_t hoff = last ? hoffL : hoff4;
             const int gamma = last ? gammaL : gamma4;
-            unsigned char* hrow = hist + (size_t)(blk * nb) * 256;
+            // S6: one shared-memory atomicAdd per dimension.  ptxas lowers it to LDS + ATOMS.CAST.SPIN, the
+            // fast hardware path; an explicit value-returning atom.shared.cas.b64 (ATOMS.CAS.64) measured
+            // 3-18x slower (profiles/r01_k_iterate_rot.md).  No two lanes of the warp share a word, so the
+            // spin only retries when another warp hit the same word in between.
+            unsigned char* hblk = hist + (size_t)(blk * nb) * 256;
 #pragma unroll
             for (int i = 0; i < NSUB; ++i) {
                 const bool active = !(last && R == 3) || ((gamma ^ i) < 3);
                 if (active) {
                     const uint32_t b256 = __byte_perm(packed[blk], 0, 0x4404 | (i << 4));   // byte i -> bits 8..15
-                    atomicAdd(reinterpret_cast<double*>(hrow + (b256 + (hoff ^ (uint32_t)(i << SH)))), v2);
+                    atomicAdd(reinterpret_cast<double*>(hblk + (b256 + (hoff ^ (uint32_t)(i << SH)))), v2);
                 }
             }
         }

@@ -51,6 +51,18 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_ubench() -> str:
+    """The step-0 pipe microbenchmark (csrc/ubench_pipes.cu), a standalone binary; not part of the library."""
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    out = os.path.join(_HERE, "ubench_pipes.bin")
+    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+                    "-cudart", "static", "-o", out, os.path.join(CSRC, "ubench_pipes.cu")], check=True)
+    return out
+
+
 if __name__ == "__main__":
     import sys
-    print(build(force=True, verbose="-v" in sys.argv))
+    if "--ubench" in sys.argv:
+        print(build_ubench())
+    else:
+        print(build(force=True, verbose="-v" in sys.argv))

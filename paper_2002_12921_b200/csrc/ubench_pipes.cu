@@ -1,0 +1,289 @@
+// ubench_pipes.cu -- step-0 pipe microbenchmarks (SURVEY.md section 7 step 0, section 8(d) "machine model"):
+// the denominators of the ALU / shared-memory rooflines that bench.py reports, measured on the box.
+// Standalone program (no torch, no library code):   python -m paper_2002_12921_b200.build --ubench
+//                                                   paper_2002_12921_b200/ubench_pipes.bin [> gpurun_out/ubench.txt]
+// Every test launches one 1024-thread CTA per SM (8 warps per scheduler), each thread runs ITER rounds of
+// UNR independent dependency chains of the instruction under test, and reports
+//     lanes/clk/SM = threads * ITER * UNR * ops / (clock64 cycles of the CTA)
+// plus the SM clock held (cycles / globaltimer).  Shared-memory tests report SM clocks per warp-wide access.
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <stdlib.h>
+
+#define CHECK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { \
+    fprintf(stderr, "%s: %s\n", #x, cudaGetErrorString(e_)); exit(1); } } while (0)
+
+constexpr int THREADS = 1024, ITER = 4096, UNR = 8;
+
+struct Stamp { long long cycles; unsigned long long ns; };
+
+__device__ __forceinline__ unsigned long long gtime() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
+}
+
+#define BENCH_PROLOG  __syncthreads(); const unsigned long long g0 = gtime(); const long long c0 = clock64();
+#define BENCH_EPILOG(sinkexpr) const long long c1 = clock64(); const unsigned long long g1 = gtime(); \
+    if ((sinkexpr) == 0x12345678) out[0].cycles = 0; __syncthreads(); \
+    if (threadIdx.x == 0) { out[blockIdx.x].cycles = c1 - c0; out[blockIdx.x].ns = g1 - g0; }
+
+__global__ void __launch_bounds__(THREADS) k_ffma(Stamp* out, float a, float b) {
+    float x[UNR];
+    for (int u = 0; u < UNR; ++u) x[u] = threadIdx.x + u;
+    BENCH_PROLOG
+    for (int i = 0; i < ITER; ++i)
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) x[u] = fmaf(x[u], a, b);
+    float s = 0; for (int u = 0; u < UNR; ++u) s += x[u];
+    BENCH_EPILOG(__float_as_int(s))
+}
+
+__global__ void __launch_bounds__(THREADS) k_dfma(Stamp* out, double a, double b) {
+    double x[UNR];
+    for (int u = 0; u < UNR; ++u) x[u] = threadIdx.x + u;
+    BENCH_PROLOG
+    for (int i = 0; i < ITER; ++i)
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) x[u] = fma(x[u], a, b);
+    double s = 0; for (int u = 0; u < UNR; ++u) s += x[u];
+    BENCH_EPILOG(__double2loint(s))
+}
+
+// 32x32 -> 64 product with both halves consumed: the Philox round multiply (IMAD.WIDE.U32)
+__global__ void __launch_bounds__(THREADS) k_imad_wide(Stamp* out, uint32_t m) {
+    uint32_t x[UNR];
+    for (int u = 0; u < UNR; ++u) x[u] = threadIdx.x * 2654435761u + u;
+    BENCH_PROLOG
+    for (int i = 0; i < ITER; ++i)
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) {
+            const uint64_t p = (uint64_t)x[u] * m;
+            x[u] = (uint32_t)(p >> 32) ^ (uint32_t)p;     // + one LOP3 per multiply
+        }
+    uint32_t s = 0; for (int u = 0; u < UNR; ++u) s ^= x[u];
+    BENCH_EPILOG(s)
+}
+
+__global__ void __launch_bounds__(THREADS) k_imad_lo(Stamp* out, uint32_t m, uint32_t c) {
+    uint32_t x[UNR];
+    for (int u = 0; u < UNR; ++u) x[u] = threadIdx.x * 2654435761u + u;
+    BENCH_PROLOG
+    for (int i = 0; i < ITER; ++i)
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) x[u] = x[u] * m + c;
+    uint32_t s = 0; for (int u = 0; u < UNR; ++u) s ^= x[u];
+    BENCH_EPILOG(s)
+}
+
+__global__ void __launch_bounds__(THREADS) k_imad_hi(Stamp* out, uint32_t m) {
+    uint32_t x[UNR];
+    for (int u = 0; u < UNR; ++u) x[u] = threadIdx.x * 2654435761u + u;
+    BENCH_PROLOG
+    for (int i = 0; i < ITER; ++i)
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) x[u] = __umulhi(x[u], m) + 0x9E3779B9u;
+    uint32_t s = 0; for (int u = 0; u < UNR; ++u) s ^= x[u];
+    BENCH_EPILOG(s)
+}
+
+__global__ void __launch_bounds__(THREADS) k_lop3(Stamp* out, uint32_t a, uint32_t b) {
+    uint32_t x[UNR];
+    for (int u = 0; u < UNR; ++u) x[u] = threadIdx.x * 2654435761u + u;
+    BENCH_PROLOG
+    for (int i = 0; i < ITER; ++i)
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) x[u] = (x[u] ^ a ^ b) + 1u;   // LOP3 + IADD
+    uint32_t s = 0; for (int u = 0; u < UNR; ++u) s ^= x[u];
+    BENCH_EPILOG(s)
+}
+
+// u32 -> fp64 conversion (I2F.F64.U32) followed by one DADD that keeps the chain alive
+__global__ void __launch_bounds__(THREADS) k_i2f64(Stamp* out, uint32_t a) {
+    uint32_t x[UNR];
+    for (int u = 0; u < UNR; ++u) x[u] = threadIdx.x * 2654435761u + u;
+    BENCH_PROLOG
+    for (int i = 0; i < ITER; ++i)
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) {
+            const double d = (double)x[u];
+            x[u] = (uint32_t)__double2hiint(d) ^ a ^ x[u];
+        }
+    uint32_t s = 0; for (int u = 0; u < UNR; ++u) s ^= x[u];
+    BENCH_EPILOG(s)
+}
+
+// m = 1 + lo 2^-32 built in the mantissa by integer ops (the kernel's current form: SHF + IMAD/LOP)
+__global__ void __launch_bounds__(THREADS) k_mant64(Stamp* out, uint32_t a) {
+    uint32_t x[UNR];
+    for (int u = 0; u < UNR; ++u) x[u] = threadIdx.x * 2654435761u + u;
+    BENCH_PROLOG
+    for (int i = 0; i < ITER; ++i)
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) {
+            const uint32_t hi = __funnelshift_r(x[u], 0x3FFu, 12), lo = (x[u] << 20) | 0x80000u;
+            x[u] = hi ^ lo ^ a;
+        }
+    uint32_t s = 0; for (int u = 0; u < UNR; ++u) s ^= x[u];
+    BENCH_EPILOG(s)
+}
+
+// ---- shared memory: one access pattern per kernel; rows x 32 lane-private columns (conflict-free) ----
+constexpr int SM_ITER = 2048;
+__device__ __forceinline__ uint32_t lcg(uint32_t& s) { s = s * 1664525u + 1013904223u; return s >> 8; }
+
+// random LDS.128 from a (rows x 8 copies x 16 B) table: lane l reads copy l&7 -> each quarter-warp wavefront is conflict-free
+__global__ void __launch_bounds__(THREADS) k_lds128(Stamp* out, int rows) {
+    extern __shared__ __align__(16) unsigned char sm[];
+    double2* t = reinterpret_cast<double2*>(sm);
+    for (int i = threadIdx.x; i < rows * 8; i += THREADS) t[i] = make_double2(i, 1.0);
+    uint32_t s = threadIdx.x * 747796405u + 1u;
+    const int lane = threadIdx.x & 31;
+    double acc = 0;
+    BENCH_PROLOG
+    for (int i = 0; i < SM_ITER; ++i) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const uint32_t r = (lcg(s) * (uint32_t)rows) >> 24;
+            const double2 e = t[r * 8 + (lane & 7)];
+            acc += e.x * e.y;
+        }
+    }
+    BENCH_EPILOG(__double2loint(acc))
+}
+
+// histogram update, one fp64 word per lane per update, lane-private columns (rows x 32 x 8 B); per-warp regions
+// when `priv` (exclusive owner: plain read-modify-write is race-free), else one region for the CTA.
+template <int MODE>   // 0 = atomicAdd(double) (CAS loop), 1 = plain LDS/DADD/STS
+__global__ void __launch_bounds__(THREADS) k_hist(Stamp* out, int rows, int regions) {
+    extern __shared__ __align__(16) unsigned char sm[];
+    double* h = reinterpret_cast<double*>(sm);
+    for (int i = threadIdx.x; i < rows * 32 * regions; i += blockDim.x) h[i] = 0.0;
+    uint32_t s = threadIdx.x * 747796405u + 1u;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double* mine = h + (size_t)(warp % regions) * rows * 32 + lane;
+    BENCH_PROLOG
+    for (int i = 0; i < SM_ITER; ++i) {
+        uint32_t r[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) r[u] = ((lcg(s) * (uint32_t)rows) >> 24) * 32u;
+        if (MODE == 0) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) atomicAdd(mine + r[u], 1.0);
+        } else {
+            // the four words may coincide (same lane, same row): merge duplicates in registers so that the
+            // pipelined loads/stores stay exact
+            double v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) v[u] = mine[r[u]];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                v[u] += 1.0;
+#pragma unroll
+                for (int w = 0; w < u; ++w) if (r[w] == r[u]) v[u] = v[w] + 1.0;
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) mine[r[u]] = v[u];
+        }
+    }
+    BENCH_EPILOG((int)s)
+}
+
+// token ring of named barriers: warp w waits on barrier 1+w (bar.sync, 64 threads), does `work` dependent DADDs,
+// signals barrier 1+((w+1) % W) (bar.arrive).  Reports SM clocks per token hand-off.
+__global__ void k_ring(Stamp* out, int work, double a) {
+    const int warp = threadIdx.x >> 5, W = blockDim.x >> 5;
+    double x = threadIdx.x;
+    BENCH_PROLOG
+    for (int i = 0; i < SM_ITER; ++i) {
+        if (!(warp == 0 && i == 0)) asm volatile("bar.sync %0, 64;" ::"r"(1 + warp) : "memory");
+        for (int k = 0; k < work; ++k) x = fma(x, a, 1.0);
+        asm volatile("bar.arrive %0, 64;" ::"r"(1 + (warp + 1) % W) : "memory");
+    }
+    if (warp == 0) asm volatile("bar.sync %0, 64;" ::"r"(1) : "memory");
+    BENCH_EPILOG(__double2loint(x))
+}
+
+static Stamp* d_out;
+static int n_sm;
+
+static void report_alu(const char* name, int ops_per_chain_step, int threads = THREADS) {
+    Stamp h[1024];
+    CHECK(cudaDeviceSynchronize());
+    CHECK(cudaMemcpy(h, d_out, sizeof(Stamp) * n_sm, cudaMemcpyDeviceToHost));
+    double cyc = 0, ns = 0;
+    for (int i = 0; i < n_sm; ++i) { cyc += (double)h[i].cycles; ns += (double)h[i].ns; }
+    cyc /= n_sm; ns /= n_sm;
+    printf("%-34s %8.2f lanes/clk/SM   (%.0f cycles, SM clock %.0f MHz)\n", name,
+           (double)threads * ITER * UNR * ops_per_chain_step / cyc, cyc, 1e3 * cyc / ns);
+}
+
+static void report_smem(const char* name, double warp_accesses_per_thread, int threads) {
+    Stamp h[1024];
+    CHECK(cudaDeviceSynchronize());
+    CHECK(cudaMemcpy(h, d_out, sizeof(Stamp) * n_sm, cudaMemcpyDeviceToHost));
+    double cyc = 0, ns = 0;
+    for (int i = 0; i < n_sm; ++i) { cyc += (double)h[i].cycles; ns += (double)h[i].ns; }
+    cyc /= n_sm; ns /= n_sm;
+    printf("%-58s %7.2f clk per warp-wide access   (SM clock %.0f MHz)\n", name,
+           cyc / (warp_accesses_per_thread * (threads / 32)), 1e3 * cyc / ns);
+}
+
+int main() {
+    cudaDeviceProp prop;
+    CHECK(cudaGetDeviceProperties(&prop, 0));
+    n_sm = prop.multiProcessorCount;
+    printf("# %s, %d SMs, %zu KB shared/SM opt-in\n", prop.name, n_sm, prop.sharedMemPerBlockOptin >> 10);
+    CHECK(cudaMalloc(&d_out, sizeof(Stamp) * 1024));
+    for (int rep = 0; rep < 2; ++rep) {          // first pass warms clocks up
+        if (rep) printf("# ALU pipes: one 1024-thread CTA per SM, %d independent chains per thread\n", UNR);
+        k_ffma<<<n_sm, THREADS>>>(d_out, 1.0001f, 0.5f);              if (rep) report_alu("FFMA", 1);
+        k_dfma<<<n_sm, THREADS>>>(d_out, 1.0001, 0.5);                if (rep) report_alu("DFMA", 1);
+        k_imad_wide<<<n_sm, THREADS>>>(d_out, 0xD2511F53u);           if (rep) report_alu("IMAD.WIDE.U32 (+1 LOP3 each)", 1);
+        k_imad_lo<<<n_sm, THREADS>>>(d_out, 0xD2511F53u, 12345u);     if (rep) report_alu("IMAD (32-bit low)", 1);
+        k_imad_hi<<<n_sm, THREADS>>>(d_out, 0xD2511F53u);             if (rep) report_alu("IMAD.HI.U32 (+1 IADD each)", 1);
+        k_lop3<<<n_sm, THREADS>>>(d_out, 0x9E3779B9u, 0xBB67AE85u);   if (rep) report_alu("LOP3 + IADD pair", 2);
+        k_i2f64<<<n_sm, THREADS>>>(d_out, 0x55555555u);               if (rep) report_alu("I2F.F64.U32 (+1 LOP3 each)", 1);
+        k_mant64<<<n_sm, THREADS>>>(d_out, 0x55555555u);              if (rep) report_alu("mantissa build (SHF+LOP/IMAD+LOP3)", 1);
+    }
+    printf("# shared memory, random rows\n");
+    for (int rows : {50, 250}) {
+        char nm[128];
+        CHECK(cudaFuncSetAttribute(k_lds128, cudaFuncAttributeMaxDynamicSharedMemorySize, rows * 128));
+        k_lds128<<<n_sm, THREADS, rows * 128>>>(d_out, rows);
+        snprintf(nm, sizeof nm, "LDS.128 table gather, %d rows x 8 copies", rows);
+        report_smem(nm, SM_ITER * 4.0, THREADS);
+    }
+    CHECK(cudaFuncSetAttribute(k_hist<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+    CHECK(cudaFuncSetAttribute(k_hist<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+    for (int threads : {256, 512}) {
+        for (int rows : {50, 250}) {
+            char nm[128];
+            k_hist<0><<<n_sm, threads, rows * 256>>>(d_out, rows, 1);
+            snprintf(nm, sizeof nm, "fp64 atomicAdd (CAS loop), %d thr, %d rows, shared region", threads, rows);
+            report_smem(nm, SM_ITER * 4.0, threads);
+        }
+    }
+    for (int warps : {3, 6, 12}) {      // exclusive owners: one region per warp, 50 rows x 256 B = 12.5 KB each
+        char nm[128];
+        k_hist<1><<<n_sm, warps * 32, warps * 50 * 256>>>(d_out, 50, warps);
+        snprintf(nm, sizeof nm, "plain LDS/DADD/STS x4, %d warps, exclusive regions", warps);
+        report_smem(nm, SM_ITER * 4.0, warps * 32);
+    }
+    printf("# named-barrier token ring (bar.sync / bar.arrive on 64 threads)\n");
+    for (int W : {2, 4, 12}) {
+        for (int work : {0, 32}) {
+            char nm[128];
+            k_ring<<<n_sm, W * 32>>>(d_out, work, 1.0000001);
+            snprintf(nm, sizeof nm, "ring of %d warps, %d dependent DFMA inside", W, work);
+            Stamp h[1024];
+            CHECK(cudaDeviceSynchronize());
+            CHECK(cudaMemcpy(h, d_out, sizeof(Stamp) * n_sm, cudaMemcpyDeviceToHost));
+            double cyc = 0; for (int i = 0; i < n_sm; ++i) cyc += (double)h[i].cycles; cyc /= n_sm;
+            printf("%-58s %7.1f clk per hand-off\n", nm, cyc / ((double)SM_ITER * W));
+        }
+    }
+    CHECK(cudaFree(d_out));
+    return 0;
+}

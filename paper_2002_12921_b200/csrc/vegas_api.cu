@@ -6,6 +6,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -71,7 +72,7 @@ struct vegas_grid {
     bool params_set[4] = {true, false, false, false};
     double derived[4][VEGAS_MAX_PARAMS] = {};
     double user[4][VEGAS_MAX_PARAMS] = {};       // the caller's arrays as given to vegas_set_params
-    int cfg_blocks = 0, cfg_threads = 0, cfg_ct = 0, cfg_ch = 0;
+    int cfg_blocks = 0, cfg_threads = 0, cfg_ct = 0, cfg_ch = 0, cfg_ept = 0;
     int active_blocks = 0;          // CTAs whose partial slots the current iteration uses
     bool profiling = false;
     std::vector<cudaEvent_t> events;   // pairs (start, stop)
@@ -169,12 +170,13 @@ bool use_rot_path(const vegas_grid* g, int fid, int precision) {
     const bool kind = fid == VEGAS_F_CONST || fid == VEGAS_F_GAUSS ||
                       (fid == VEGAS_F_GENZ_PRODUCT_PEAK && precision == VEGAS_FP64);
     if (!kind) return false;
-    if (g->cfg_threads > vegas::kRotThreads) return false;
-    return vegas::rot_shared_bytes(g->dim, g->n_bins) <= g->smem_optin;
+    if (g->cfg_threads > vegas::kRotMaxThreads) return false;
+    return vegas::rot_shared_bytes(g->dim, g->n_bins, 1) <= g->smem_optin;
 }
 
 // shift_j, scale_j, post_scale, fin0 of the affine pre-composition (see vegas_iterate_rot.cuh)
-void rot_constants(const vegas_grid* g, int fid, double* shift, double* scale, double* post_scale, double* fin0) {
+void rot_constants(const vegas_grid* g, int fid, int precision, double* shift, double* scale, double* post_scale,
+                   double* fin0, double* jac_init) {
     const int dim = g->dim;
     const double nb = (double)g->n_bins;
     *post_scale = 1.0;
@@ -195,36 +197,53 @@ void rot_constants(const vegas_grid* g, int fid, double* shift, double* scale, d
         }
         *post_scale = ps;
     }
+    // fp64 table entries carry 2^-32 per dimension (RotEntry<double>): start the running Jacobian product at
+    // 2^(32 floor(d/2)) and give the rest back in post_scale -- exact powers of two, the product stays in range
+    *jac_init = 1.0;
+    if (precision == VEGAS_FP64) {
+        const int h = dim / 2;
+        *jac_init = std::ldexp(1.0, 32 * h);
+        *post_scale *= std::ldexp(1.0, 32 * (dim - h));
+    }
 }
 
 struct RotShape {
-    int blocks, threads;
+    int blocks, threads, n_groups, ring, ept;
     size_t shmem;
 };
 
+// One CTA per SM.  W warps (default 12 = 3 per scheduler, 170 registers each); as many histogram copies as
+// fit next to the table, W a multiple of the copy count; ring = warps per copy (1 = no token passing).
 RotShape rot_shape(const vegas_grid* g) {
     RotShape s;
-    s.shmem = vegas::rot_shared_bytes(g->dim, g->n_bins);
-    s.threads = g->cfg_threads > 0 ? g->cfg_threads : vegas::kRotThreads;
-    int per_sm = (int)(g->smem_total_sm / (s.shmem + 1024));
-    if (per_sm < 1) per_sm = 1;
-    if (per_sm > vegas::kRotMinBlocks) per_sm = vegas::kRotMinBlocks;
-    s.blocks = g->cfg_blocks > 0 ? g->cfg_blocks : g->sm_count * per_sm;
+    int W = g->cfg_threads > 0 ? (g->cfg_threads + 31) / 32 : vegas::kRotDefaultWarps;
+    const size_t one = vegas::rot_shared_bytes(g->dim, g->n_bins, 1), base = vegas::rot_shared_bytes(g->dim, g->n_bins, 0);
+    int fit = (int)((g->smem_optin - base) / (one - base));
+    if (fit < 1) fit = 1;
+    if (fit < W && W > vegas::kRotMaxRingWarps) W = vegas::kRotMaxRingWarps;     // rings need named barriers 1..15
+    int ng = fit < W ? fit : W;
+    while (W % ng) --ng;
+    s.n_groups = ng;
+    s.ring = W / ng;
+    s.threads = 32 * W;
+    s.shmem = vegas::rot_shared_bytes(g->dim, g->n_bins, ng);
+    s.blocks = g->cfg_blocks > 0 ? g->cfg_blocks : g->sm_count;
+    s.ept = g->cfg_ept > 0 ? g->cfg_ept : 1;
     return s;
 }
 
 cudaError_t launch_rot(int fid, int precision, int dim, const vegas::RotArgs& a, const RotShape& s, cudaStream_t st) {
     if (precision == VEGAS_FP64) {
         switch (fid) {
-        case VEGAS_F_CONST: return vegas::launch_iterate_rot<VEGAS_F_CONST, double>(dim, a, s.blocks, s.threads, s.shmem, st);
-        case VEGAS_F_GAUSS: return vegas::launch_iterate_rot<VEGAS_F_GAUSS, double>(dim, a, s.blocks, s.threads, s.shmem, st);
+        case VEGAS_F_CONST: return vegas::launch_iterate_rot<VEGAS_F_CONST, double>(dim, s.ept, a, s.blocks, s.threads, s.shmem, st);
+        case VEGAS_F_GAUSS: return vegas::launch_iterate_rot<VEGAS_F_GAUSS, double>(dim, s.ept, a, s.blocks, s.threads, s.shmem, st);
         case VEGAS_F_GENZ_PRODUCT_PEAK:
-            return vegas::launch_iterate_rot<VEGAS_F_GENZ_PRODUCT_PEAK, double>(dim, a, s.blocks, s.threads, s.shmem, st);
+            return vegas::launch_iterate_rot<VEGAS_F_GENZ_PRODUCT_PEAK, double>(dim, s.ept, a, s.blocks, s.threads, s.shmem, st);
         }
     } else {
         switch (fid) {
-        case VEGAS_F_CONST: return vegas::launch_iterate_rot<VEGAS_F_CONST, float>(dim, a, s.blocks, s.threads, s.shmem, st);
-        case VEGAS_F_GAUSS: return vegas::launch_iterate_rot<VEGAS_F_GAUSS, float>(dim, a, s.blocks, s.threads, s.shmem, st);
+        case VEGAS_F_CONST: return vegas::launch_iterate_rot<VEGAS_F_CONST, float>(dim, s.ept, a, s.blocks, s.threads, s.shmem, st);
+        case VEGAS_F_GAUSS: return vegas::launch_iterate_rot<VEGAS_F_GAUSS, float>(dim, s.ept, a, s.blocks, s.threads, s.shmem, st);
         }
     }
     return cudaErrorInvalidValue;
@@ -274,6 +293,7 @@ int vegas_create(int dim, int n_bins, void* dev_workspace, size_t bytes, vegas_g
     g->smem_total_sm = prop.sharedMemPerMultiprocessor;
     g->ws = (unsigned char*)dev_workspace;
     g->L = L;
+    if (const char* e = std::getenv("VEGAS_ROT_EPT")) g->cfg_ept = std::atoi(e) == 2 ? 2 : 1;
     g->d_edges = (double*)(g->ws + L.edges);
     g->d_totals = (double*)(g->ws + L.totals);
     g->d_result = (double*)(g->ws + L.result);
@@ -412,7 +432,9 @@ int vegas_accumulate(vegas_grid* g, uint64_t first_event, uint64_t count, uint64
         ra.key1 = (uint32_t)(seed >> 32);
         ra.iteration = iteration;
         ra.n_bins = g->n_bins;
-        rot_constants(g, fid, ra.shift, ra.scale, &ra.post_scale, &ra.fin0);
+        ra.n_groups = rs.n_groups;
+        ra.ring = rs.ring;
+        rot_constants(g, fid, precision, ra.shift, ra.scale, &ra.post_scale, &ra.fin0, &ra.jac_init);
     } else {
         if (resolve_launch(g, precision, &s)) return VEGAS_EINVAL;
         if (s.blocks > g->active_blocks) return VEGAS_EINVAL;
@@ -614,7 +636,7 @@ int vegas_debug_sample(vegas_grid* g, uint64_t first_event, uint32_t count, uint
     a.x = (double*)base;                       base += align_up(per_dim * 8);
     a.fJ = (double*)base;
     const bool rot = use_rot_path(g, fid, precision);
-    if (rot) rot_constants(g, fid, a.shift, a.scale, &a.post_scale, &a.fin0);
+    if (rot) rot_constants(g, fid, precision, a.shift, a.scale, &a.post_scale, &a.fin0, &a.jac_init);
     CUDA_TRY(g, vegas::launch_debug(fid, precision, rot, a, g->derived[fid], st));
     g->launches++;
     if (words) CUDA_TRY(g, cudaMemcpyAsync(words, a.words, per_dim * 4, cudaMemcpyDeviceToHost, st));
@@ -654,7 +676,7 @@ int vegas_get_launch(vegas_grid* g, int integrand_id, int precision, int* path, 
         if (blocks) *blocks = r.blocks;
         if (threads) *threads = r.threads;
         if (table_copies) *table_copies = precision == VEGAS_FP64 ? 2 : 4;
-        if (hist_copies) *hist_copies = 8;
+        if (hist_copies) *hist_copies = 8 * r.n_groups;
         if (shared_bytes) *shared_bytes = r.shmem;
         if (path) *path = 1;
         return VEGAS_OK;

@@ -2,15 +2,16 @@
 //
 // Same computation as the generic k_iterate (vegas_kernels.cu), for integrands whose dependence on
 // x_j goes through a per-dimension affine variable u_j = scale_j (x_j - shift_j)
-// (CONST, GAUSS: u = n_bins (x - 1/2); GENZ product peak: u = c_j (x - w_j)).  Three changes, each
-// driven by a counter of profiles/r01_k_iterate_v1.md:
+// (CONST, GAUSS: u = n_bins (x - 1/2); GENZ product peak: u = c_j (x - w_j)).  Design points, each
+// driven by a counter in profiles/ (r01_s2_baseline.md, r01_s2_ubench_hist.md, r01_s7_ubench_pipes.md):
 //
 //  1. DIM is a compile-time constant: no per-dimension guards, fully unrolled, bins packed one byte
 //     per dimension in registers.
 //  2. Affine pre-composition: the shared-memory table holds, per (dimension, bin), the pair
-//     (A', B) with u = A' + B m, where m in [1,2) is built from the 32 low product bits by two funnel
-//     shifts (fp64: m = 1 + r exactly; fp32: 23 bits, centred).  One FMA gives u; x_j itself is never
-//     formed, and B is the Jacobian factor up to a per-dimension constant folded into post_scale.
+//     (A, B) with u = A + B w, where w is the low product word of the split (C3) converted by one
+//     I2F (fp64: exact; u = scale (x - shift) with r = (w + 1/2) 2^-32 folded into A and B) or the
+//     top 23 bits put into a float mantissa (fp32).  One FMA gives u; x_j itself is never formed,
+//     and B is the Jacobian factor up to a per-dimension constant folded into post_scale.
 //     No integrand parameter is read inside the event loop.
 //  3. Bank rotation.  A Philox block serves 4 dimensions.  The 32 lanes of a warp are split into 4
 //     groups gamma = (lane>>1)&3; at sub-step i group gamma works on dimension 4 blk + (gamma ^ i)
@@ -19,9 +20,19 @@
 //         table [blk*n_bins + bin] : 128 B = 4 dim-slots x 2 copies x 16 B   (fp32: 4 x 4 x 8 B)
 //         hist  [blk*n_bins + bin] : 256 B = 2 half-warps x 4 dim-slots x 4 copies x 8 B
 //     are conflict-free whatever bins the lanes drew, with 2 table copies and 8 histogram copies
-//     instead of 8 and 16, and no two lanes of a warp ever update the same histogram word (no CAS
-//     retries inside a warp).  A last block with 2 (1) dimensions uses 2 (1) groups and 4 (8) table
-//     copies in the same row size; with 3 dimensions it uses 4 groups and one idle sub-step.
+//     instead of 8 and 32, and no two lanes of a warp ever touch the same histogram word in one
+//     instruction.  A last block with 2 (1) dimensions uses 2 (1) groups and 4 (8) table copies in
+//     the same row size; with 3 dimensions it uses 4 groups and one idle sub-step.
+//  4. Exclusive histogram ownership instead of atomics.  sm_100a has no native fp64 (or fp32, or
+//     64-bit integer) shared-memory atomic: atomicAdd(double) is an LDS + DADD + ATOMS.CAST.SPIN + BRA
+//     loop that costs 6.4 shared wavefronts and serialises the 20 updates of an event.  Here the CTA
+//     (one per SM, sharing one table) holds n_groups histogram copies; the `ring` warps of a group
+//     pass a token round a ring of named barriers (bar.sync / bar.arrive on 64 threads, 42 clk per
+//     hand-off) and only the token holder updates the group's histogram, with plain LDS.64 / DADD /
+//     STS.64 (4 wavefronts), the updates of the independent Philox blocks pipelined.  The critical
+//     section is ~10 % of a warp's loop iteration, so a ring of 4..6 warps rarely waits.  When the
+//     shared memory holds one histogram per warp (small dim * n_bins) the ring has length 1 and there
+//     is no synchronisation at all.
 #pragma once
 #include "vegas_device.cuh"
 #include "vegas_kernels.h"
@@ -53,15 +64,17 @@ template <typename T> struct IntegrandU<VEGAS_F_GENZ_PRODUCT_PEAK, T> {   // PAP
 template <typename T> struct RotEntry;
 template <> struct RotEntry<double> {
     using type = double2;
+    // u = scale (X_b + Delta r - shift), r = (w + 1/2) 2^-32  ==>  u = A + B' w with
+    // B' = scale Delta 2^-32 (exact scaling) and A = scale (X_b - shift) + B'/2.  The Jacobian factor is
+    // B' 2^32 / scale; the 2^32 per dimension goes into post_scale (vegas_api.cu: rot_constants).
     static __device__ __forceinline__ double2 make(double x0, double x1, double shift, double scale) {
         const double B = (x1 - x0) * scale, A = (x0 - shift) * scale;
-        return make_double2(A - B, B);                              // u = (A - B) + B m,  m = 1 + r
+        return make_double2(fma(B, 1.1641532182693481e-10, A), B * 2.3283064365386963e-10);   // 2^-33, 2^-32
     }
     static __device__ __forceinline__ double u(double2 e, uint32_t lo) {
-        // hi word: (0x3FF : lo) >> 12 (one funnel shift); lo word: lo * 2^20 + 2^19 (one IMAD, FMA pipe)
-        const double m = __hiloint2double((int)__funnelshift_r(lo, 0x3FFu, 12), (int)(lo * 0x100000u + 0x80000u));
-        return fma(e.y, m, e.x);
+        return fma(e.y, (double)lo, e.x);              // I2F.F64.U32 (its own pipe) + DFMA
     }
+    static constexpr double kJacUnit = 4294967296.0;   // table B = kJacUnit^-1 * scale * Delta
 };
 template <> struct RotEntry<float> {
     using type = float2;
@@ -74,6 +87,7 @@ template <> struct RotEntry<float> {
         const float m = __uint_as_float(__funnelshift_r(lo, 0x7Fu, 9));
         return fmaf(e.y, m, e.x);
     }
+    static constexpr double kJacUnit = 1.0;
 };
 
 // 32-bit shared-window addressing: one register per address, no generic-to-shared conversion
@@ -88,6 +102,17 @@ template <> __device__ __forceinline__ float2 lds_entry<float2>(uint32_t addr) {
     asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
     return v;
 }
+__device__ __forceinline__ double lds_f64(uint32_t addr) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_f64(uint32_t addr, double v) {
+    asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory");
+}
+// named barriers 1..15 on 64 threads: the waiting warp syncs, the signalling warp arrives
+__device__ __forceinline__ void token_wait(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
+__device__ __forceinline__ void token_pass(int id) { asm volatile("bar.arrive %0, 64;" ::"r"(id) : "memory"); }
 
 struct RotArgs {
     const double* edges;            // device, [DIM][n_bins+1]
@@ -95,13 +120,16 @@ struct RotArgs {
     unsigned long long first_event, count;
     uint32_t key0, key1, iteration;
     int n_bins;
-    double post_scale;              // v = f_u * prod_j B_j * post_scale
+    int n_groups, ring;             // histogram copies in the CTA; warps per copy (blockDim = 32 n_groups ring)
+    double post_scale;              // v = f_u * jac * post_scale
+    double jac_init;                // start value of the running Jacobian product (a power of two, see RotEntry)
     double fin0;                    // integrand finish constant
     double shift[VEGAS_MAX_DIM], scale[VEGAS_MAX_DIM];
 };
 
-constexpr int kRotThreads = 512;
-constexpr int kRotMinBlocks = 2;     // 64 registers per thread
+constexpr int kRotMaxThreads = 512;
+constexpr int kRotDefaultWarps = 12;
+constexpr int kRotMaxRingWarps = 15;   // named barriers 1..15
 
 __host__ __device__ constexpr int rot_groups(int r) { return r >= 3 ? 4 : r; }   // dims in block -> lane groups
 
@@ -128,23 +156,136 @@ __device__ __forceinline__ int rot_gamma(int lane) {
     return (lane & 7) >> (3 - LG);
 }
 
+// per-thread constants of the event loop
+template <typename T, int DIM>
+struct RotLane {
+    static constexpr int NBLK = (DIM + 3) / 4;
+    static constexpr int R = DIM - 4 * (NBLK - 1);               // dimensions in the last block, 1..4
+    static constexpr int GL = rot_groups(R);
+    uint32_t tbase, toff4, toffL, hbase, hoff4, hoffL;
+    int gamma4, gammaL;
+};
+
+// S1..S5 for one event: Philox -> split -> table -> u -> integrand; returns v = f J, leaves the bins
+// of block blk packed in packed[blk] (byte i = bin of sub-step i).
 template <int FID, typename T, int DIM>
-__global__ void __launch_bounds__(kRotThreads, kRotMinBlocks)
+__device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, DIM>& L, const PhiloxKey& ks,
+                                            unsigned long long ev, T fin0, uint32_t (&packed)[(DIM + 3) / 4]) {
+    using E = RotEntry<T>;
+    using T2 = typename E::type;
+    constexpr int NBLK = RotLane<T, DIM>::NBLK, R = RotLane<T, DIM>::R, GL = RotLane<T, DIM>::GL;
+    const int nb = a.n_bins;
+    const uint32_t e_lo = (uint32_t)ev, e_hi = (uint32_t)(ev >> 32);
+    IntegrandU<FID, T> f;
+    f.begin();
+    T jac = (T)a.jac_init;
+#pragma unroll
+    for (int blk = 0; blk < NBLK; ++blk) {
+        const bool last = (blk == NBLK - 1);
+        const int G = last ? GL : 4;
+        const int SH = (G == 4) ? 5 : (G == 2) ? 6 : 7;             // slot -> byte offset shift
+        const int NSUB = last ? ((R == 3) ? 4 : R) : 4;             // sub-steps of this block
+        const uint32_t toff = last ? L.toffL : L.toff4;
+        const int gamma = last ? L.gammaL : L.gamma4;
+        uint32_t w[4];
+        philox4x32_10((uint32_t)blk, a.iteration, e_lo, e_hi, ks, w);
+        // w'[i] = w[gamma ^ i]
+        if (G == 4) {
+            const bool g1 = gamma & 1, g2 = gamma & 2;
+            const uint32_t t0 = g1 ? w[1] : w[0], t1 = g1 ? w[0] : w[1], t2 = g1 ? w[3] : w[2], t3 = g1 ? w[2] : w[3];
+            w[0] = g2 ? t2 : t0; w[1] = g2 ? t3 : t1; w[2] = g2 ? t0 : t2; w[3] = g2 ? t1 : t3;
+        } else if (G == 2) {
+            const bool g1 = gamma & 1;
+            const uint32_t t0 = g1 ? w[1] : w[0], t1 = g1 ? w[0] : w[1];
+            w[0] = t0; w[1] = t1;
+        }
+        // the block's table reads are issued together, then consumed (their latency overlaps)
+        const uint32_t tblk = L.tbase + (uint32_t)(blk * nb) * 128u;
+        uint32_t lo[4], pk = 0;
+        T2 ent[4];
+#pragma unroll
+        for (int i = 0; i < NSUB; ++i) {
+            const bool active = !(last && R == 3) || ((gamma ^ i) < 3);
+            uint32_t b = 0;
+            lo[i] = 0;
+            ent[i] = T2{};
+            if (active) {
+                split_word(w[i], (uint32_t)nb, b, lo[i]);
+                ent[i] = lds_entry<T2>(tblk + (b * 128u + (toff ^ (uint32_t)(i << SH))));
+                pk |= b << (8 * i);
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < NSUB; ++i) {
+            const bool active = !(last && R == 3) || ((gamma ^ i) < 3);
+            if (active) {
+                jac *= ent[i].y;
+                f.dim(E::u(ent[i], lo[i]));
+            }
+        }
+        packed[blk] = pk;
+    }
+    return (double)(f.finish(fin0) * jac) * a.post_scale;
+}
+
+// S6 for one event, by the warp that holds its group's token: H[j][b_j] += v2 with plain loads and
+// stores.  Round i handles sub-step i of every Philox block: within a round the lanes of the warp touch
+// pairwise different words (different rows per block; inside a row each lane has its own column), so the
+// NBLK read-modify-writes of a round are independent and pipeline.  Consecutive rounds can touch the
+// same word from different lanes, hence the __syncwarp() (shared memory is processed in order per warp).
+template <typename T, int DIM>
+__device__ __forceinline__ void rot_hist_update(const RotLane<T, DIM>& L, int nb, const uint32_t (&packed)[(DIM + 3) / 4],
+                                                double v2) {
+    constexpr int NBLK = RotLane<T, DIM>::NBLK, R = RotLane<T, DIM>::R, GL = RotLane<T, DIM>::GL;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        uint32_t addr[NBLK];
+        double h[NBLK];
+#pragma unroll
+        for (int blk = 0; blk < NBLK; ++blk) {
+            const bool last = (blk == NBLK - 1);
+            const int G = last ? GL : 4;
+            const int SH = (G == 4) ? 5 : (G == 2) ? 6 : 7;
+            const int NSUB = last ? ((R == 3) ? 4 : R) : 4;
+            const uint32_t hoff = last ? L.hoffL : L.hoff4;
+            const int gamma = last ? L.gammaL : L.gamma4;
+            const bool active = (i < NSUB) && (!(last && R == 3) || ((gamma ^ i) < 3));
+            if (active) {
+                const uint32_t b256 = __byte_perm(packed[blk], 0, 0x4404 | (i << 4));   // byte i -> bits 8..15
+                addr[blk] = L.hbase + (uint32_t)(blk * nb) * 256u + (b256 + (hoff ^ (uint32_t)(i << SH)));
+                h[blk] = lds_f64(addr[blk]);
+            }
+        }
+#pragma unroll
+        for (int blk = 0; blk < NBLK; ++blk) {
+            const bool last = (blk == NBLK - 1);
+            const int NSUB = last ? ((R == 3) ? 4 : R) : 4;
+            const int gamma = last ? L.gammaL : L.gamma4;
+            const bool active = (i < NSUB) && (!(last && R == 3) || ((gamma ^ i) < 3));
+            if (active) sts_f64(addr[blk], h[blk] + v2);
+        }
+        __syncwarp();
+    }
+}
+
+// EPT = events per thread per loop iteration (independent chains for the scheduler to interleave).
+template <int FID, typename T, int DIM, int EPT>
+__global__ void __launch_bounds__(kRotMaxThreads, 1)
 k_iterate_rot(const __grid_constant__ RotArgs a) {
     using E = RotEntry<T>;
     using T2 = typename E::type;
-    constexpr int NBLK = (DIM + 3) / 4;
-    constexpr int R = DIM - 4 * (NBLK - 1);               // dimensions in the last block, 1..4
-    constexpr int GL = rot_groups(R);
+    using Lane = RotLane<T, DIM>;
+    constexpr int NBLK = Lane::NBLK, GL = Lane::GL;
     constexpr int ENTRY = (int)sizeof(T2);
     extern __shared__ __align__(256) unsigned char smem_rot[];
     const int nb = a.n_bins;
     const int rows = NBLK * nb;
+    const int NG = a.n_groups, S = a.ring;
     unsigned char* table = smem_rot;                           // rows x 128 B
-    unsigned char* hist = smem_rot + (size_t)rows * 128;       // rows x 256 B
-    dd* red = reinterpret_cast<dd*>(hist + (size_t)rows * 256);
+    unsigned char* hist = smem_rot + (size_t)rows * 128;       // NG x rows x 256 B
+    dd* red = reinterpret_cast<dd*>(hist + (size_t)NG * rows * 256);
 
-    // ---- prologue: table from the master grid, zero histogram
+    // ---- prologue: table from the master grid, zero histograms
     for (int idx = threadIdx.x; idx < rows * (128 / ENTRY); idx += blockDim.x) {
         const int row = idx / (128 / ENTRY), e = idx - row * (128 / ENTRY);   // entry e of the row
         const int blk = row / nb, b = row - blk * nb;
@@ -158,104 +299,51 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
         }
         reinterpret_cast<T2*>(table)[idx] = ent;
     }
-    for (int idx = threadIdx.x; idx < rows * 32; idx += blockDim.x) reinterpret_cast<double*>(hist)[idx] = 0.0;
+    for (int idx = threadIdx.x; idx < NG * rows * 32; idx += blockDim.x) reinterpret_cast<double*>(hist)[idx] = 0.0;
     __syncthreads();
 
-    const int lane = threadIdx.x & 31;
-    const uint32_t tbase = (uint32_t)__cvta_generic_to_shared(table);
-    const uint32_t toff4 = rot_table_off0<4, ENTRY>(lane), hoff4 = rot_hist_off0<4>(lane);
-    const uint32_t toffL = rot_table_off0<GL, ENTRY>(lane), hoffL = rot_hist_off0<GL>(lane);
-    const int gamma4 = rot_gamma<4>(lane), gammaL = rot_gamma<GL>(lane);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int grp = warp / S, pos = warp - grp * S;            // histogram copy of this warp, place in its ring
+    Lane L;
+    L.tbase = (uint32_t)__cvta_generic_to_shared(table);
+    L.hbase = (uint32_t)__cvta_generic_to_shared(hist) + (uint32_t)grp * (uint32_t)rows * 256u;
+    L.toff4 = rot_table_off0<4, ENTRY>(lane);  L.hoff4 = rot_hist_off0<4>(lane);
+    L.toffL = rot_table_off0<GL, ENTRY>(lane); L.hoffL = rot_hist_off0<GL>(lane);
+    L.gamma4 = rot_gamma<4>(lane);             L.gammaL = rot_gamma<GL>(lane);
     const PhiloxKey ks = philox_key_schedule(a.key0, a.key1);
     const T fin0 = (T)a.fin0;
+    const int my_token = 1 + warp, next_token = 1 + grp * S + ((pos + 1 == S) ? 0 : pos + 1);
 
     double s1 = 0.0, c1 = 0.0, s2 = 0.0, c2 = 0.0;
-    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
-    for (unsigned long long q = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; q < a.count; q += stride) {
-        const unsigned long long ev = a.first_event + q;
-        const uint32_t e_lo = (uint32_t)ev, e_hi = (uint32_t)(ev >> 32);
-        IntegrandU<FID, T> f;
-        f.begin();
-        T jac = (T)1;
-        uint32_t packed[NBLK];
+    // every warp runs the same number of loop iterations (the ring hands the token on once per iteration);
+    // events past the end of the range contribute v = 0
+    const unsigned long long nthr = (unsigned long long)gridDim.x * blockDim.x;
+    const unsigned long long per_iter = nthr * EPT;
+    const unsigned long long n_iter = (a.count + per_iter - 1) / per_iter;
+    unsigned long long q = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    for (unsigned long long it = 0; it < n_iter; ++it, q += per_iter) {
+        uint32_t packed[EPT][NBLK];
+        double v2[EPT];
 #pragma unroll
-        for (int blk = 0; blk < NBLK; ++blk) {
-            const bool last = (blk == NBLK - 1);
-            const int G = last ? GL : 4;
-            const int SH = (G == 4) ? 5 : (G == 2) ? 6 : 7;             // slot -> byte offset shift
-            const int NSUB = last ? ((R == 3) ? 4 : R) : 4;             // sub-steps of this block
-            const uint32_t toff = last ? toffL : toff4;
-            const int gamma = last ? gammaL : gamma4;
-            uint32_t w[4];
-            philox4x32_10((uint32_t)blk, a.iteration, e_lo, e_hi, ks, w);
-            // w'[i] = w[gamma ^ i]
-            if (G == 4) {
-                const bool g1 = gamma & 1, g2 = gamma & 2;
-                const uint32_t t0 = g1 ? w[1] : w[0], t1 = g1 ? w[0] : w[1], t2 = g1 ? w[3] : w[2], t3 = g1 ? w[2] : w[3];
-                w[0] = g2 ? t2 : t0; w[1] = g2 ? t3 : t1; w[2] = g2 ? t0 : t2; w[3] = g2 ? t1 : t3;
-            } else if (G == 2) {
-                const bool g1 = gamma & 1;
-                const uint32_t t0 = g1 ? w[1] : w[0], t1 = g1 ? w[0] : w[1];
-                w[0] = t0; w[1] = t1;
-            }
-            // the block's table reads are issued together, then consumed (their latency overlaps)
-            const uint32_t tblk = tbase + (uint32_t)(blk * nb) * 128u;
-            uint32_t lo[4], pk = 0;
-            T2 ent[4];
-#pragma unroll
-            for (int i = 0; i < NSUB; ++i) {
-                const bool active = !(last && R == 3) || ((gamma ^ i) < 3);
-                uint32_t b = 0;
-                lo[i] = 0;
-                ent[i] = T2{};
-                if (active) {
-                    split_word(w[i], (uint32_t)nb, b, lo[i]);
-                    ent[i] = lds_entry<T2>(tblk + (b * 128u + (toff ^ (uint32_t)(i << SH))));
-                    pk |= b << (8 * i);
-                }
-            }
-#pragma unroll
-            for (int i = 0; i < NSUB; ++i) {
-                const bool active = !(last && R == 3) || ((gamma ^ i) < 3);
-                if (active) {
-                    jac *= ent[i].y;
-                    f.dim(E::u(ent[i], lo[i]));
-                }
-            }
-            packed[blk] = pk;
+        for (int k = 0; k < EPT; ++k) {
+            const unsigned long long qk = q + (unsigned long long)k * nthr;
+            double v = rot_event<FID, T, DIM>(a, L, ks, a.first_event + qk, fin0, packed[k]);
+            if (qk >= a.count) v = 0.0;
+            v2[k] = v * v;
+            kahan_add(s1, c1, v);
+            kahan_add(s2, c2, v2[k]);
         }
-        const double v = (double)(f.finish(fin0) * jac) * a.post_scale;
-        const double v2 = v * v;
-        kahan_add(s1, c1, v);
-        kahan_add(s2, c2, v2);
+        if (S > 1 && (pos != 0 || it != 0)) token_wait(my_token);
 #pragma unroll
-        for (int blk = 0; blk < NBLK; ++blk) {
-            const bool last = (blk == NBLK - 1);
-            const int G = last ? GL : 4;
-            const int SH = (G == 4) ? 5 : (G == 2) ? 6 : 7;
-            const int NSUB = last ? ((R == 3) ? 4 : R) : 4;
-            const uint32_t hoff = last ? hoffL : hoff4;
-            const int gamma = last ? gammaL : gamma4;
-            // S6: one shared-memory atomicAdd per dimension.  ptxas lowers it to LDS + ATOMS.CAST.SPIN, the
-            // fast hardware path; an explicit value-returning atom.shared.cas.b64 (ATOMS.CAS.64) measured
-            // 3-18x slower (profiles/r01_k_iterate_rot.md).  No two lanes of the warp share a word, so the
-            // spin only retries when another warp hit the same word in between.
-            unsigned char* hblk = hist + (size_t)(blk * nb) * 256;
-#pragma unroll
-            for (int i = 0; i < NSUB; ++i) {
-                const bool active = !(last && R == 3) || ((gamma ^ i) < 3);
-                if (active) {
-                    const uint32_t b256 = __byte_perm(packed[blk], 0, 0x4404 | (i << 4));   // byte i -> bits 8..15
-                    atomicAdd(reinterpret_cast<double*>(hblk + (b256 + (hoff ^ (uint32_t)(i << SH)))), v2);
-                }
-            }
-        }
+        for (int k = 0; k < EPT; ++k) rot_hist_update<T, DIM>(L, nb, packed[k], v2[k]);
+        if (S > 1) token_pass(next_token);
     }
+    if (S > 1 && pos == 0 && n_iter > 0) token_wait(my_token);   // absorbs the ring's last hand-off
 
     // ---- S5: warp shuffle -> CTA -> this CTA's partial (accumulated over the launches of an iteration)
     dd t1 = dd_warp_sum(fast_two_sum(s1, -c1));
     dd t2 = dd_warp_sum(fast_two_sum(s2, -c2));
-    const int warp = threadIdx.x >> 5, nwarps = (blockDim.x + 31) >> 5;
+    const int nwarps = (blockDim.x + 31) >> 5;
     if (lane == 0) { red[2 * warp] = t1; red[2 * warp + 1] = t2; }
     __syncthreads();
     double* part = a.partials + (size_t)blockIdx.x * (4 + DIM * nb);
@@ -276,21 +364,23 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
         const int blk = j >> 2, slot = j & 3;
         const int G = (blk < NBLK - 1) ? 4 : GL;
         const int per = 16 / G;                                   // copies per half-warp row half
-        const double* row = reinterpret_cast<const double*>(hist + (size_t)(blk * nb + b) * 256);
         double h = 0.0;
-        for (int half = 0; half < 2; ++half)
-            for (int c = 0; c < per; ++c) h += row[half * 16 + slot * per + c];
+        for (int g = 0; g < NG; ++g) {
+            const double* row = reinterpret_cast<const double*>(hist + ((size_t)g * rows + (size_t)(blk * nb + b)) * 256);
+            for (int half = 0; half < 2; ++half)
+                for (int c = 0; c < per; ++c) h += row[half * 16 + slot * per + c];
+        }
         part[4 + idx] += h;
     }
 }
 
-inline size_t rot_shared_bytes(int dim, int n_bins) {
+inline size_t rot_shared_bytes(int dim, int n_bins, int n_groups) {
     const size_t rows = (size_t)((dim + 3) / 4) * n_bins;
-    return rows * (128 + 256) + 2 * sizeof(dd) * (kRotThreads / 32);
+    return rows * (128 + 256 * (size_t)n_groups) + 2 * sizeof(dd) * (kRotMaxThreads / 32);
 }
 
 // one translation unit per (FID, T) instantiates DIM = 1..32 (vegas_rot_inst.cu)
 template <int FID, typename T>
-cudaError_t launch_iterate_rot(int dim, const RotArgs& a, int blocks, int threads, size_t shmem, cudaStream_t st);
+cudaError_t launch_iterate_rot(int dim, int ept, const RotArgs& a, int blocks, int threads, size_t shmem, cudaStream_t st);
 
 }  // namespace vegas

@@ -303,7 +303,7 @@ __global__ void k_debug_rot(const __grid_constant__ DebugArgs a) {
     const PhiloxKey ks = philox_key_schedule(a.key0, a.key1);
     IntegrandU<FID, T> f;
     f.begin();
-    T jac = (T)1;
+    T jac = (T)a.jac_init;
     uint32_t w[4] = {0, 0, 0, 0};
     for (int j = 0; j < dim; ++j) {
         if ((j & 3) == 0) philox4x32_10((uint32_t)(j >> 2), a.iteration, (uint32_t)e, (uint32_t)(e >> 32), ks, w);

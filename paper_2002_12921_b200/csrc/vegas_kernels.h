@@ -41,7 +41,7 @@ struct DebugArgs {
     double* x;
     double* fJ;
     // fast ("rotated") path only: the affine map and constants of vegas_iterate_rot.cuh
-    double post_scale, fin0;
+    double post_scale, fin0, jac_init;
     double shift[VEGAS_MAX_DIM], scale[VEGAS_MAX_DIM];
 };
 

@@ -66,6 +66,29 @@ __global__ void __launch_bounds__(THREADS) k_imad_wide(Stamp* out, uint32_t m) {
     BENCH_EPILOG(s)
 }
 
+// one IMAD.WIDE.U32 per chain step plus NX independent cheap instructions of another pipe (LOP3/IADD on the ALU,
+// or DFMA on the fp64 pipe): does the wide multiply hold the dispatch port, or only its own pipe?
+template <int NX, int KIND>
+__global__ void __launch_bounds__(THREADS) k_wide_mix(Stamp* out, uint32_t m, uint32_t a, double da) {
+    uint32_t x[UNR], y[UNR];
+    double z[UNR];
+    for (int u = 0; u < UNR; ++u) { x[u] = threadIdx.x * 2654435761u + u; y[u] = x[u] ^ 0x5bd1e995u; z[u] = u; }
+    BENCH_PROLOG
+    for (int i = 0; i < ITER; ++i)
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) {
+            const uint64_t p = (uint64_t)x[u] * m;
+            x[u] = (uint32_t)(p >> 32) + (uint32_t)p;      // IADD keeps both halves live
+#pragma unroll
+            for (int k = 0; k < NX; ++k) {
+                if (KIND == 0) y[u] = (y[u] ^ a) + 0x9E3779B9u * (k + 1);      // LOP3 + IADD
+                else z[u] = fma(z[u], da, 1.0);
+            }
+        }
+    uint32_t s = 0; for (int u = 0; u < UNR; ++u) s ^= x[u] ^ y[u] ^ (uint32_t)__double2loint(z[u]);
+    BENCH_EPILOG(s)
+}
+
 __global__ void __launch_bounds__(THREADS) k_imad_lo(Stamp* out, uint32_t m, uint32_t c) {
     uint32_t x[UNR];
     for (int u = 0; u < UNR; ++u) x[u] = threadIdx.x * 2654435761u + u;
@@ -241,6 +264,12 @@ int main() {
         k_ffma<<<n_sm, THREADS>>>(d_out, 1.0001f, 0.5f);              if (rep) report_alu("FFMA", 1);
         k_dfma<<<n_sm, THREADS>>>(d_out, 1.0001, 0.5);                if (rep) report_alu("DFMA", 1);
         k_imad_wide<<<n_sm, THREADS>>>(d_out, 0xD2511F53u);           if (rep) report_alu("IMAD.WIDE.U32 (+1 LOP3 each)", 1);
+        k_wide_mix<0, 0><<<n_sm, THREADS>>>(d_out, 0xD2511F53u, 0x55u, 1.0001);  if (rep) report_alu("IMAD.WIDE.U32 + IADD (chain steps)", 1);
+        k_wide_mix<1, 0><<<n_sm, THREADS>>>(d_out, 0xD2511F53u, 0x55u, 1.0001);  if (rep) report_alu("  same + 1 x (LOP3+IADD) (chain steps)", 1);
+        k_wide_mix<2, 0><<<n_sm, THREADS>>>(d_out, 0xD2511F53u, 0x55u, 1.0001);  if (rep) report_alu("  same + 2 x (LOP3+IADD) (chain steps)", 1);
+        k_wide_mix<4, 0><<<n_sm, THREADS>>>(d_out, 0xD2511F53u, 0x55u, 1.0001);  if (rep) report_alu("  same + 4 x (LOP3+IADD) (chain steps)", 1);
+        k_wide_mix<1, 1><<<n_sm, THREADS>>>(d_out, 0xD2511F53u, 0x55u, 1.0001);  if (rep) report_alu("  same + 1 DFMA (chain steps)", 1);
+        k_wide_mix<2, 1><<<n_sm, THREADS>>>(d_out, 0xD2511F53u, 0x55u, 1.0001);  if (rep) report_alu("  same + 2 DFMA (chain steps)", 1);
         k_imad_lo<<<n_sm, THREADS>>>(d_out, 0xD2511F53u, 12345u);     if (rep) report_alu("IMAD (32-bit low)", 1);
         k_imad_hi<<<n_sm, THREADS>>>(d_out, 0xD2511F53u);             if (rep) report_alu("IMAD.HI.U32 (+1 IADD each)", 1);
         k_lop3<<<n_sm, THREADS>>>(d_out, 0x9E3779B9u, 0xBB67AE85u);   if (rep) report_alu("LOP3 + IADD pair", 2);

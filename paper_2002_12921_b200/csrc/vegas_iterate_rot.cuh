@@ -321,22 +321,50 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     const unsigned long long per_iter = nthr * EPT;
     const unsigned long long n_iter = (a.count + per_iter - 1) / per_iter;
     unsigned long long q = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
-    for (unsigned long long it = 0; it < n_iter; ++it, q += per_iter) {
+    // Software pipeline: the histogram update of the events of loop iteration it-1 is done after the
+    // per-event work of iteration it, so that the token has a whole iteration to come round the ring
+    // before this warp needs it (the barrier stall of the unpipelined loop was 20 % of the warp time,
+    // profiles/r01_s7_ring.md).
+    uint32_t ppacked[EPT][NBLK];
+    double pv2[EPT];
+#pragma unroll
+    for (int k = 0; k < EPT; ++k) {
+        pv2[k] = 0.0;
+#pragma unroll
+        for (int b = 0; b < NBLK; ++b) ppacked[k][b] = 0;
+    }
+    for (unsigned long long it = 0; it <= n_iter; ++it, q += per_iter) {
         uint32_t packed[EPT][NBLK];
         double v2[EPT];
 #pragma unroll
         for (int k = 0; k < EPT; ++k) {
-            const unsigned long long qk = q + (unsigned long long)k * nthr;
-            double v = rot_event<FID, T, DIM>(a, L, ks, a.first_event + qk, fin0, packed[k]);
-            if (qk >= a.count) v = 0.0;
-            v2[k] = v * v;
-            kahan_add(s1, c1, v);
-            kahan_add(s2, c2, v2[k]);
-        }
-        if (S > 1 && (pos != 0 || it != 0)) token_wait(my_token);
+            v2[k] = 0.0;
 #pragma unroll
-        for (int k = 0; k < EPT; ++k) rot_hist_update<T, DIM>(L, nb, packed[k], v2[k]);
-        if (S > 1) token_pass(next_token);
+            for (int b = 0; b < NBLK; ++b) packed[k][b] = 0;
+        }
+        if (it < n_iter) {
+#pragma unroll
+            for (int k = 0; k < EPT; ++k) {
+                const unsigned long long qk = q + (unsigned long long)k * nthr;
+                double v = rot_event<FID, T, DIM>(a, L, ks, a.first_event + qk, fin0, packed[k]);
+                if (qk >= a.count) v = 0.0;
+                v2[k] = v * v;
+                kahan_add(s1, c1, v);
+                kahan_add(s2, c2, v2[k]);
+            }
+        }
+        if (it > 0) {
+            if (S > 1 && (pos != 0 || it != 1)) token_wait(my_token);
+#pragma unroll
+            for (int k = 0; k < EPT; ++k) rot_hist_update<T, DIM>(L, nb, ppacked[k], pv2[k]);
+            if (S > 1) token_pass(next_token);
+        }
+#pragma unroll
+        for (int k = 0; k < EPT; ++k) {
+            pv2[k] = v2[k];
+#pragma unroll
+            for (int b = 0; b < NBLK; ++b) ppacked[k][b] = packed[k][b];
+        }
     }
     if (S > 1 && pos == 0 && n_iter > 0) token_wait(my_token);   // absorbs the ring's last hand-off
 

@@ -72,7 +72,7 @@ struct vegas_grid {
     bool params_set[4] = {true, false, false, false};
     double derived[4][VEGAS_MAX_PARAMS] = {};
     double user[4][VEGAS_MAX_PARAMS] = {};       // the caller's arrays as given to vegas_set_params
-    int cfg_blocks = 0, cfg_threads = 0, cfg_ct = 0, cfg_ch = 0, cfg_ept = 0;
+    int cfg_blocks = 0, cfg_threads = 0, cfg_ct = 0, cfg_ch = 0;
     int active_blocks = 0;          // CTAs whose partial slots the current iteration uses
     bool profiling = false;
     std::vector<cudaEvent_t> events;   // pairs (start, stop)
@@ -208,7 +208,7 @@ void rot_constants(const vegas_grid* g, int fid, int precision, double* shift, d
 }
 
 struct RotShape {
-    int blocks, threads, n_groups, ring, ept;
+    int blocks, threads, n_groups, ring;
     size_t shmem;
 };
 
@@ -228,22 +228,21 @@ RotShape rot_shape(const vegas_grid* g) {
     s.threads = 32 * W;
     s.shmem = vegas::rot_shared_bytes(g->dim, g->n_bins, ng);
     s.blocks = g->cfg_blocks > 0 ? g->cfg_blocks : g->sm_count;
-    s.ept = g->cfg_ept > 0 ? g->cfg_ept : 1;
     return s;
 }
 
 cudaError_t launch_rot(int fid, int precision, int dim, const vegas::RotArgs& a, const RotShape& s, cudaStream_t st) {
     if (precision == VEGAS_FP64) {
         switch (fid) {
-        case VEGAS_F_CONST: return vegas::launch_iterate_rot<VEGAS_F_CONST, double>(dim, s.ept, a, s.blocks, s.threads, s.shmem, st);
-        case VEGAS_F_GAUSS: return vegas::launch_iterate_rot<VEGAS_F_GAUSS, double>(dim, s.ept, a, s.blocks, s.threads, s.shmem, st);
+        case VEGAS_F_CONST: return vegas::launch_iterate_rot<VEGAS_F_CONST, double>(dim, a, s.blocks, s.threads, s.shmem, st);
+        case VEGAS_F_GAUSS: return vegas::launch_iterate_rot<VEGAS_F_GAUSS, double>(dim, a, s.blocks, s.threads, s.shmem, st);
         case VEGAS_F_GENZ_PRODUCT_PEAK:
-            return vegas::launch_iterate_rot<VEGAS_F_GENZ_PRODUCT_PEAK, double>(dim, s.ept, a, s.blocks, s.threads, s.shmem, st);
+            return vegas::launch_iterate_rot<VEGAS_F_GENZ_PRODUCT_PEAK, double>(dim, a, s.blocks, s.threads, s.shmem, st);
         }
     } else {
         switch (fid) {
-        case VEGAS_F_CONST: return vegas::launch_iterate_rot<VEGAS_F_CONST, float>(dim, s.ept, a, s.blocks, s.threads, s.shmem, st);
-        case VEGAS_F_GAUSS: return vegas::launch_iterate_rot<VEGAS_F_GAUSS, float>(dim, s.ept, a, s.blocks, s.threads, s.shmem, st);
+        case VEGAS_F_CONST: return vegas::launch_iterate_rot<VEGAS_F_CONST, float>(dim, a, s.blocks, s.threads, s.shmem, st);
+        case VEGAS_F_GAUSS: return vegas::launch_iterate_rot<VEGAS_F_GAUSS, float>(dim, a, s.blocks, s.threads, s.shmem, st);
         }
     }
     return cudaErrorInvalidValue;
@@ -293,7 +292,6 @@ int vegas_create(int dim, int n_bins, void* dev_workspace, size_t bytes, vegas_g
     g->smem_total_sm = prop.sharedMemPerMultiprocessor;
     g->ws = (unsigned char*)dev_workspace;
     g->L = L;
-    if (const char* e = std::getenv("VEGAS_ROT_EPT")) g->cfg_ept = std::atoi(e) == 2 ? 2 : 1;
     g->d_edges = (double*)(g->ws + L.edges);
     g->d_totals = (double*)(g->ws + L.totals);
     g->d_result = (double*)(g->ws + L.result);
@@ -428,8 +426,10 @@ int vegas_accumulate(vegas_grid* g, uint64_t first_event, uint64_t count, uint64
         if (rs.blocks > g->active_blocks) return VEGAS_EINVAL;
         ra.edges = g->d_edges;
         ra.partials = g->d_partials;
-        ra.key0 = (uint32_t)(seed & 0xFFFFFFFFu);
-        ra.key1 = (uint32_t)(seed >> 32);
+        for (int r = 0; r < 10; ++r) {                            // C1 key schedule
+            ra.k0[r] = (uint32_t)(seed & 0xFFFFFFFFu) + (uint32_t)r * 0x9E3779B9u;
+            ra.k1[r] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u;
+        }
         ra.iteration = iteration;
         ra.n_bins = g->n_bins;
         ra.n_groups = rs.n_groups;

@@ -51,7 +51,7 @@ template <typename T> struct IntegrandU<VEGAS_F_GAUSS, T> {   // PAPER.md:65 Eq.
     T s;
     __device__ __forceinline__ void begin() { s = (T)0; }
     __device__ __forceinline__ void dim(T u) { s = t_fma(u, u, s); }
-    __device__ __forceinline__ T finish(T fin0) const { return t_exp<T>(-s * fin0); }   // fin0 = 1/(n_bins a)^2
+    __device__ __forceinline__ T finish(T fin0) const { return t_exp_fast<T>(-s * fin0); }   // fin0 = 1/(n_bins a)^2
 };
 template <typename T> struct IntegrandU<VEGAS_F_GENZ_PRODUCT_PEAK, T> {   // PAPER.md:74 Eq.(3); u = c_j (x - w_j)
     T prod;
@@ -118,7 +118,8 @@ struct RotArgs {
     const double* edges;            // device, [DIM][n_bins+1]
     double* partials;               // device, [gridDim.x][4 + DIM*n_bins]
     unsigned long long first_event, count;
-    uint32_t key0, key1, iteration;
+    uint32_t iteration;
+    uint32_t k0[10], k1[10];        // Philox key schedule (C1), built on the host: LOP3 reads it from the constant bank
     int n_bins;
     int n_groups, ring;             // histogram copies in the CTA; warps per copy (blockDim = 32 n_groups ring)
     double post_scale;              // v = f_u * jac * post_scale
@@ -127,9 +128,9 @@ struct RotArgs {
     double shift[VEGAS_MAX_DIM], scale[VEGAS_MAX_DIM];
 };
 
-constexpr int kRotMaxThreads = 512;
+constexpr int kRotMaxThreads = 384;    // one CTA per SM: 12 warps, up to 168 registers per thread
 constexpr int kRotDefaultWarps = 12;
-constexpr int kRotMaxRingWarps = 15;   // named barriers 1..15
+constexpr int kRotMaxRingWarps = 12;   // named barriers 1..15 would allow 15; the register budget allows 12
 
 __host__ __device__ constexpr int rot_groups(int r) { return r >= 3 ? 4 : r; }   // dims in block -> lane groups
 
@@ -156,21 +157,43 @@ __device__ __forceinline__ int rot_gamma(int lane) {
     return (lane & 7) >> (3 - LG);
 }
 
-// per-thread constants of the event loop
+// per-thread constants of the event loop.  Addresses are 32-bit shared-window addresses.
+//   table entry of (blk, bin, sub-step i):  taddr = tbase + (blk nb + bin) 128 + tx[i]
+//   histogram word of the same:             haddr = hbase + (blk nb + bin) 256 + hx[i] = 2 taddr + hc[i]
+// so the histogram address costs one LEA from the table address kept in a register (no bin packing).
 template <typename T, int DIM>
 struct RotLane {
     static constexpr int NBLK = (DIM + 3) / 4;
     static constexpr int R = DIM - 4 * (NBLK - 1);               // dimensions in the last block, 1..4
     static constexpr int GL = rot_groups(R);
-    uint32_t tbase, toff4, toffL, hbase, hoff4, hoffL;
+    uint32_t tbase;
+    uint32_t tx4[4], txL[4];      // full blocks / last block: row offset of sub-step i (lane-dependent)
+    uint32_t hc4[4], hcL[4];      // haddr - 2 taddr
     int gamma4, gammaL;
 };
 
-// S1..S5 for one event: Philox -> split -> table -> u -> integrand; returns v = f J, leaves the bins
-// of block blk packed in packed[blk] (byte i = bin of sub-step i).
+// C1 with the key schedule taken from the kernel arguments
+__device__ __forceinline__ void philox4x32_10_args(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                                   const RotArgs& a, uint32_t (&out)[4]) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ a.k0[r];
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ a.k1[r];
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// S1..S5 for one event: Philox -> split -> table -> u -> integrand; returns v = f J and leaves the
+// table address of every (block, sub-step) in taddr (the histogram update derives its addresses from them).
 template <int FID, typename T, int DIM>
-__device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, DIM>& L, const PhiloxKey& ks,
-                                            unsigned long long ev, T fin0, uint32_t (&packed)[(DIM + 3) / 4]) {
+__device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, DIM>& L, unsigned long long ev, T fin0,
+                                            uint32_t (&taddr)[(DIM + 3) / 4][4]) {
     using E = RotEntry<T>;
     using T2 = typename E::type;
     constexpr int NBLK = RotLane<T, DIM>::NBLK, R = RotLane<T, DIM>::R, GL = RotLane<T, DIM>::GL;
@@ -183,12 +206,10 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
     for (int blk = 0; blk < NBLK; ++blk) {
         const bool last = (blk == NBLK - 1);
         const int G = last ? GL : 4;
-        const int SH = (G == 4) ? 5 : (G == 2) ? 6 : 7;             // slot -> byte offset shift
         const int NSUB = last ? ((R == 3) ? 4 : R) : 4;             // sub-steps of this block
-        const uint32_t toff = last ? L.toffL : L.toff4;
         const int gamma = last ? L.gammaL : L.gamma4;
         uint32_t w[4];
-        philox4x32_10((uint32_t)blk, a.iteration, e_lo, e_hi, ks, w);
+        philox4x32_10_args((uint32_t)blk, a.iteration, e_lo, e_hi, a, w);
         // w'[i] = w[gamma ^ i]
         if (G == 4) {
             const bool g1 = gamma & 1, g2 = gamma & 2;
@@ -201,18 +222,23 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
         }
         // the block's table reads are issued together, then consumed (their latency overlaps)
         const uint32_t tblk = L.tbase + (uint32_t)(blk * nb) * 128u;
-        uint32_t lo[4], pk = 0;
+        uint32_t lo[4];
         T2 ent[4];
 #pragma unroll
-        for (int i = 0; i < NSUB; ++i) {
-            const bool active = !(last && R == 3) || ((gamma ^ i) < 3);
-            uint32_t b = 0;
-            lo[i] = 0;
-            ent[i] = T2{};
-            if (active) {
-                split_word(w[i], (uint32_t)nb, b, lo[i]);
-                ent[i] = lds_entry<T2>(tblk + (b * 128u + (toff ^ (uint32_t)(i << SH))));
-                pk |= b << (8 * i);
+        for (int i = 0; i < 4; ++i) {
+            taddr[blk][i] = 0;
+            if (i < NSUB) {
+                const bool active = !(last && R == 3) || ((gamma ^ i) < 3);
+                uint32_t b = 0;
+                lo[i] = 0;
+                ent[i] = T2{};
+                if (active) {
+                    split_word(w[i], (uint32_t)nb, b, lo[i]);
+                    // one multiply-add (ptxas: LEA/IMAD); written in C the compiler folds the shift into a
+                    // 64-bit funnel shift of the product plus a mask plus an add
+                    asm("mad.lo.u32 %0, %1, 128, %2;" : "=r"(taddr[blk][i]) : "r"(b), "r"(tblk + (last ? L.txL[i] : L.tx4[i])));
+                    ent[i] = lds_entry<T2>(taddr[blk][i]);
+                }
             }
         }
 #pragma unroll
@@ -223,7 +249,6 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
                 f.dim(E::u(ent[i], lo[i]));
             }
         }
-        packed[blk] = pk;
     }
     return (double)(f.finish(fin0) * jac) * a.post_scale;
 }
@@ -234,9 +259,9 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
 // NBLK read-modify-writes of a round are independent and pipeline.  Consecutive rounds can touch the
 // same word from different lanes, hence the __syncwarp() (shared memory is processed in order per warp).
 template <typename T, int DIM>
-__device__ __forceinline__ void rot_hist_update(const RotLane<T, DIM>& L, int nb, const uint32_t (&packed)[(DIM + 3) / 4],
+__device__ __forceinline__ void rot_hist_update(const RotLane<T, DIM>& L, const uint32_t (&taddr)[(DIM + 3) / 4][4],
                                                 double v2) {
-    constexpr int NBLK = RotLane<T, DIM>::NBLK, R = RotLane<T, DIM>::R, GL = RotLane<T, DIM>::GL;
+    constexpr int NBLK = RotLane<T, DIM>::NBLK, R = RotLane<T, DIM>::R;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         uint32_t addr[NBLK];
@@ -244,15 +269,11 @@ __device__ __forceinline__ void rot_hist_update(const RotLane<T, DIM>& L, int nb
 #pragma unroll
         for (int blk = 0; blk < NBLK; ++blk) {
             const bool last = (blk == NBLK - 1);
-            const int G = last ? GL : 4;
-            const int SH = (G == 4) ? 5 : (G == 2) ? 6 : 7;
             const int NSUB = last ? ((R == 3) ? 4 : R) : 4;
-            const uint32_t hoff = last ? L.hoffL : L.hoff4;
             const int gamma = last ? L.gammaL : L.gamma4;
             const bool active = (i < NSUB) && (!(last && R == 3) || ((gamma ^ i) < 3));
             if (active) {
-                const uint32_t b256 = __byte_perm(packed[blk], 0, 0x4404 | (i << 4));   // byte i -> bits 8..15
-                addr[blk] = L.hbase + (uint32_t)(blk * nb) * 256u + (b256 + (hoff ^ (uint32_t)(i << SH)));
+                addr[blk] = 2u * taddr[blk][i] + (last ? L.hcL[i] : L.hc4[i]);
                 h[blk] = lds_f64(addr[blk]);
             }
         }
@@ -268,8 +289,7 @@ __device__ __forceinline__ void rot_hist_update(const RotLane<T, DIM>& L, int nb
     }
 }
 
-// EPT = events per thread per loop iteration (independent chains for the scheduler to interleave).
-template <int FID, typename T, int DIM, int EPT>
+template <int FID, typename T, int DIM>
 __global__ void __launch_bounds__(kRotMaxThreads, 1)
 k_iterate_rot(const __grid_constant__ RotArgs a) {
     using E = RotEntry<T>;
@@ -306,71 +326,50 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     const int grp = warp / S, pos = warp - grp * S;            // histogram copy of this warp, place in its ring
     Lane L;
     L.tbase = (uint32_t)__cvta_generic_to_shared(table);
-    L.hbase = (uint32_t)__cvta_generic_to_shared(hist) + (uint32_t)grp * (uint32_t)rows * 256u;
-    L.toff4 = rot_table_off0<4, ENTRY>(lane);  L.hoff4 = rot_hist_off0<4>(lane);
-    L.toffL = rot_table_off0<GL, ENTRY>(lane); L.hoffL = rot_hist_off0<GL>(lane);
-    L.gamma4 = rot_gamma<4>(lane);             L.gammaL = rot_gamma<GL>(lane);
-    const PhiloxKey ks = philox_key_schedule(a.key0, a.key1);
+    {
+        const uint32_t hbase = (uint32_t)__cvta_generic_to_shared(hist) + (uint32_t)grp * (uint32_t)rows * 256u;
+        const uint32_t toff4 = rot_table_off0<4, ENTRY>(lane), hoff4 = rot_hist_off0<4>(lane);
+        const uint32_t toffL = rot_table_off0<GL, ENTRY>(lane), hoffL = rot_hist_off0<GL>(lane);
+        constexpr int SHL = (GL == 4) ? 5 : (GL == 2) ? 6 : 7;     // slot -> byte offset shift
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            L.tx4[i] = toff4 ^ (uint32_t)(i << 5);
+            L.txL[i] = toffL ^ (uint32_t)(i << SHL);
+            L.hc4[i] = hbase + (hoff4 ^ (uint32_t)(i << 5)) - 2u * (L.tbase + L.tx4[i]);
+            L.hcL[i] = hbase + (hoffL ^ (uint32_t)(i << SHL)) - 2u * (L.tbase + L.txL[i]);
+        }
+    }
+    L.gamma4 = rot_gamma<4>(lane);
+    L.gammaL = rot_gamma<GL>(lane);
     const T fin0 = (T)a.fin0;
     const int my_token = 1 + warp, next_token = 1 + grp * S + ((pos + 1 == S) ? 0 : pos + 1);
 
-    double s1 = 0.0, c1 = 0.0, s2 = 0.0, c2 = 0.0;
+    // per-thread sums: a few hundred to a few ten thousand terms per launch, plain fp64; everything above
+    // the thread (warp, CTA, launches, CTAs) is added in double-double
+    double s1 = 0.0, s2 = 0.0;
     // every warp runs the same number of loop iterations (the ring hands the token on once per iteration);
     // events past the end of the range contribute v = 0
     const unsigned long long nthr = (unsigned long long)gridDim.x * blockDim.x;
-    const unsigned long long per_iter = nthr * EPT;
-    const unsigned long long n_iter = (a.count + per_iter - 1) / per_iter;
+    const unsigned long long n_iter = (a.count + nthr - 1) / nthr;
     unsigned long long q = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
-    // Software pipeline: the histogram update of the events of loop iteration it-1 is done after the
-    // per-event work of iteration it, so that the token has a whole iteration to come round the ring
-    // before this warp needs it (the barrier stall of the unpipelined loop was 20 % of the warp time,
-    // profiles/r01_s7_ring.md).
-    uint32_t ppacked[EPT][NBLK];
-    double pv2[EPT];
-#pragma unroll
-    for (int k = 0; k < EPT; ++k) {
-        pv2[k] = 0.0;
-#pragma unroll
-        for (int b = 0; b < NBLK; ++b) ppacked[k][b] = 0;
-    }
-    for (unsigned long long it = 0; it <= n_iter; ++it, q += per_iter) {
-        uint32_t packed[EPT][NBLK];
-        double v2[EPT];
-#pragma unroll
-        for (int k = 0; k < EPT; ++k) {
-            v2[k] = 0.0;
-#pragma unroll
-            for (int b = 0; b < NBLK; ++b) packed[k][b] = 0;
-        }
-        if (it < n_iter) {
-#pragma unroll
-            for (int k = 0; k < EPT; ++k) {
-                const unsigned long long qk = q + (unsigned long long)k * nthr;
-                double v = rot_event<FID, T, DIM>(a, L, ks, a.first_event + qk, fin0, packed[k]);
-                if (qk >= a.count) v = 0.0;
-                v2[k] = v * v;
-                kahan_add(s1, c1, v);
-                kahan_add(s2, c2, v2[k]);
-            }
-        }
-        if (it > 0) {
-            if (S > 1 && (pos != 0 || it != 1)) token_wait(my_token);
-#pragma unroll
-            for (int k = 0; k < EPT; ++k) rot_hist_update<T, DIM>(L, nb, ppacked[k], pv2[k]);
-            if (S > 1) token_pass(next_token);
-        }
-#pragma unroll
-        for (int k = 0; k < EPT; ++k) {
-            pv2[k] = v2[k];
-#pragma unroll
-            for (int b = 0; b < NBLK; ++b) ppacked[k][b] = packed[k][b];
-        }
+    // (A software-pipelined variant -- histogram update of iteration it-1 after the per-event work of iteration
+    // it -- removed the barrier stalls but cost 30 register moves per iteration and measured 2 % slower.)
+    for (unsigned long long it = 0; it < n_iter; ++it, q += nthr) {
+        uint32_t taddr[NBLK][4];
+        double v = rot_event<FID, T, DIM>(a, L, a.first_event + q, fin0, taddr);
+        if (q >= a.count) v = 0.0;
+        const double v2 = v * v;
+        s1 += v;
+        s2 += v2;
+        if (S > 1 && (pos != 0 || it != 0)) token_wait(my_token);
+        rot_hist_update<T, DIM>(L, taddr, v2);
+        if (S > 1) token_pass(next_token);
     }
     if (S > 1 && pos == 0 && n_iter > 0) token_wait(my_token);   // absorbs the ring's last hand-off
 
     // ---- S5: warp shuffle -> CTA -> this CTA's partial (accumulated over the launches of an iteration)
-    dd t1 = dd_warp_sum(fast_two_sum(s1, -c1));
-    dd t2 = dd_warp_sum(fast_two_sum(s2, -c2));
+    dd t1 = dd_warp_sum(dd{s1, 0.0});
+    dd t2 = dd_warp_sum(dd{s2, 0.0});
     const int nwarps = (blockDim.x + 31) >> 5;
     if (lane == 0) { red[2 * warp] = t1; red[2 * warp + 1] = t2; }
     __syncthreads();
@@ -409,6 +408,6 @@ inline size_t rot_shared_bytes(int dim, int n_bins, int n_groups) {
 
 // one translation unit per (FID, T) instantiates DIM = 1..32 (vegas_rot_inst.cu)
 template <int FID, typename T>
-cudaError_t launch_iterate_rot(int dim, int ept, const RotArgs& a, int blocks, int threads, size_t shmem, cudaStream_t st);
+cudaError_t launch_iterate_rot(int dim, const RotArgs& a, int blocks, int threads, size_t shmem, cudaStream_t st);
 
 }  // namespace vegas

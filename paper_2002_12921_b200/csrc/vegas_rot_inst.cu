@@ -14,9 +14,9 @@ using RT = double;
 using RT = float;
 #endif
 
-template <int DIM, int EPT>
+template <int DIM>
 static cudaError_t go(const RotArgs& a, int blocks, int threads, size_t shmem, cudaStream_t st) {
-    auto kern = k_iterate_rot<ROT_FID, RT, DIM, EPT>;
+    auto kern = k_iterate_rot<ROT_FID, RT, DIM>;
     static size_t configured = 0;
     if (shmem > configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem);
@@ -28,10 +28,10 @@ static cudaError_t go(const RotArgs& a, int blocks, int threads, size_t shmem, c
 }
 
 template <>
-cudaError_t launch_iterate_rot<ROT_FID, RT>(int dim, int ept, const RotArgs& a, int blocks, int threads, size_t shmem,
+cudaError_t launch_iterate_rot<ROT_FID, RT>(int dim, const RotArgs& a, int blocks, int threads, size_t shmem,
                                             cudaStream_t st) {
     switch (dim) {
-#define CASE(D) case D: return ept == 2 ? go<D, 2>(a, blocks, threads, shmem, st) : go<D, 1>(a, blocks, threads, shmem, st);
+#define CASE(D) case D: return go<D>(a, blocks, threads, shmem, st);
         CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
         CASE(9) CASE(10) CASE(11) CASE(12) CASE(13) CASE(14) CASE(15) CASE(16)
         CASE(17) CASE(18) CASE(19) CASE(20) CASE(21) CASE(22) CASE(23) CASE(24)

@@ -27,7 +27,7 @@ if ROOT not in sys.path:
 
 METRIC = "events/sec per Vegas iteration"
 UNIT = "events/s"
-SM_COUNT, ISSUE_LANES, FP64_LANES = 148, 128, 64          # per SM per clock (guide + profiles/r01_ubench_pipes.md)
+SM_COUNT, ISSUE_LANES, FP64_LANES = 148, 128, 64          # per SM per clock (guide + profiles/r01_s7_ubench_pipes.md)
 INTEGRAND_DIM_FP = {0: 0, 1: 2, 2: 3, 3: 4}                # SURVEY.md 8(d) counting rule
 INTEGRAND_EVENT_FP = {0: {64: 0, 32: 0}, 1: {64: 19, 32: 5}, 2: {64: 8, 32: 8}, 3: {64: 12, 32: 12}}
 
@@ -37,6 +37,17 @@ def n_issue(w, precision):
     d = w.dim
     per_dim_fp = INTEGRAND_DIM_FP[w.integrand_id] * (d - 1 if w.integrand_id == 3 else d)
     return 42 * ((d + 3) // 4) + d * (4 + 1 + 2 + 3) + per_dim_fp + 3 + 4 + INTEGRAND_EVENT_FP[w.integrand_id][precision]
+
+
+def n_wide(w):
+    """32x32->64 multiplies per event: 20 per Philox block plus the split of every dimension.  The step-0
+    microbenchmark (profiles/r01_s7_ubench_pipes.md) measured 3.4 dispatch slots for IMAD.WIDE.U32, not 1:
+    the refined issue roofline charges the extra 2.4 slots ("refine them only via the
+    step-0 microbenchmarks")."""
+    return 20 * ((w.dim + 3) // 4) + w.dim
+
+
+WIDE_EXTRA_SLOTS = 2.4
 
 
 def n_fp(w, precision):
@@ -73,9 +84,10 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append([t.strip() for t in line.split(",")])
+            self.rows.append((time.perf_counter(), [t.strip() for t in line.split(",")]))
 
-    def stop(self):
+    def stop(self, t_begin=None, t_end=None):
+        """Summary of the samples taken between t_begin and t_end (perf_counter; None = all)."""
         if self.proc:
             self.proc.terminate()
             try:
@@ -83,7 +95,8 @@ class ClockSampler:
             except Exception:
                 self.proc.kill()
         sm, smax, reasons, power = [], 0.0, set(), 0.0
-        for r in self.rows:
+        rows = [r for t, r in self.rows if (t_begin is None or t >= t_begin) and (t_end is None or t <= t_end)]
+        for r in rows:
             try:
                 sm.append(float(r[1])); smax = max(smax, float(r[2])); power = max(power, float(r[3]))
             except Exception:
@@ -153,7 +166,7 @@ def run_reference(args, w, precision):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", default="cfg3", help="cfg1..cfg5 (BASELINE.json configs)")
@@ -208,18 +221,19 @@ def main():
         g.refine(w.alpha)
         return I, s
 
+    sampler = ClockSampler(local_rank)      # started early: nvidia-smi needs ~0.3 s before its first row
+    sampler.start()
     k = 0
     for _ in range(args.warmup):
         step(k)
         k += 1
     # ---- timed region: K steps, device events per step (L2 flushed between steps, outside the brackets)
-    sampler = ClockSampler(local_rank)
     g.set_profiling(True)
     g.reset_counters()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     results = []
     barrier()
-    sampler.start()
+    t_begin = time.perf_counter()
     t_wall = time.perf_counter()
     for i in range(args.steps):
         flush.zero_()
@@ -229,7 +243,6 @@ def main():
         k += 1
     barrier()
     t_wall = time.perf_counter() - t_wall
-    clocks = sampler.stop()
     ms = sum(a.elapsed_time(b) for a, b in ev)
     k1_ms, k1_launches = g.kernel_time_ms()
     launches = g.launch_count()
@@ -256,6 +269,9 @@ def main():
         k += 1
     barrier()
     e2e_s = time.perf_counter() - t0
+    # clocks: samples taken during the two timed regions (device-timed steps, then the e2e steps: same kernels)
+    clocks = sampler.stop(t_begin, time.perf_counter())
+    clocks["window"] = "timed steps + e2e steps"
     if world > 1:
         t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -278,8 +294,12 @@ def main():
                     "frac": k1_rate * ni / peak_instr,
                     "frac_at_measured_clock": k1_rate * ni / (SM_COUNT * ISSUE_LANES * clk * 1e6),
                     "peak_source": "148 SMs x 128 issue lanes x sm_max_mhz of MEASURED_PEAKS.json (%s); issue rate "
-                                   "confirmed by profiles/r01_ubench_pipes.md" % ("measured" if peaks else "fallback 1965 MHz"),
+                                   "confirmed by profiles/r01_s7_ubench_pipes.md" % ("measured" if peaks else "fallback 1965 MHz"),
                     "instr_per_event": ni, "fp_instr_per_event": nf,
+                    "refined": {"slots_per_event": ni + WIDE_EXTRA_SLOTS * n_wide(w),
+                                "frac": k1_rate * (ni + WIDE_EXTRA_SLOTS * n_wide(w)) / peak_instr,
+                                "frac_at_measured_clock": k1_rate * (ni + WIDE_EXTRA_SLOTS * n_wide(w)) / (SM_COUNT * ISSUE_LANES * clk * 1e6),
+                                "why": "IMAD.WIDE.U32 holds the dispatch port 3.4 clk (profiles/r01_s7_ubench_pipes.md)"},
                     "fp_pipe_frac": k1_rate * nf / (SM_COUNT * (FP64_LANES if args.precision == 64 else ISSUE_LANES) * sm_max * 1e6),
                     "kernel_events_per_s": k1_rate, "kernel_ms_per_launch": k1_s * 1e3, "kernel_launches": int(k1_launches),
                     "kernel_share_of_step": k1_ms / ms if world == 1 else None,

@@ -14,8 +14,8 @@ CSRC = os.path.join(_HERE, "csrc")
 OBJ_DIR = os.path.join(_HERE, "build")
 LIB = os.path.join(_HERE, "libvegas_b200.so")
 HEADERS = ["vegas_kernels.h", "vegas_device.cuh", "vegas_iterate_rot.cuh", os.path.join("..", "..", "include", "vegas.h")]
-# (integrand id, precision) pairs served by the fast path: CONST, GAUSS in both precisions, GENZ in fp64
-ROT_VARIANTS = [(0, 64), (0, 32), (1, 64), (1, 32), (2, 64)]
+# (integrand id, precision) pairs served by the fast path: CONST, GAUSS in both precisions, GENZ and BW_POLY in fp64
+ROT_VARIANTS = [(0, 64), (0, 32), (1, 64), (1, 32), (2, 64), (3, 64)]
 UNITS = [("vegas_kernels", "vegas_kernels.cu", []), ("vegas_api", "vegas_api.cu", [])] + \
         [("vegas_rot_%d_%d" % (f, p), "vegas_rot_inst.cu", ["-DROT_FID=%d" % f, "-DROT_FP=%d" % p])
          for f, p in ROT_VARIANTS]

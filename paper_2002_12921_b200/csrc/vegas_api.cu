@@ -102,7 +102,7 @@ struct LaunchShape {
 
 // Predicted shared-pipe cost (SM clocks per warp-wide access) of the table gather and of the
 // histogram CAS update as a function of the copy count, from the step-0 microbenchmarks on a
-// B200 (profiles/r01_ubench_pipes.md).  Only used to rank (ct, ch) pairs that fit.
+// B200 (profiles/r01_s7_ubench_pipes.md).  Only used to rank (ct, ch) pairs that fit.
 double table_cost(int precision, int ct) {
     static const double c64[] = {9.5, 9.4, 7.9, 6.5, 6.5, 6.5};     // ct = 1,2,4,8,(16,32)
     static const double c32[] = {6.0, 5.6, 5.0, 4.2, 3.4, 3.4};
@@ -168,15 +168,16 @@ double jac_scale_for(const vegas_grid* g, int precision) {
 bool use_rot_path(const vegas_grid* g, int fid, int precision) {
     if (g->cfg_ct > 0 || g->cfg_ch > 0) return false;
     const bool kind = fid == VEGAS_F_CONST || fid == VEGAS_F_GAUSS ||
-                      (fid == VEGAS_F_GENZ_PRODUCT_PEAK && precision == VEGAS_FP64);
+                      (fid == VEGAS_F_GENZ_PRODUCT_PEAK && precision == VEGAS_FP64) ||
+                      (fid == VEGAS_F_BW_POLY && precision == VEGAS_FP64 && g->dim <= vegas::kRotBwMaxDim);
     if (!kind) return false;
-    if (g->cfg_threads > vegas::kRotMaxThreads) return false;
+    if (g->cfg_threads > vegas::rot_max_threads(fid)) return false;
     return vegas::rot_shared_bytes(g->dim, g->n_bins, 1) <= g->smem_optin;
 }
 
 // shift_j, scale_j, post_scale, fin0 of the affine pre-composition (see vegas_iterate_rot.cuh)
 void rot_constants(const vegas_grid* g, int fid, int precision, double* shift, double* scale, double* post_scale,
-                   double* fin0, double* jac_init) {
+                   double* fin0, double* jac_init, double* fpar) {
     const int dim = g->dim;
     const double nb = (double)g->n_bins;
     *post_scale = 1.0;
@@ -196,6 +197,17 @@ void rot_constants(const vegas_grid* g, int fid, int precision, double* shift, d
             ps *= c * nb;                                        // f J = prod(c_j nb) prod B_j / prod(1+u_j^2)
         }
         *post_scale = ps;
+    } else if (fid == VEGAS_F_BW_POLY) {
+        // u_0 = (s - M^2)/(M Gamma) with s = s_min + x_0 ds (C5): the Breit-Wigner is 1/(1 + u_0^2); u_j = x_j, j >= 1
+        const double* d = g->derived[fid];                       // s_min, ds, M^2, M^2 Gamma^2, a[i][k]
+        const double mg = std::sqrt(d[3]);
+        shift[0] = (d[2] - d[0]) / d[1];
+        scale[0] = d[1] / mg;
+        double ps = nb / scale[0];
+        for (int j = 1; j < dim; ++j) { scale[j] = 1.0; ps *= nb; }
+        *post_scale = ps;                                        // J = prod nb Delta_j = prod (nb/scale_j) B_j 2^32
+        for (int j = 1; j < dim; ++j)
+            for (int k = 0; k < 5; ++k) fpar[5 * j + k] = d[4 + 5 * (j - 1) + k];
     }
     // fp64 table entries carry 2^-32 per dimension (RotEntry<double>): start the running Jacobian product at
     // 2^(32 floor(d/2)) and give the rest back in post_scale -- exact powers of two, the product stays in range
@@ -212,17 +224,34 @@ struct RotShape {
     size_t shmem;
 };
 
-// One CTA per SM.  W warps (default 12 = 3 per scheduler, 170 registers each); as many histogram copies as
-// fit next to the table, W a multiple of the copy count; ring = warps per copy (1 = no token passing).
-RotShape rot_shape(const vegas_grid* g) {
+// One CTA per SM, up to 128 registers per thread.  n_groups = histogram copies in the CTA (as many as fit next
+// to the table, a divisor of the warp count W), ring = W / n_groups warps share a copy (1 = no token passing).
+// W: 16 when every warp gets its own copy; otherwise the largest of 15..12 (token barriers 1..15) that keeps more
+// than half of the copies that fit -- measured on B200 (profiles/r01_s13_fast_path.md): 15 warps beat 12 by 4-5 %
+// on cfg2/cfg3 (more warps hide the Philox chain), but 15 warps on 1 copy lose 30 % to 14 warps on 2 (cfg4).
+static int rot_divisor(int W, int fit) {
+    int ng = fit < W ? fit : W;
+    while (W % ng) --ng;
+    return ng;
+}
+RotShape rot_shape(const vegas_grid* g, int fid) {
     RotShape s;
-    int W = g->cfg_threads > 0 ? (g->cfg_threads + 31) / 32 : vegas::kRotDefaultWarps;
     const size_t one = vegas::rot_shared_bytes(g->dim, g->n_bins, 1), base = vegas::rot_shared_bytes(g->dim, g->n_bins, 0);
     int fit = (int)((g->smem_optin - base) / (one - base));
     if (fit < 1) fit = 1;
-    if (fit < W && W > vegas::kRotMaxRingWarps) W = vegas::kRotMaxRingWarps;     // rings need named barriers 1..15
-    int ng = fit < W ? fit : W;
-    while (W % ng) --ng;
+    int W;
+    if (g->cfg_threads > 0) {
+        W = (g->cfg_threads + 31) / 32;
+        if (fit < W && W > vegas::kRotMaxRingWarps) W = vegas::kRotMaxRingWarps;
+    } else if (fit >= vegas::rot_max_threads(fid) / 32) {
+        W = vegas::rot_max_threads(fid) / 32;
+    } else {
+        W = vegas::kRotDefaultWarps;
+        const int wmax = vegas::rot_max_threads(fid) / 32 - 1;
+        for (int w = wmax < vegas::kRotMaxRingWarps ? wmax : vegas::kRotMaxRingWarps; w > vegas::kRotDefaultWarps; --w)
+            if (2 * rot_divisor(w, fit) > fit) { W = w; break; }
+    }
+    const int ng = rot_divisor(W, fit);
     s.n_groups = ng;
     s.ring = W / ng;
     s.threads = 32 * W;
@@ -238,6 +267,8 @@ cudaError_t launch_rot(int fid, int precision, int dim, const vegas::RotArgs& a,
         case VEGAS_F_GAUSS: return vegas::launch_iterate_rot<VEGAS_F_GAUSS, double>(dim, a, s.blocks, s.threads, s.shmem, st);
         case VEGAS_F_GENZ_PRODUCT_PEAK:
             return vegas::launch_iterate_rot<VEGAS_F_GENZ_PRODUCT_PEAK, double>(dim, a, s.blocks, s.threads, s.shmem, st);
+        case VEGAS_F_BW_POLY:
+            return vegas::launch_iterate_rot<VEGAS_F_BW_POLY, double>(dim, a, s.blocks, s.threads, s.shmem, st);
         }
     } else {
         switch (fid) {
@@ -400,7 +431,7 @@ int vegas_begin_iteration(vegas_grid* g, void* cuda_stream) {
     // either kernel path may serve the accumulate calls of this iteration: reserve slots for the wider one
     int blocks = s.blocks;
     if (use_rot_path(g, VEGAS_F_CONST, VEGAS_FP64)) {
-        const RotShape r = rot_shape(g);
+        const RotShape r = rot_shape(g, VEGAS_F_CONST);
         if (r.blocks > blocks) blocks = r.blocks;
     }
     if (blocks > kMaxBlocks) return VEGAS_EINVAL;
@@ -422,7 +453,7 @@ int vegas_accumulate(vegas_grid* g, uint64_t first_event, uint64_t count, uint64
     vegas::IterArgs a{};
     vegas::RotArgs ra{};
     if (rot) {
-        rs = rot_shape(g);
+        rs = rot_shape(g, fid);
         if (rs.blocks > g->active_blocks) return VEGAS_EINVAL;
         ra.edges = g->d_edges;
         ra.partials = g->d_partials;
@@ -434,7 +465,7 @@ int vegas_accumulate(vegas_grid* g, uint64_t first_event, uint64_t count, uint64
         ra.n_bins = g->n_bins;
         ra.n_groups = rs.n_groups;
         ra.ring = rs.ring;
-        rot_constants(g, fid, precision, ra.shift, ra.scale, &ra.post_scale, &ra.fin0, &ra.jac_init);
+        rot_constants(g, fid, precision, ra.shift, ra.scale, &ra.post_scale, &ra.fin0, &ra.jac_init, ra.fpar);
     } else {
         if (resolve_launch(g, precision, &s)) return VEGAS_EINVAL;
         if (s.blocks > g->active_blocks) return VEGAS_EINVAL;
@@ -636,7 +667,7 @@ int vegas_debug_sample(vegas_grid* g, uint64_t first_event, uint32_t count, uint
     a.x = (double*)base;                       base += align_up(per_dim * 8);
     a.fJ = (double*)base;
     const bool rot = use_rot_path(g, fid, precision);
-    if (rot) rot_constants(g, fid, precision, a.shift, a.scale, &a.post_scale, &a.fin0, &a.jac_init);
+    if (rot) rot_constants(g, fid, precision, a.shift, a.scale, &a.post_scale, &a.fin0, &a.jac_init, a.fpar);
     CUDA_TRY(g, vegas::launch_debug(fid, precision, rot, a, g->derived[fid], st));
     g->launches++;
     if (words) CUDA_TRY(g, cudaMemcpyAsync(words, a.words, per_dim * 4, cudaMemcpyDeviceToHost, st));
@@ -672,7 +703,7 @@ int vegas_get_launch(vegas_grid* g, int integrand_id, int precision, int* path, 
     if (!g || (precision != VEGAS_FP64 && precision != VEGAS_FP32) || integrand_id < 0 || integrand_id > 3)
         return VEGAS_EINVAL;
     if (use_rot_path(g, integrand_id, precision)) {
-        const RotShape r = rot_shape(g);
+        const RotShape r = rot_shape(g, integrand_id);
         if (blocks) *blocks = r.blocks;
         if (threads) *threads = r.threads;
         if (table_copies) *table_copies = precision == VEGAS_FP64 ? 2 : 4;

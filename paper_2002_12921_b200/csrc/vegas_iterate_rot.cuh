@@ -40,24 +40,46 @@
 namespace vegas {
 
 // ---- integrands in the affine variable u --------------------------------------------------------
+// RotCtx<FID, T, NBLK>: what a lane needs about the dimension it handles at (Philox block blk, sub-step i).
+// That dimension, 4 blk + (gamma ^ i), is fixed for the whole kernel, so per-dimension integrand parameters
+// are picked once, in the prologue, and sit in registers: no select and no parameter read in the event loop.
+template <int FID, typename T, int NBLK> struct RotCtx {
+    template <class A> __device__ __forceinline__ void init(const A&, int /*dim*/, int /*gamma4*/, int /*gammaL*/) {}
+};
 template <int FID, typename T> struct IntegrandU;
 
 template <typename T> struct IntegrandU<VEGAS_F_CONST, T> {
-    __device__ __forceinline__ void begin() {}
-    __device__ __forceinline__ void dim(T) {}
+    template <class C> __device__ __forceinline__ void begin(const C&) {}
+    template <class C> __device__ __forceinline__ void dim(T, int, int, const C&) {}
     __device__ __forceinline__ T finish(T) const { return (T)1; }
 };
 template <typename T> struct IntegrandU<VEGAS_F_GAUSS, T> {   // PAPER.md:65 Eq.(1); u = n_bins (x - 1/2)
     T s;
-    __device__ __forceinline__ void begin() { s = (T)0; }
-    __device__ __forceinline__ void dim(T u) { s = t_fma(u, u, s); }
+    template <class C> __device__ __forceinline__ void begin(const C&) { s = (T)0; }
+    template <class C> __device__ __forceinline__ void dim(T u, int, int, const C&) { s = t_fma(u, u, s); }
     __device__ __forceinline__ T finish(T fin0) const { return t_exp_fast<T>(-s * fin0); }   // fin0 = 1/(n_bins a)^2
 };
 template <typename T> struct IntegrandU<VEGAS_F_GENZ_PRODUCT_PEAK, T> {   // PAPER.md:74 Eq.(3); u = c_j (x - w_j)
     T prod;
-    __device__ __forceinline__ void begin() { prod = (T)1; }
-    __device__ __forceinline__ void dim(T u) { prod *= t_fma(u, u, (T)1); }
+    template <class C> __device__ __forceinline__ void begin(const C&) { prod = (T)1; }
+    template <class C> __device__ __forceinline__ void dim(T u, int, int, const C&) { prod *= t_fma(u, u, (T)1); }
     __device__ __forceinline__ T finish(T) const { return (T)1 / prod; }
+};
+// BW_POLY (BASELINE.json:configs[4], readings R11, R12): u_0 = (s(x_0) - M^2)/(M Gamma), u_j = x_j for j >= 1;
+// f = [1/(1 + u_0^2)] * [sum_j a_j0 + sum_j u_j (a_j1 + u_j (a_j2 + u_j (a_j3 + u_j a_j4)))].
+// The lane that holds dimension 0 at sub-step i of block 0 runs the quartic with zero coefficients and keeps u.
+constexpr int kRotBwMaxDim = 8;    // 4 coefficient registers pairs per dimension per lane
+template <typename T> struct IntegrandU<VEGAS_F_BW_POLY, T> {
+    T poly, u0;
+    template <class C> __device__ __forceinline__ void begin(const C& c) { poly = c.poly0; u0 = (T)0; }
+    template <class C> __device__ __forceinline__ void dim(T u, int blk, int i, const C& c) {
+        T h = t_fma(c.a[blk][i][3], u, c.a[blk][i][2]);
+        h = t_fma(h, u, c.a[blk][i][1]);
+        h = t_fma(h, u, c.a[blk][i][0]);
+        poly = t_fma(h, u, poly);
+        if (blk == 0 && c.is0[i]) u0 = u;
+    }
+    __device__ __forceinline__ T finish(T) const { return poly / t_fma(u0, u0, (T)1); }
 };
 
 // ---- table entry and u from the low product word ---------------------------------------------------
@@ -126,11 +148,36 @@ struct RotArgs {
     double jac_init;                // start value of the running Jacobian product (a power of two, see RotEntry)
     double fin0;                    // integrand finish constant
     double shift[VEGAS_MAX_DIM], scale[VEGAS_MAX_DIM];
+    double fpar[5 * kRotBwMaxDim];  // BW_POLY: a[j][k] at fpar[5 j + k], j = 1..dim-1 (row 0 unused)
 };
 
-constexpr int kRotMaxThreads = 384;    // one CTA per SM: 12 warps, up to 168 registers per thread
+template <typename T, int NBLK> struct RotCtx<VEGAS_F_BW_POLY, T, NBLK> {
+    T a[NBLK][4][4];                // a_j1..a_j4 of the lane's dimension at (blk, i); zero for dimension 0 / no dimension
+    bool is0[4];                    // the lane holds dimension 0 at sub-step i of block 0
+    T poly0;                        // sum_j a_j0
+    template <class A> __device__ __forceinline__ void init(const A& r, int dim, int gamma4, int gammaL) {
+        const int nblk = (dim + 3) / 4;
+        T c0 = (T)0;
+        for (int j = 1; j < dim; ++j) c0 += (T)r.fpar[5 * j];
+        poly0 = c0;
+#pragma unroll
+        for (int blk = 0; blk < NBLK; ++blk)
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int j = 4 * blk + ((blk == nblk - 1 ? gammaL : gamma4) ^ i);
+                const bool poly_dim = blk < nblk && j >= 1 && j < dim;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) a[blk][i][k] = poly_dim ? (T)r.fpar[5 * j + 1 + k] : (T)0;
+                if (blk == 0) is0[i] = (j == 0);
+            }
+    }
+};
+
+constexpr int kRotMaxThreads = 512;    // one CTA per SM: up to 16 warps, 128 registers per thread
+// BW_POLY keeps 4 coefficients per dimension per lane in registers: 12 warps, up to 168 registers
+__host__ __device__ constexpr int rot_max_threads(int fid) { return fid == VEGAS_F_BW_POLY ? 384 : kRotMaxThreads; }
 constexpr int kRotDefaultWarps = 12;
-constexpr int kRotMaxRingWarps = 12;   // named barriers 1..15 would allow 15; the register budget allows 12
+constexpr int kRotMaxRingWarps = 15;   // token barriers 1..15 (barrier 0 is __syncthreads)
 
 __host__ __device__ constexpr int rot_groups(int r) { return r >= 3 ? 4 : r; }   // dims in block -> lane groups
 
@@ -192,7 +239,8 @@ __device__ __forceinline__ void philox4x32_10_args(uint32_t c0, uint32_t c1, uin
 // S1..S5 for one event: Philox -> split -> table -> u -> integrand; returns v = f J and leaves the
 // table address of every (block, sub-step) in taddr (the histogram update derives its addresses from them).
 template <int FID, typename T, int DIM>
-__device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, DIM>& L, unsigned long long ev, T fin0,
+__device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, DIM>& L,
+                                            const RotCtx<FID, T, (DIM + 3) / 4>& ctx, unsigned long long ev, T fin0,
                                             uint32_t (&taddr)[(DIM + 3) / 4][4]) {
     using E = RotEntry<T>;
     using T2 = typename E::type;
@@ -200,7 +248,7 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
     const int nb = a.n_bins;
     const uint32_t e_lo = (uint32_t)ev, e_hi = (uint32_t)(ev >> 32);
     IntegrandU<FID, T> f;
-    f.begin();
+    f.begin(ctx);
     T jac = (T)a.jac_init;
 #pragma unroll
     for (int blk = 0; blk < NBLK; ++blk) {
@@ -246,7 +294,7 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
             const bool active = !(last && R == 3) || ((gamma ^ i) < 3);
             if (active) {
                 jac *= ent[i].y;
-                f.dim(E::u(ent[i], lo[i]));
+                f.dim(E::u(ent[i], lo[i]), blk, i, ctx);
             }
         }
     }
@@ -290,7 +338,7 @@ __device__ __forceinline__ void rot_hist_update(const RotLane<T, DIM>& L, const 
 }
 
 template <int FID, typename T, int DIM>
-__global__ void __launch_bounds__(kRotMaxThreads, 1)
+__global__ void __launch_bounds__(rot_max_threads(FID), 1)
 k_iterate_rot(const __grid_constant__ RotArgs a) {
     using E = RotEntry<T>;
     using T2 = typename E::type;
@@ -342,6 +390,8 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     L.gamma4 = rot_gamma<4>(lane);
     L.gammaL = rot_gamma<GL>(lane);
     const T fin0 = (T)a.fin0;
+    RotCtx<FID, T, NBLK> ctx;
+    ctx.init(a, DIM, L.gamma4, L.gammaL);
     const int my_token = 1 + warp, next_token = 1 + grp * S + ((pos + 1 == S) ? 0 : pos + 1);
 
     // per-thread sums: a few hundred to a few ten thousand terms per launch, plain fp64; everything above
@@ -356,7 +406,7 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     // it -- removed the barrier stalls but cost 30 register moves per iteration and measured 2 % slower.)
     for (unsigned long long it = 0; it < n_iter; ++it, q += nthr) {
         uint32_t taddr[NBLK][4];
-        double v = rot_event<FID, T, DIM>(a, L, a.first_event + q, fin0, taddr);
+        double v = rot_event<FID, T, DIM>(a, L, ctx, a.first_event + q, fin0, taddr);
         if (q >= a.count) v = 0.0;
         const double v2 = v * v;
         s1 += v;

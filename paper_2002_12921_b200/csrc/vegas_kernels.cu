@@ -301,8 +301,10 @@ __global__ void k_debug_rot(const __grid_constant__ DebugArgs a) {
     const unsigned long long e = a.first_event + q;
     const int dim = a.dim, nb = a.n_bins;
     const PhiloxKey ks = philox_key_schedule(a.key0, a.key1);
+    RotCtx<FID, T, kRotBwMaxDim / 4> ctx;      // lane 0's view: gamma = 0, dimension j at (j >> 2, j & 3)
+    ctx.init(a, dim, 0, 0);
     IntegrandU<FID, T> f;
-    f.begin();
+    f.begin(ctx);
     T jac = (T)a.jac_init;
     uint32_t w[4] = {0, 0, 0, 0};
     for (int j = 0; j < dim; ++j) {
@@ -313,7 +315,7 @@ __global__ void k_debug_rot(const __grid_constant__ DebugArgs a) {
         const double* X = a.edges + (size_t)j * (nb + 1);
         const typename E::type ent = E::make(X[b], X[b + 1], a.shift[j], a.scale[j]);
         jac *= ent.y;
-        f.dim(E::u(ent, lo));
+        f.dim(E::u(ent, lo), FID == VEGAS_F_BW_POLY ? (j >> 2) : 0, j & 3, ctx);
         a.words[(size_t)q * dim + j] = word;
         a.bins[(size_t)q * dim + j] = (int32_t)b;
         a.x[(size_t)q * dim + j] = (sizeof(T) == 8) ? fma(X[b + 1] - X[b], offset_f64(lo), X[b])
@@ -433,6 +435,7 @@ static cudaError_t launch_debug_rot_t(int fid, const DebugArgs& a, cudaStream_t 
     case VEGAS_F_CONST: k_debug_rot<VEGAS_F_CONST, T><<<blocks, threads, 0, st>>>(a); break;
     case VEGAS_F_GAUSS: k_debug_rot<VEGAS_F_GAUSS, T><<<blocks, threads, 0, st>>>(a); break;
     case VEGAS_F_GENZ_PRODUCT_PEAK: k_debug_rot<VEGAS_F_GENZ_PRODUCT_PEAK, T><<<blocks, threads, 0, st>>>(a); break;
+    case VEGAS_F_BW_POLY: k_debug_rot<VEGAS_F_BW_POLY, T><<<blocks, threads, 0, st>>>(a); break;
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();

@@ -103,7 +103,7 @@ def test_p3_iterate_on_oracle_grids_fp64(B, chains, cfg, path):
     g = _grid(B, w)
     if path == "generic":
         g.set_launch(0, 0, 2, 8)                     # pinning the copy counts pins the generic kernel
-    assert g.get_launch(w.integrand_id, 64)["path"] == ("generic" if path == "generic" or cfg == 5 else "rotated")
+    assert g.get_launch(w.integrand_id, 64)["path"] == ("generic" if path == "generic" else "rotated")
     for k in range(w.n_iter):
         g.set_edges(ch["edges_trace"][k])
         I, s, H, st = g.iterate(w.n_events, w.seed, k, w.integrand_id, 64, chunk_events=w.chunk_events)
@@ -330,12 +330,19 @@ def test_edge_shapes(B):
 
 
 def test_bw_poly_other_dimensions(B):
-    for dim in (2, 3, 9):
+    """Every shape of the last Philox block (1..4 dimensions) on the fast path (dim <= 8), and the generic
+    kernel beyond it (dim 9, 13): the per-lane coefficient registers must follow the lane's dimension."""
+    for dim in (2, 3, 4, 5, 6, 7, 8, 9, 13):
         p = W.bw_poly_params(dim, 77)
         edges = W.adapted_edges(dim, 40, seed=dim)
         g = B.VegasGrid(dim, 40)
         g.set_params(B.VEGAS_F_BW_POLY, p)
         g.set_edges(edges)
+        assert g.get_launch(B.VEGAS_F_BW_POLY, 64)["path"] == ("rotated" if dim <= 8 else "generic")
+        gw, gb, gx, gf = g.debug_sample(5, 4096, 3, 2, B.VEGAS_F_BW_POLY, 64)
+        ow, ob, ox, of = O.sample(edges, 3, 2, 5, 4096, O.BW_POLY, p)
+        assert np.array_equal(gb, ob)
+        np.testing.assert_allclose(gf, of, rtol=1e-12, atol=0)
         I, s, H, st = g.iterate(100_001, 3, 0, B.VEGAS_F_BW_POLY, 64)
         oI, oS, oH = O.iterate(edges, 100_001, 3, 0, O.BW_POLY, p)
         assert I == pytest.approx(oI, rel=RTOL64) and s == pytest.approx(oS, rel=RTOL64)

@@ -38,7 +38,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     def compile_unit(unit):
         name, src, defs = unit
         obj = os.path.join(OBJ_DIR, name + ".o")
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + defs + ["-c", os.path.join(CSRC, src), "-o", obj]
+        cmd = [nvcc] + NVCC_FLAGS + os.environ.get("VEGAS_NVCC_EXTRA", "").split() + (["-Xptxas", "-v"] if verbose else []) + defs + ["-c", os.path.join(CSRC, src), "-o", obj]
         subprocess.run(cmd, check=True)
         return obj
 

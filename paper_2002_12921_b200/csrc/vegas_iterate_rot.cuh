@@ -46,40 +46,73 @@ namespace vegas {
 template <int FID, typename T, int NBLK> struct RotCtx {
     template <class A> __device__ __forceinline__ void init(const A&, int /*dim*/, int /*gamma4*/, int /*gammaL*/) {}
 };
-template <int FID, typename T> struct IntegrandU;
+// independent accumulator chains per event: 4 for d <= 12; one for larger d, where the 128-register budget of the
+// 15-warp CTA is tight and the extra accumulators cost more than the shorter chains give (cfg3: 3.85e10 events/s
+// with 1 chain and Horner exp, 3.76e10 with 2 chains, 3.68e10 with 4 chains and Estrin; cfg4: 4.93e10 -> 5.24e10
+// and cfg2: 8.03e10 -> 8.10e10 with 4)
+__host__ __device__ constexpr int rot_chains(int dim) { return dim > 12 ? 1 : 4; }
+template <int NCH, typename T> __device__ __forceinline__ T chain_sum(const T (&s)[NCH]) {
+    if (NCH == 4) return (s[0] + s[NCH > 1 ? 1 : 0]) + (s[NCH > 2 ? 2 : 0] + s[NCH > 3 ? 3 : 0]);
+    if (NCH == 2) return s[0] + s[NCH > 1 ? 1 : 0];
+    return s[0];
+}
+template <int NCH, typename T> __device__ __forceinline__ T chain_prod(const T (&s)[NCH]) {
+    if (NCH == 4) return (s[0] * s[NCH > 1 ? 1 : 0]) * (s[NCH > 2 ? 2 : 0] * s[NCH > 3 ? 3 : 0]);
+    if (NCH == 2) return s[0] * s[NCH > 1 ? 1 : 0];
+    return s[0];
+}
+template <int FID, typename T, int NCH> struct IntegrandU;
 
-template <typename T> struct IntegrandU<VEGAS_F_CONST, T> {
+template <typename T, int NCH> struct IntegrandU<VEGAS_F_CONST, T, NCH> {
     template <class C> __device__ __forceinline__ void begin(const C&) {}
     template <class C> __device__ __forceinline__ void dim(T, int, int, const C&) {}
     __device__ __forceinline__ T finish(T) const { return (T)1; }
 };
-template <typename T> struct IntegrandU<VEGAS_F_GAUSS, T> {   // PAPER.md:65 Eq.(1); u = n_bins (x - 1/2)
-    T s;
-    template <class C> __device__ __forceinline__ void begin(const C&) { s = (T)0; }
-    template <class C> __device__ __forceinline__ void dim(T u, int, int, const C&) { s = t_fma(u, u, s); }
-    __device__ __forceinline__ T finish(T fin0) const { return t_exp_fast<T>(-s * fin0); }   // fin0 = 1/(n_bins a)^2
+// Every integrand keeps NCH partial accumulators, picked by the sub-step i (NCH independent chains instead of one
+// chain of d links: a dependent DFMA issues every ~14 clk on sm_100, r01_s7_ubench_pipes.md), combined in finish().
+template <typename T, int NCH> struct IntegrandU<VEGAS_F_GAUSS, T, NCH> {   // PAPER.md:65 Eq.(1); u = n_bins (x - 1/2)
+    T s[NCH];
+    template <class C> __device__ __forceinline__ void begin(const C&) {
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) s[c] = (T)0;
+    }
+    template <class C> __device__ __forceinline__ void dim(T u, int, int i, const C&) {
+        s[i & (NCH - 1)] = t_fma(u, u, s[i & (NCH - 1)]);
+    }
+    __device__ __forceinline__ T finish(T fin0) const {        // fin0 = 1/(n_bins a)^2
+        return ExpFast<T, (NCH > 1)>::f(-chain_sum<NCH, T>(s) * fin0);
+    }
 };
-template <typename T> struct IntegrandU<VEGAS_F_GENZ_PRODUCT_PEAK, T> {   // PAPER.md:74 Eq.(3); u = c_j (x - w_j)
-    T prod;
-    template <class C> __device__ __forceinline__ void begin(const C&) { prod = (T)1; }
-    template <class C> __device__ __forceinline__ void dim(T u, int, int, const C&) { prod *= t_fma(u, u, (T)1); }
-    __device__ __forceinline__ T finish(T) const { return (T)1 / prod; }
+template <typename T, int NCH> struct IntegrandU<VEGAS_F_GENZ_PRODUCT_PEAK, T, NCH> {   // PAPER.md:74 Eq.(3); u = c_j (x - w_j)
+    T prod[NCH];
+    template <class C> __device__ __forceinline__ void begin(const C&) {
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) prod[c] = (T)1;
+    }
+    template <class C> __device__ __forceinline__ void dim(T u, int, int i, const C&) {
+        prod[i & (NCH - 1)] *= t_fma(u, u, (T)1);
+    }
+    __device__ __forceinline__ T finish(T) const { return (T)1 / chain_prod<NCH, T>(prod); }
 };
 // BW_POLY (BASELINE.json:configs[4], readings R11, R12): u_0 = (s(x_0) - M^2)/(M Gamma), u_j = x_j for j >= 1;
 // f = [1/(1 + u_0^2)] * [sum_j a_j0 + sum_j u_j (a_j1 + u_j (a_j2 + u_j (a_j3 + u_j a_j4)))].
 // The lane that holds dimension 0 at sub-step i of block 0 runs the quartic with zero coefficients and keeps u.
 constexpr int kRotBwMaxDim = 8;    // 4 coefficient registers pairs per dimension per lane
-template <typename T> struct IntegrandU<VEGAS_F_BW_POLY, T> {
-    T poly, u0;
-    template <class C> __device__ __forceinline__ void begin(const C& c) { poly = c.poly0; u0 = (T)0; }
+template <typename T, int NCH> struct IntegrandU<VEGAS_F_BW_POLY, T, NCH> {
+    T poly[NCH], u0;
+    template <class C> __device__ __forceinline__ void begin(const C& c) {
+#pragma unroll
+        for (int k = 0; k < NCH; ++k) poly[k] = k ? (T)0 : c.poly0;
+        u0 = (T)0;
+    }
     template <class C> __device__ __forceinline__ void dim(T u, int blk, int i, const C& c) {
         T h = t_fma(c.a[blk][i][3], u, c.a[blk][i][2]);
         h = t_fma(h, u, c.a[blk][i][1]);
         h = t_fma(h, u, c.a[blk][i][0]);
-        poly = t_fma(h, u, poly);
+        poly[i & (NCH - 1)] = t_fma(h, u, poly[i & (NCH - 1)]);
         if (blk == 0 && c.is0[i]) u0 = u;
     }
-    __device__ __forceinline__ T finish(T) const { return poly / t_fma(u0, u0, (T)1); }
+    __device__ __forceinline__ T finish(T) const { return chain_sum<NCH, T>(poly) / t_fma(u0, u0, (T)1); }
 };
 
 // ---- table entry and u from the low product word ---------------------------------------------------
@@ -240,16 +273,19 @@ __device__ __forceinline__ void philox4x32_10_args(uint32_t c0, uint32_t c1, uin
 // table address of every (block, sub-step) in taddr (the histogram update derives its addresses from them).
 template <int FID, typename T, int DIM>
 __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, DIM>& L,
-                                            const RotCtx<FID, T, (DIM + 3) / 4>& ctx, unsigned long long ev, T fin0,
-                                            uint32_t (&taddr)[(DIM + 3) / 4][4]) {
+                                            const RotCtx<FID, T, (DIM + 3) / 4>& ctx, unsigned long long ev, bool live,
+                                            T fin0, uint32_t (&taddr)[(DIM + 3) / 4][4]) {
     using E = RotEntry<T>;
     using T2 = typename E::type;
     constexpr int NBLK = RotLane<T, DIM>::NBLK, R = RotLane<T, DIM>::R, GL = RotLane<T, DIM>::GL;
     const int nb = a.n_bins;
     const uint32_t e_lo = (uint32_t)ev, e_hi = (uint32_t)(ev >> 32);
-    IntegrandU<FID, T> f;
+    constexpr int NCH = rot_chains(DIM);
+    IntegrandU<FID, T, NCH> f;
     f.begin(ctx);
-    T jac = (T)a.jac_init;
+    T jac[NCH];                                          // partial Jacobian products (see IntegrandU)
+#pragma unroll
+    for (int c = 0; c < NCH; ++c) jac[c] = c ? (T)1 : (T)a.jac_init;
 #pragma unroll
     for (int blk = 0; blk < NBLK; ++blk) {
         const bool last = (blk == NBLK - 1);
@@ -293,12 +329,19 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
         for (int i = 0; i < NSUB; ++i) {
             const bool active = !(last && R == 3) || ((gamma ^ i) < 3);
             if (active) {
-                jac *= ent[i].y;
+                jac[i & (NCH - 1)] *= ent[i].y;
                 f.dim(E::u(ent[i], lo[i]), blk, i, ctx);
             }
         }
     }
-    return (double)(f.finish(fin0) * jac) * a.post_scale;
+    // events past the end of the launch's range get weight 0 (every built-in f is finite); the weight is ready
+    // before f, so only one multiply follows the integrand's tail
+    const T jall = chain_prod<NCH, T>(jac);
+    if (sizeof(T) == 8) {
+        const double wgt = live ? (double)jall * a.post_scale : 0.0;
+        return (double)f.finish(fin0) * wgt;
+    }
+    return (double)(f.finish(fin0) * jall) * (live ? a.post_scale : 0.0);      // C11: v formed in fp32, then widened
 }
 
 // S6 for one event, by the warp that holds its group's token: H[j][b_j] += v2 with plain loads and
@@ -406,8 +449,7 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     // it -- removed the barrier stalls but cost 30 register moves per iteration and measured 2 % slower.)
     for (unsigned long long it = 0; it < n_iter; ++it, q += nthr) {
         uint32_t taddr[NBLK][4];
-        double v = rot_event<FID, T, DIM>(a, L, ctx, a.first_event + q, fin0, taddr);
-        if (q >= a.count) v = 0.0;
+        const double v = rot_event<FID, T, DIM>(a, L, ctx, a.first_event + q, q < a.count, fin0, taddr);
         const double v2 = v * v;
         s1 += v;
         s2 += v2;

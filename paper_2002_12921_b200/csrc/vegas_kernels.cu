@@ -303,7 +303,7 @@ __global__ void k_debug_rot(const __grid_constant__ DebugArgs a) {
     const PhiloxKey ks = philox_key_schedule(a.key0, a.key1);
     RotCtx<FID, T, kRotBwMaxDim / 4> ctx;      // lane 0's view: gamma = 0, dimension j at (j >> 2, j & 3)
     ctx.init(a, dim, 0, 0);
-    IntegrandU<FID, T> f;
+    IntegrandU<FID, T, 1> f;
     f.begin(ctx);
     T jac = (T)a.jac_init;
     uint32_t w[4] = {0, 0, 0, 0};

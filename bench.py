@@ -48,6 +48,9 @@ def n_wide(w):
 
 
 WIDE_EXTRA_SLOTS = 2.4
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE K1 launch, from the `ncu --set full` captures summarised in
+# profiles/r01_s13_fast_path.md (bench.py never runs under a profiler): (workload, precision) -> bytes per launch
+NCU_TRAFFIC_BYTES = {("cfg3_gauss_d20", 64): 1.24e6, ("cfg3_gauss_d20", 32): 1.23e6, ("cfg4_genz_pp_d12", 64): 1.47e6}
 
 
 def n_fp(w, precision):
@@ -228,7 +231,6 @@ def main():
         step(k)
         k += 1
     # ---- timed region: K steps, device events per step (L2 flushed between steps, outside the brackets)
-    g.set_profiling(True)
     g.reset_counters()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     results = []
@@ -244,14 +246,29 @@ def main():
     barrier()
     t_wall = time.perf_counter() - t_wall
     ms = sum(a.elapsed_time(b) for a, b in ev)
-    k1_ms, k1_launches = g.kernel_time_ms()
     launches = g.launch_count()
-    g.set_profiling(False)
     if world > 1:
         t = torch.tensor([ms], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t.item())
     value = n_step * args.steps / (ms * 1e-3)
+
+    # ---- the dominant kernel alone: the same steps again with the library's per-launch CUDA events switched on
+    # (event pairs on the caller's stream around every K1 launch; kept out of the region `value` is taken from)
+    k1_steps = min(args.steps, 50)
+    g.set_profiling(True)
+    g.reset_counters()
+    evk = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(k1_steps)]
+    for i in range(k1_steps):
+        flush.zero_()
+        evk[i][0].record()
+        step(k)
+        evk[i][1].record()
+        k += 1
+    barrier()
+    k1_ms, k1_launches = g.kernel_time_ms()
+    k1_region_ms = sum(a.elapsed_time(b) for a, b in evk)
+    g.set_profiling(False)
 
     # ---- e2e: the same step through the C ABI with HOST buffers (edges in, I/sigma/hist/edges out)
     edges_host = g.get_edges()
@@ -302,8 +319,11 @@ def main():
                                 "why": "IMAD.WIDE.U32 holds the dispatch port 3.4 clk (profiles/r01_s7_ubench_pipes.md)"},
                     "fp_pipe_frac": k1_rate * nf / (SM_COUNT * (FP64_LANES if args.precision == 64 else ISSUE_LANES) * sm_max * 1e6),
                     "kernel_events_per_s": k1_rate, "kernel_ms_per_launch": k1_s * 1e3, "kernel_launches": int(k1_launches),
-                    "kernel_share_of_step": k1_ms / ms if world == 1 else None,
-                    "traffic": None}
+                    "kernel_share_of_step": k1_ms / k1_region_ms if world == 1 else None,
+                    "traffic": NCU_TRAFFIC_BYTES.get((w.name, args.precision)),
+                    "traffic_note": "DRAM bytes per K1 launch (ncu, profiles/r01_s13_fast_path.md); algorithmic global bytes "
+                                    "per launch = grid read + partial row read/write per CTA = %d" % (
+                                        shape["blocks"] * 8 * (w.dim * (w.n_bins + 1) + 2 * (4 + w.dim * w.n_bins)))}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64" if args.precision == 64 else "f32", "data": "synthetic",

@@ -159,23 +159,35 @@ k_iterate(const IterArgs a, const __grid_constant__ FParams<T> fp) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// K2: totals[i] = sum over CTAs, in CTA order, of partials[cta][i]  (i >= 4: histogram, plain fp64;
-// i < 4: the two double-double sums, merged by one thread).
+// K2: totals[i] = sum over CTAs, in CTA order, of partials[cta][i]  (i >= 4: histogram, plain fp64, one thread
+// each; i < 4: the two double-double sums, one warp each).
 // ---------------------------------------------------------------------------------------------
 __global__ void k_reduce(const double* __restrict__ partials, int n_parts, int n_tot, double* __restrict__ totals) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n_tot) return;
-    if (i >= 4) {
-        double h = 0.0;
-        for (int p = 0; p < n_parts; ++p) h += partials[(size_t)p * n_tot + i];
-        totals[i] = h;
-    } else if (i == 0 || i == 2) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < 64) {
+        // S1 (warp 0) and S2 (warp 1): lane l adds the partials of CTAs l, l+32, ... in that order, then a fixed
+        // shuffle tree -- the same association for every run of a given launch shape
+        const int i = 2 * (t >> 5), lane = t & 31;
         dd s{0.0, 0.0};
-        for (int p = 0; p < n_parts; ++p)
+        for (int p = lane; p < n_parts; p += 32)
             s = dd_add(s, dd{partials[(size_t)p * n_tot + i], partials[(size_t)p * n_tot + i + 1]});
-        totals[i] = s.hi;
-        totals[i + 1] = s.lo;
+        s = dd_warp_sum(s);
+        if (lane == 0) { totals[i] = s.hi; totals[i + 1] = s.lo; }
+        return;
     }
+    const int i = 4 + (t - 64);
+    if (i >= n_tot) return;
+    double h = 0.0;
+    int p = 0;
+    for (; p + 8 <= n_parts; p += 8) {           // 8 loads in flight; the additions stay in CTA order
+        double v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v[u] = partials[(size_t)(p + u) * n_tot + i];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) h += v[u];
+    }
+    for (; p < n_parts; ++p) h += partials[(size_t)p * n_tot + i];
+    totals[i] = h;
 }
 
 // S7 (C7): I = S1/n; Var = (S2/n - I^2)/(n-1); sigma = sqrt(max(Var, 0)).
@@ -397,7 +409,7 @@ size_t iterate_shared_bytes(int dim, int n_bins, int precision, int table_copies
 
 cudaError_t launch_reduce(const double* partials, int n_parts, int n_tot, double* totals, cudaStream_t st) {
     const int threads = 128;
-    k_reduce<<<(n_tot + threads - 1) / threads, threads, 0, st>>>(partials, n_parts, n_tot, totals);
+    k_reduce<<<(n_tot - 4 + 64 + threads - 1) / threads, threads, 0, st>>>(partials, n_parts, n_tot, totals);
     return cudaGetLastError();
 }
 

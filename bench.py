@@ -176,6 +176,8 @@ def main():
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32])
     ap.add_argument("--n-events", type=int, default=0, help="override events per step per GPU")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--user-integrand", action="store_true",
+                    help="run the workload's integrand as a run-time compiled user integrand (VEGAS_F_USER; gauss / genz only)")
     ap.add_argument("--launch", default="", help="blocks,threads,table_copies,hist_copies (0 = auto)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
@@ -214,12 +216,18 @@ def main():
     g.set_params(w.integrand_id, w.params)
     if args.launch:
         g.set_launch(*[int(v) for v in args.launch.split(",")])
-    shape = g.get_launch(w.integrand_id, args.precision)
+    fid = w.integrand_id
+    if args.user_integrand:
+        from paper_2002_12921_b200 import user_integrands as U
+        src = {W.GAUSS: U.GAUSS, W.GENZ_PRODUCT_PEAK: U.GENZ_PRODUCT_PEAK}[w.integrand_id]
+        g.set_user_integrand(src, w.params)
+        fid = B.VEGAS_F_USER
+    shape = g.get_launch(fid, args.precision)
     n_step = w.n_events * world                                   # weak scaling: n_events per GPU per step
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
 
     def step(k):
-        I, s, _, st = D.iterate_sharded(g, n_step, w.seed, k, w.integrand_id, args.precision, w.chunk_events,
+        I, s, _, st = D.iterate_sharded(g, n_step, w.seed, k, fid, args.precision, w.chunk_events,
                                         rank, world, want_hist=False)
         g.refine(w.alpha)
         return I, s
@@ -277,10 +285,10 @@ def main():
     for i in range(args.steps):
         g.set_edges(edges_host)
         if world > 1:
-            I, s, H, st = D.iterate_sharded(g, n_step, w.seed, k, w.integrand_id, args.precision, w.chunk_events,
+            I, s, H, st = D.iterate_sharded(g, n_step, w.seed, k, fid, args.precision, w.chunk_events,
                                             rank, world, want_hist=True)
         else:
-            I, s, H, st = g.iterate(n_step, w.seed, k, w.integrand_id, args.precision, w.chunk_events, want_hist=True)
+            I, s, H, st = g.iterate(n_step, w.seed, k, fid, args.precision, w.chunk_events, want_hist=True)
         g.refine(w.alpha, hist=H)
         edges_host = g.get_edges()
         k += 1
@@ -327,7 +335,7 @@ def main():
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64" if args.precision == 64 else "f32", "data": "synthetic",
-                "config": {"workload": w.name, "dim": w.dim, "n_bins": w.n_bins, "integrand": W.INTEGRAND_NAMES[w.integrand_id],
+                "config": {"workload": w.name, "dim": w.dim, "n_bins": w.n_bins, "integrand": W.INTEGRAND_NAMES[w.integrand_id] + (" (user source, NVRTC)" if args.user_integrand else ""),
                            "n_events_per_gpu_per_step": w.n_events, "chunk_events": w.chunk_events, "alpha": w.alpha,
                            "seed": w.seed, "launch": shape, "l2": "256 MiB memset between timed steps, outside the event brackets "
                            "(the path reads ~10 KB of global memory per launch)",

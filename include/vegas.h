@@ -71,6 +71,10 @@ extern "C" {
 #define VEGAS_F_GAUSS 1
 #define VEGAS_F_GENZ_PRODUCT_PEAK 2
 #define VEGAS_F_BW_POLY 3
+/*   VEGAS_F_USER               an integrand supplied as CUDA source and compiled at run time for this grid:
+ *                              see vegas_set_user_integrand() below; fp64 only, n_params <= VEGAS_USER_MAX_PARAMS */
+#define VEGAS_F_USER 4
+#define VEGAS_USER_MAX_PARAMS 64
 
 /* precision of the per-event arithmetic (reading C11): 64 = everything fp64; 32 = grid table, r, x,
  * J, f and v in fp32, v widened to fp64 before S1 += v, S2 += v^2, H += v^2.  Words, bins, the master
@@ -94,6 +98,29 @@ int vegas_destroy(vegas_grid* g);
  * to the kernels by value at every launch.  Required before iterating with that integrand id
  * (except VEGAS_F_CONST).  Parameters of several ids can be set; each id keeps its own array. */
 int vegas_set_params(vegas_grid* g, int integrand_id, const double* params_host, int n_params);
+
+/* User-supplied integrand (integrands "written in Fortran, C/C++ or even CUDA" are the paper's
+ * usability claim).  cuda_source (host, NUL-terminated) is CUDA C++ that defines
+ *
+ *     struct vegas_user_integrand {
+ *         __device__ void   begin(int dim, const double* p);          // start of an event
+ *         __device__ void   dim(int j, double x, const double* p);    // once per dimension j, x = x_j in (0,1);
+ *                                                                     // the ORDER of the calls is unspecified
+ *         __device__ double finish(const double* p);                  // f(x); must be finite on (0,1)^d
+ *     };
+ *
+ * (any members, helper functions and constants it needs; no #include of host headers; p points to the
+ * n_params doubles given here, read-only).  The library compiles it with NVRTC for sm_100a into the SAME fused
+ * iterate kernel the built-in integrands use (streaming form: x is consumed dimension by dimension, nothing per
+ * event is stored) for this grid's dim, and selects it with integrand_id = VEGAS_F_USER, precision VEGAS_FP64,
+ * in vegas_iterate / vegas_accumulate / vegas_integrate.  vegas_set_params(g, VEGAS_F_USER, ...) replaces the
+ * parameters without recompiling.  log (host, may be NULL) receives the NUL-terminated compiler log, truncated
+ * to log_bytes.  Needs libnvrtc.so.12 at run time (loaded on first use).
+ * Errors: VEGAS_EINVAL (NULL source, n_params out of range, compile error -> see log; dim * n_bins too large for
+ * the fused kernel's shared memory), VEGAS_ECUDA (NVRTC or the CUDA runtime unavailable / module load failed).
+ * vegas_debug_sample() does not take VEGAS_F_USER. */
+int vegas_set_user_integrand(vegas_grid* g, const char* cuda_source, const double* params_host, int n_params,
+                             char* log, size_t log_bytes);
 
 /* Inject / read the master grid: edges_host is [dim][n_bins+1] fp64, every row strictly increasing
  * with first element 0 and last element 1 (checked -> VEGAS_EINVAL).  Synchronous on `stream`. */

@@ -18,7 +18,7 @@ import numpy as np
 
 from .build import build as _build
 
-CONST, GAUSS, GENZ_PRODUCT_PEAK, BW_POLY = 0, 1, 2, 3
+CONST, GAUSS, GENZ_PRODUCT_PEAK, BW_POLY, GENZ_DISCONTINUOUS = 0, 1, 2, 3, 4
 OK, EINVAL, ENUMERIC = 0, -1, -3
 
 _lib = None

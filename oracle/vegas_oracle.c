@@ -42,7 +42,7 @@
 
 #define ORACLE_MAX_DIM 64
 
-enum { F_CONST = 0, F_GAUSS = 1, F_GENZ_PRODUCT_PEAK = 2, F_BW_POLY = 3 };
+enum { F_CONST = 0, F_GAUSS = 1, F_GENZ_PRODUCT_PEAK = 2, F_BW_POLY = 3, F_GENZ_DISCONTINUOUS = 4 };
 
 /* ---------------------------------------------------------------------------------------
  * C1  Philox4x32-10 (north_star: "counter-based Philox4x32-10 stream").
@@ -97,6 +97,8 @@ void oracle_split(uint32_t word, int n_bins, int32_t *bin, double *r)
  *   id 2  PAPER.md:74 Eq.(3), N = 1                  params = { c[0..d-1], w[0..d-1] }
  *   id 3  BASELINE.json:configs[4] (reading R11,R12) params = { M, Gamma, m_min, m_max,
  *                                                               a[i][k], i=1..d-1, k=0..4 }
+ *   id 4  PAPER.md:69 Eq.(2) AS PRINTED, N = 1 (reading R19): f = 0 if any x_j <= a_j, otherwise
+ *         exp(sum_j c_j x_j)                         params = { c[0..d-1], a[0..d-1] }
  *   id 0  f = 1 */
 int oracle_n_params(int integrand_id, int dim)
 {
@@ -105,6 +107,7 @@ int oracle_n_params(int integrand_id, int dim)
     case F_GAUSS: return 1;
     case F_GENZ_PRODUCT_PEAK: return 2 * dim;
     case F_BW_POLY: return 4 + 5 * (dim - 1);
+    case F_GENZ_DISCONTINUOUS: return 2 * dim;
     default: return -1;
     }
 }
@@ -150,6 +153,15 @@ double oracle_f(int integrand_id, int dim, const double *x, const double *params
             }
         }
         return bw * poly;
+    }
+    case F_GENZ_DISCONTINUOUS: {
+        const double *c = params, *a = params + dim;
+        double sum = 0.0;
+        for (int j = 0; j < dim; ++j) {
+            if (x[j] <= a[j]) return 0.0;
+            sum += c[j] * x[j];
+        }
+        return exp(sum);
     }
     default:
         return NAN;

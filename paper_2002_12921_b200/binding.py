@@ -16,7 +16,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libvegas_b200.so")
 
 VEGAS_OK, VEGAS_EINVAL, VEGAS_ECUDA, VEGAS_ENUMERIC = 0, -1, -2, -3
-VEGAS_F_CONST, VEGAS_F_GAUSS, VEGAS_F_GENZ_PRODUCT_PEAK, VEGAS_F_BW_POLY = 0, 1, 2, 3
+VEGAS_F_CONST, VEGAS_F_GAUSS, VEGAS_F_GENZ_PRODUCT_PEAK, VEGAS_F_BW_POLY, VEGAS_F_USER = 0, 1, 2, 3, 4
+VEGAS_USER_MAX_PARAMS = 64
 VEGAS_FP64, VEGAS_FP32 = 64, 32
 VEGAS_MAX_DIM, VEGAS_MAX_BINS, VEGAS_MAX_PARAMS = 32, 256, 160
 
@@ -36,6 +37,7 @@ SIGNATURES = {
     "vegas_create": (C.c_int, [C.c_int, C.c_int, _vp, C.c_size_t, C.POINTER(_vp)]),
     "vegas_destroy": (C.c_int, [_vp]),
     "vegas_set_params": (C.c_int, [_vp, C.c_int, _f64p, C.c_int]),
+    "vegas_set_user_integrand": (C.c_int, [_vp, C.c_char_p, _f64p, C.c_int, C.c_char_p, C.c_size_t]),
     "vegas_set_edges": (C.c_int, [_vp, _f64p, _vp]),
     "vegas_get_edges": (C.c_int, [_vp, _f64p, _vp]),
     "vegas_get_hist": (C.c_int, [_vp, _f64p, _vp]),
@@ -159,6 +161,19 @@ class VegasGrid:
     def set_params(self, integrand_id, params):
         p = np.ascontiguousarray(np.atleast_1d(np.asarray(params if params is not None else [], dtype=np.float64)))
         self._check(lib.vegas_set_params(self._h, integrand_id, _ptr(p) if p.size else None, p.size))
+
+    def set_user_integrand(self, cuda_source, params=None):
+        """Compile `cuda_source` (struct vegas_user_integrand, see include/vegas.h) into the fused kernel for this
+        grid; use integrand_id VEGAS_F_USER afterwards.  Returns the compiler log; raises VegasError (with the log
+        as detail) when the source does not compile."""
+        p = np.ascontiguousarray(np.atleast_1d(np.asarray(params if params is not None else [], dtype=np.float64)))
+        log = C.create_string_buffer(1 << 16)
+        rc = lib.vegas_set_user_integrand(self._h, cuda_source.encode(), _ptr(p) if p.size else None, p.size,
+                                          log, len(log))
+        text = log.value.decode(errors="replace")
+        if rc != VEGAS_OK:
+            raise VegasError(rc, text or lib.vegas_last_cuda_error(self._h).decode())
+        return text
 
     def set_edges(self, edges, stream=None):
         e = np.ascontiguousarray(edges, dtype=np.float64)

@@ -14,6 +14,7 @@
 #include "../../include/vegas.h"
 #include "vegas_kernels.h"
 #include "vegas_iterate_rot.cuh"
+#include "vegas_user.h"
 
 namespace {
 
@@ -69,9 +70,10 @@ struct vegas_grid {
     int* d_status = nullptr;
     double* d_hist_up = nullptr;
     double* d_partials = nullptr;
-    bool params_set[4] = {true, false, false, false};
-    double derived[4][VEGAS_MAX_PARAMS] = {};
-    double user[4][VEGAS_MAX_PARAMS] = {};       // the caller's arrays as given to vegas_set_params
+    bool params_set[5] = {true, false, false, false, false};
+    double derived[5][VEGAS_MAX_PARAMS] = {};
+    double user[5][VEGAS_MAX_PARAMS] = {};       // the caller's arrays as given to vegas_set_params
+    vegas::UserKernel ukernel;                   // VEGAS_F_USER: the run-time compiled fused kernel
     int cfg_blocks = 0, cfg_threads = 0, cfg_ct = 0, cfg_ch = 0;
     int active_blocks = 0;          // CTAs whose partial slots the current iteration uses
     bool profiling = false;
@@ -150,7 +152,8 @@ int ilog2(int v) {
 
 bool check_call(const vegas_grid* g, int fid, int precision) {
     if (!g) return false;
-    if (fid < 0 || fid > 3 || !g->params_set[fid]) return false;
+    if (fid < 0 || fid > VEGAS_F_USER || !g->params_set[fid]) return false;
+    if (fid == VEGAS_F_USER) return g->ukernel.kernel != nullptr && precision == VEGAS_FP64;
     if (expected_n_params(fid, g->dim) < 0) return false;
     return precision == VEGAS_FP64 || precision == VEGAS_FP32;
 }
@@ -166,6 +169,7 @@ double jac_scale_for(const vegas_grid* g, int precision) {
 // variables; it is taken unless the caller pinned the copy counts of the generic kernel with
 // vegas_set_launch (which is also how the tests keep the generic kernel covered).
 bool use_rot_path(const vegas_grid* g, int fid, int precision) {
+    if (fid == VEGAS_F_USER) return true;          // a user integrand exists only as a fast-path kernel
     if (g->cfg_ct > 0 || g->cfg_ch > 0) return false;
     const bool kind = fid == VEGAS_F_CONST || fid == VEGAS_F_GAUSS ||
                       (fid == VEGAS_F_GENZ_PRODUCT_PEAK && precision == VEGAS_FP64) ||
@@ -197,6 +201,11 @@ void rot_constants(const vegas_grid* g, int fid, int precision, double* shift, d
             ps *= c * nb;                                        // f J = prod(c_j nb) prod B_j / prod(1+u_j^2)
         }
         *post_scale = ps;
+    } else if (fid == VEGAS_F_USER) {
+        double ps = 1.0;                                         // u_j = x_j; J = prod nb Delta_j = nb^d prod B_j 2^32
+        for (int j = 0; j < dim; ++j) { scale[j] = 1.0; ps *= nb; }
+        *post_scale = ps;
+        for (int k = 0; k < vegas::kRotParams; ++k) fpar[k] = g->user[fid][k];
     } else if (fid == VEGAS_F_BW_POLY) {
         // u_0 = (s - M^2)/(M Gamma) with s = s_min + x_0 ds (C5): the Breit-Wigner is 1/(1 + u_0^2); u_j = x_j, j >= 1
         const double* d = g->derived[fid];                       // s_min, ds, M^2, M^2 Gamma^2, a[i][k]
@@ -260,7 +269,9 @@ RotShape rot_shape(const vegas_grid* g, int fid) {
     return s;
 }
 
-cudaError_t launch_rot(int fid, int precision, int dim, const vegas::RotArgs& a, const RotShape& s, cudaStream_t st) {
+cudaError_t launch_rot(vegas_grid* g, int fid, int precision, int dim, const vegas::RotArgs& a, const RotShape& s,
+                       cudaStream_t st) {
+    if (fid == VEGAS_F_USER) return vegas::user_launch(&g->ukernel, a, s.blocks, s.threads, s.shmem, st);
     if (precision == VEGAS_FP64) {
         switch (fid) {
         case VEGAS_F_CONST: return vegas::launch_iterate_rot<VEGAS_F_CONST, double>(dim, a, s.blocks, s.threads, s.shmem, st);
@@ -342,11 +353,21 @@ int vegas_create(int dim, int n_bins, void* dev_workspace, size_t bytes, vegas_g
 int vegas_destroy(vegas_grid* g) {
     if (!g) return VEGAS_EINVAL;
     for (cudaEvent_t ev : g->events) cudaEventDestroy(ev);
+    vegas::user_unload(&g->ukernel);
     delete g;
     return VEGAS_OK;
 }
 
 int vegas_set_params(vegas_grid* g, int fid, const double* p, int n_params) {
+    if (g && fid == VEGAS_F_USER) {
+        if (n_params < 0 || n_params > VEGAS_USER_MAX_PARAMS || (n_params > 0 && !p)) return VEGAS_EINVAL;
+        for (int i = 0; i < n_params; ++i)
+            if (!std::isfinite(p[i])) return VEGAS_EINVAL;
+        std::memset(g->user[fid], 0, sizeof(g->user[fid]));
+        for (int i = 0; i < n_params; ++i) g->user[fid][i] = p[i];
+        g->params_set[fid] = true;
+        return VEGAS_OK;
+    }
     if (!g || fid < 0 || fid > 3) return VEGAS_EINVAL;
     const int want = expected_n_params(fid, g->dim);
     if (want < 0 || n_params != want || want > VEGAS_MAX_PARAMS || (want > 0 && !p)) return VEGAS_EINVAL;
@@ -386,6 +407,25 @@ int vegas_set_params(vegas_grid* g, int fid, const double* p, int n_params) {
     }
     g->params_set[fid] = true;
     return VEGAS_OK;
+}
+
+int vegas_set_user_integrand(vegas_grid* g, const char* cuda_source, const double* params_host, int n_params,
+                             char* log, size_t log_bytes) {
+    if (log && log_bytes) log[0] = '\0';
+    if (!g || !cuda_source) return VEGAS_EINVAL;
+    if (vegas::rot_shared_bytes(g->dim, g->n_bins, 1) > g->smem_optin) return VEGAS_EINVAL;
+    const int rc_p = vegas_set_params(g, VEGAS_F_USER, params_host, n_params);
+    if (rc_p != VEGAS_OK) return rc_p;
+    CUDA_TRY(g, cudaSetDevice(g->device));
+    std::string clog, err;
+    const int rc = vegas::user_compile(cuda_source, g->dim, &clog, &g->ukernel, &err);
+    if (log && log_bytes) {
+        const std::string& msg = clog.empty() ? err : clog;
+        snprintf(log, log_bytes, "%s", msg.c_str());
+    }
+    if (rc == 0) return VEGAS_OK;
+    snprintf(g->cuda_err, sizeof(g->cuda_err), "%s", err.c_str());
+    return rc == -1 ? VEGAS_EINVAL : VEGAS_ECUDA;
 }
 
 int vegas_set_edges(vegas_grid* g, const double* edges_host, void* cuda_stream) {
@@ -499,7 +539,7 @@ int vegas_accumulate(vegas_grid* g, uint64_t first_event, uint64_t count, uint64
             CUDA_TRY(g, cudaEventRecord(e0, st));
         }
         if (rot)
-            CUDA_TRY(g, launch_rot(fid, precision, g->dim, ra, rs, st));
+            CUDA_TRY(g, launch_rot(g, fid, precision, g->dim, ra, rs, st));
         else
             CUDA_TRY(g, vegas::launch_iterate(fid, precision, a, g->derived[fid], s.blocks, s.threads, s.shmem, st));
         if (g->profiling) CUDA_TRY(g, cudaEventRecord(e1, st));
@@ -646,7 +686,7 @@ size_t vegas_debug_scratch_bytes(int dim, uint32_t count) {
 int vegas_debug_sample(vegas_grid* g, uint64_t first_event, uint32_t count, uint64_t seed, uint32_t iteration,
                        int fid, int precision, void* dev_scratch, void* cuda_stream, uint32_t* words,
                        int32_t* bins, double* x, double* fJ) {
-    if (!check_call(g, fid, precision) || !dev_scratch || count == 0) return VEGAS_EINVAL;
+    if (!check_call(g, fid, precision) || fid == VEGAS_F_USER || !dev_scratch || count == 0) return VEGAS_EINVAL;
     if (((uintptr_t)dev_scratch) % kAlign) return VEGAS_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     CUDA_TRY(g, cudaSetDevice(g->device));
@@ -700,7 +740,7 @@ int vegas_set_launch(vegas_grid* g, int blocks, int threads, int table_copies, i
 
 int vegas_get_launch(vegas_grid* g, int integrand_id, int precision, int* path, int* blocks, int* threads,
                      int* table_copies, int* hist_copies, size_t* shared_bytes) {
-    if (!g || (precision != VEGAS_FP64 && precision != VEGAS_FP32) || integrand_id < 0 || integrand_id > 3)
+    if (!g || (precision != VEGAS_FP64 && precision != VEGAS_FP32) || integrand_id < 0 || integrand_id > VEGAS_F_USER)
         return VEGAS_EINVAL;
     if (use_rot_path(g, integrand_id, precision)) {
         const RotShape r = rot_shape(g, integrand_id);

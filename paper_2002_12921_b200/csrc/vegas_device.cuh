@@ -2,10 +2,25 @@
 // hook (K4): Philox4x32-10, word split, grid map, the built-in integrands, compensated sums.
 // sm_100a only.  Readings C1..C11 are those of DESIGN.md; citations are PAPER.md lines.
 #pragma once
+#ifdef __CUDACC_RTC__
+// run-time compilation of a user integrand (vegas_user.cu): NVRTC has no host headers; the fixed-width types
+// and the few constants of include/vegas.h the device code uses are restated here
+typedef unsigned int uint32_t;
+typedef unsigned long long uint64_t;
+typedef unsigned long size_t;
+#define VEGAS_MAX_DIM 32
+#define VEGAS_MAX_PARAMS 160
+#define VEGAS_F_CONST 0
+#define VEGAS_F_GAUSS 1
+#define VEGAS_F_GENZ_PRODUCT_PEAK 2
+#define VEGAS_F_BW_POLY 3
+#define VEGAS_F_USER 4
+#else
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 #include "../../include/vegas.h"
+#endif
 
 namespace vegas {
 

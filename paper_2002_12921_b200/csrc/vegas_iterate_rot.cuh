@@ -35,7 +35,9 @@
 //     is no synchronisation at all.
 #pragma once
 #include "vegas_device.cuh"
+#ifndef __CUDACC_RTC__
 #include "vegas_kernels.h"
+#endif
 
 namespace vegas {
 
@@ -98,6 +100,7 @@ template <typename T, int NCH> struct IntegrandU<VEGAS_F_GENZ_PRODUCT_PEAK, T, N
 // f = [1/(1 + u_0^2)] * [sum_j a_j0 + sum_j u_j (a_j1 + u_j (a_j2 + u_j (a_j3 + u_j a_j4)))].
 // The lane that holds dimension 0 at sub-step i of block 0 runs the quartic with zero coefficients and keeps u.
 constexpr int kRotBwMaxDim = 8;    // 4 coefficient registers pairs per dimension per lane
+constexpr int kRotParams = 64;     // doubles of integrand parameters carried in the kernel arguments (VEGAS_USER_MAX_PARAMS)
 template <typename T, int NCH> struct IntegrandU<VEGAS_F_BW_POLY, T, NCH> {
     T poly[NCH], u0;
     template <class C> __device__ __forceinline__ void begin(const C& c) {
@@ -181,7 +184,7 @@ struct RotArgs {
     double jac_init;                // start value of the running Jacobian product (a power of two, see RotEntry)
     double fin0;                    // integrand finish constant
     double shift[VEGAS_MAX_DIM], scale[VEGAS_MAX_DIM];
-    double fpar[5 * kRotBwMaxDim];  // BW_POLY: a[j][k] at fpar[5 j + k], j = 1..dim-1 (row 0 unused)
+    double fpar[kRotParams];        // BW_POLY: a[j][k] at fpar[5 j + k], j = 1..dim-1 (row 0 unused); USER: the caller's array
 };
 
 template <typename T, int NBLK> struct RotCtx<VEGAS_F_BW_POLY, T, NBLK> {
@@ -206,9 +209,34 @@ template <typename T, int NBLK> struct RotCtx<VEGAS_F_BW_POLY, T, NBLK> {
     }
 };
 
+#ifdef VEGAS_USER_INTEGRAND
+// A user-supplied integrand compiled at run time (vegas_user.cu): the caller's
+// source defines `struct vegas_user_integrand` in streaming form (include/vegas.h: vegas_set_user_integrand);
+// it sees x_j itself (scale 1, shift 0) and the index j of the dimension this lane holds at (blk, i).
+template <typename T, int NBLK> struct RotCtx<VEGAS_F_USER, T, NBLK> {
+    const double* p;
+    int gamma4, gammaL, nblk, dim;
+    template <class A> __device__ __forceinline__ void init(const A& r, int d, int g4, int gL) {
+        p = r.fpar; gamma4 = g4; gammaL = gL; nblk = (d + 3) / 4; dim = d;
+    }
+};
+template <typename T, int NCH> struct IntegrandU<VEGAS_F_USER, T, NCH> {
+    vegas_user_integrand f;
+    const double* p;
+    template <class C> __device__ __forceinline__ void begin(const C& c) { p = c.p; f.begin(c.dim, p); }
+    template <class C> __device__ __forceinline__ void dim(T u, int blk, int i, const C& c) {
+        f.dim(4 * blk + ((blk == c.nblk - 1 ? c.gammaL : c.gamma4) ^ i), (double)u, p);
+    }
+    __device__ __forceinline__ T finish(T) { return (T)f.finish(p); }
+};
+#endif
+
 constexpr int kRotMaxThreads = 512;    // one CTA per SM: up to 16 warps, 128 registers per thread
 // BW_POLY keeps 4 coefficients per dimension per lane in registers: 12 warps, up to 168 registers
-__host__ __device__ constexpr int rot_max_threads(int fid) { return fid == VEGAS_F_BW_POLY ? 384 : kRotMaxThreads; }
+// (and so does a user integrand, whose register needs are unknown)
+__host__ __device__ constexpr int rot_max_threads(int fid) {
+    return (fid == VEGAS_F_BW_POLY || fid == VEGAS_F_USER) ? 384 : kRotMaxThreads;
+}
 constexpr int kRotDefaultWarps = 12;
 constexpr int kRotMaxRingWarps = 15;   // token barriers 1..15 (barrier 0 is __syncthreads)
 
@@ -493,6 +521,7 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     }
 }
 
+#ifndef __CUDACC_RTC__
 inline size_t rot_shared_bytes(int dim, int n_bins, int n_groups) {
     const size_t rows = (size_t)((dim + 3) / 4) * n_bins;
     return rows * (128 + 256 * (size_t)n_groups) + 2 * sizeof(dd) * (kRotMaxThreads / 32);
@@ -501,5 +530,6 @@ inline size_t rot_shared_bytes(int dim, int n_bins, int n_groups) {
 // one translation unit per (FID, T) instantiates DIM = 1..32 (vegas_rot_inst.cu)
 template <int FID, typename T>
 cudaError_t launch_iterate_rot(int dim, const RotArgs& a, int blocks, int threads, size_t shmem, cudaStream_t st);
+#endif
 
 }  // namespace vegas

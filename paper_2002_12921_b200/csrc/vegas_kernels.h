@@ -43,7 +43,7 @@ struct DebugArgs {
     // fast ("rotated") path only: the affine map and constants of vegas_iterate_rot.cuh
     double post_scale, fin0, jac_init;
     double shift[VEGAS_MAX_DIM], scale[VEGAS_MAX_DIM];
-    double fpar[40];                // RotArgs::fpar
+    double fpar[64];                // RotArgs::fpar (kRotParams)
 };
 
 size_t iterate_shared_bytes(int dim, int n_bins, int precision, int table_copies, int hist_copies);

@@ -24,9 +24,9 @@ from dataclasses import dataclass, field
 
 import numpy as np
 
-CONST, GAUSS, GENZ_PRODUCT_PEAK, BW_POLY = 0, 1, 2, 3
+CONST, GAUSS, GENZ_PRODUCT_PEAK, BW_POLY, GENZ_DISCONTINUOUS = 0, 1, 2, 3, 4
 INTEGRAND_NAMES = {CONST: "const", GAUSS: "gauss", GENZ_PRODUCT_PEAK: "genz_product_peak",
-                   BW_POLY: "bw_poly"}
+                   BW_POLY: "bw_poly", GENZ_DISCONTINUOUS: "genz_discontinuous"}
 
 _M0, _M1 = 0xD2511F53, 0xCD9E8D57
 _W0, _W1 = 0x9E3779B9, 0xBB67AE85
@@ -106,7 +106,19 @@ def closed_form(integrand_id: int, dim: int, params) -> float:
                                           - math.atan((s_min - M * M) / (M * G)))
         poly = sum(a[i, k] / (k + 1.0) for i in range(dim - 1) for k in range(5))
         return bw * poly
+    if integrand_id == GENZ_DISCONTINUOUS:        # PAPER.md:69 Eq.(2) as printed, N = 1: zero where any x_j <= a_j
+        c, a = p[:dim], p[dim:2 * dim]
+        val = 1.0
+        for cj, aj in zip(c, a):
+            val *= (math.exp(cj) - math.exp(cj * aj)) / cj
+        return val
     raise ValueError("unknown integrand id %r" % integrand_id)
+
+
+def genz_discontinuous_params(dim: int, seed: int) -> np.ndarray:
+    """c_j = 0.5 + u_j, a_j = 0.3 u_{dim+j} (C10 draws): the zero region removes 1 - prod(1 - a_j) of the volume."""
+    u = parameter_uniforms(seed, 2 * dim)
+    return np.concatenate([0.5 + u[:dim], 0.3 * u[dim:2 * dim]])
 
 
 def gauss_params(a: float = 0.1) -> np.ndarray:

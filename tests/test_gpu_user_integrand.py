@@ -1,0 +1,117 @@
+"""User-supplied integrands compiled at run time (vegas_set_user_integrand) against the
+CPU oracle: the same P3/P4/P5 protocol as the built-in integrands, fp64 tolerances of north_star."""
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import oracle as O
+from paper_2002_12921_b200 import user_integrands as U
+from paper_2002_12921_b200 import workloads as W
+
+THREADS = os.cpu_count() or 8
+RTOL64 = 1e-10
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
+    from paper_2002_12921_b200 import binding
+    return binding
+
+
+def _hist_ok(h_gpu, h_ref):
+    np.testing.assert_allclose(h_gpu, h_ref, rtol=RTOL64, atol=0)
+    assert np.all(h_gpu[h_ref == 0] == 0)
+
+
+CASES = [
+    # (user source, oracle id, dim, n_bins, params)
+    ("GAUSS", O.GAUSS, 4, 50, lambda d: W.gauss_params(0.1)),
+    ("GAUSS", O.GAUSS, 7, 33, lambda d: W.gauss_params(0.2)),                 # last Philox block with 3 dimensions
+    ("GENZ_PRODUCT_PEAK", O.GENZ_PRODUCT_PEAK, 12, 100, lambda d: W.genz_params(d, 4)),
+    ("GENZ_PRODUCT_PEAK", O.GENZ_PRODUCT_PEAK, 5, 20, lambda d: W.genz_params(d, 11)),   # last block with 1
+    ("GENZ_DISCONTINUOUS", O.GENZ_DISCONTINUOUS, 16, 50, lambda d: W.genz_discontinuous_params(d, 9)),
+    ("GENZ_DISCONTINUOUS", O.GENZ_DISCONTINUOUS, 2, 8, lambda d: W.genz_discontinuous_params(d, 2)),    # last block with 2
+]
+
+
+@pytest.mark.parametrize("name,oid,dim,nb,pf", CASES)
+def test_user_integrand_iterations_on_oracle_grids(B, name, oid, dim, nb, pf):
+    """P3/P4 teacher-forced: every iteration of an oracle chain is repeated on the oracle's grid."""
+    p = pf(dim)
+    n, seed, alpha = 300_007, 21, 1.5
+    ch = O.integrate(dim, nb, 3, n, seed, alpha, oid, p, threads=THREADS)
+    g = B.VegasGrid(dim, nb)
+    g.set_user_integrand(getattr(U, name), p)
+    assert g.get_launch(B.VEGAS_F_USER, 64)["path"] == "rotated"
+    for k in range(3):
+        g.set_edges(ch["edges_trace"][k])
+        I, s, H, st = g.iterate(n, seed, k, B.VEGAS_F_USER, 64, chunk_events=100_000 if k == 1 else 0)
+        assert st == 0
+        assert I == pytest.approx(ch["per_iter"][k, 0], rel=RTOL64)
+        assert s == pytest.approx(ch["per_iter"][k, 1], rel=RTOL64)
+        _hist_ok(H, ch["hist_trace"][k])
+        assert g.refine(alpha) == 0
+        nxt = ch["edges_trace"][k + 1] if k + 1 < 3 else ch["edges"]
+        np.testing.assert_allclose(g.get_edges(), nxt, rtol=0, atol=1e-10)
+    g.close()
+
+
+def test_user_integrand_equals_builtin_and_closed_form(B):
+    """The user-written Gaussian runs in the same fused kernel as the built-in one: same sample, same result to
+    rounding; a free-running vegas_integrate lands on the closed form (5 sigma rule, P7)."""
+    w = W.config(2).scaled(n_events=2_000_003, n_iter=6)
+    g = B.VegasGrid(w.dim, w.n_bins)
+    g.set_params(w.integrand_id, w.params)
+    g.set_user_integrand(U.GAUSS, w.params)
+    Ib, sb, Hb, _ = g.iterate(w.n_events, w.seed, 0, w.integrand_id, 64)
+    Iu, su, Hu, _ = g.iterate(w.n_events, w.seed, 0, B.VEGAS_F_USER, 64)
+    assert Iu == pytest.approx(Ib, rel=1e-12) and su == pytest.approx(sb, rel=1e-12)
+    np.testing.assert_allclose(Hu, Hb, rtol=1e-11)
+    r = g.integrate(w.n_iter, w.n_events, w.seed, w.alpha, B.VEGAS_F_USER, 64, n_skip=2)
+    assert abs(r["I"] - w.closed_form) < 5 * r["sigma"] and r["sigma"] < 1e-3
+    g.close()
+
+
+def test_user_integrand_parameters_and_errors(B):
+    p = W.genz_discontinuous_params(6, 3)
+    g = B.VegasGrid(6, 50)
+    # not compiled yet
+    with pytest.raises(B.VegasError):
+        g.iterate(1000, 1, 0, B.VEGAS_F_USER, 64)
+    # a source that does not compile: EINVAL with the compiler's message, and no kernel is installed
+    with pytest.raises(B.VegasError) as ei:
+        g.set_user_integrand(U.BROKEN, p)
+    assert ei.value.code == B.VEGAS_EINVAL and "undeclared_symbol" in str(ei.value)
+    with pytest.raises(B.VegasError):
+        g.iterate(1000, 1, 0, B.VEGAS_F_USER, 64)
+    with pytest.raises(B.VegasError):
+        g.set_user_integrand(U.GENZ_DISCONTINUOUS, np.zeros(B.VEGAS_USER_MAX_PARAMS + 1))
+    g.set_user_integrand(U.GENZ_DISCONTINUOUS, p)
+    with pytest.raises(B.VegasError):
+        g.iterate(1000, 1, 0, B.VEGAS_F_USER, 32)                 # fp64 only
+    with pytest.raises(B.VegasError):
+        g.debug_sample(0, 16, 1, 0, B.VEGAS_F_USER, 64)
+    edges = W.adapted_edges(6, 50, seed=6)
+    g.set_edges(edges)
+    I1, s1, H1, _ = g.iterate(100_003, 5, 0, B.VEGAS_F_USER, 64)
+    oI, oS, oH = O.iterate(edges, 100_003, 5, 0, O.GENZ_DISCONTINUOUS, p)
+    assert I1 == pytest.approx(oI, rel=RTOL64) and s1 == pytest.approx(oS, rel=RTOL64)
+    # new parameters without recompiling
+    p2 = W.genz_discontinuous_params(6, 4)
+    g.set_params(B.VEGAS_F_USER, p2)
+    I2, s2, H2, _ = g.iterate(100_003, 5, 0, B.VEGAS_F_USER, 64)
+    oI2, oS2, oH2 = O.iterate(edges, 100_003, 5, 0, O.GENZ_DISCONTINUOUS, p2)
+    assert I2 == pytest.approx(oI2, rel=RTOL64) and s2 == pytest.approx(oS2, rel=RTOL64)
+    _hist_ok(H2, oH2)
+    # replacing the integrand replaces the kernel
+    g.set_user_integrand(U.GENZ_PRODUCT_PEAK, W.genz_params(6, 8))
+    I3, _, _, _ = g.iterate(100_003, 5, 0, B.VEGAS_F_USER, 64)
+    oI3, _, _ = O.iterate(edges, 100_003, 5, 0, O.GENZ_PRODUCT_PEAK, W.genz_params(6, 8))
+    assert I3 == pytest.approx(oI3, rel=RTOL64)
+    g.close()

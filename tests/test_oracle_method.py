@@ -156,6 +156,27 @@ def test_c5_bw_poly_integral_matches_closed_form(probe):
     assert O.f(O.BW_POLY, [0.3, 1.0, 1.0], p) == pytest.approx(bw * p[4:].sum(), rel=1e-12)
 
 
+def test_c5_genz_discontinuous_as_printed_matches_closed_form():
+    """PAPER.md:69 Eq.(2) as printed (reading R19), N = 1: zero where ANY x_j <= a_j, exp(sum c_j x_j) elsewhere.
+    Pinned by quadrature with a break at the discontinuity, by point values on both sides of it, and by a chain."""
+    p = W.genz_discontinuous_params(2, 9)
+    c, a = p[:2], p[2:]
+    nodes = [_gl_nodes(np.array([0.0, a[j], 1.0]), 16) for j in range(2)]
+    got = _tensor_quadrature(O.GENZ_DISCONTINUOUS, p, nodes)
+    want = np.prod([(math.exp(cj) - math.exp(cj * aj)) / cj for cj, aj in zip(c, a)])
+    assert got == pytest.approx(want, rel=1e-12)
+    assert W.closed_form(W.GENZ_DISCONTINUOUS, 2, p) == pytest.approx(want, rel=1e-14)
+    # the zero region is x_j <= a_j (not >=), and one coordinate inside it is enough
+    assert O.f(O.GENZ_DISCONTINUOUS, [a[0] * 0.5, 0.9], p) == 0.0
+    assert O.f(O.GENZ_DISCONTINUOUS, [0.9, a[1]], p) == 0.0                       # boundary belongs to the zero side
+    assert O.f(O.GENZ_DISCONTINUOUS, [0.9, 0.8], p) == pytest.approx(math.exp(c[0] * 0.9 + c[1] * 0.8), rel=1e-15)
+    # the paper's 16-d case as a chain: within 5 sigma of the closed form once adapted
+    p16 = W.genz_discontinuous_params(16, 9)
+    r = O.integrate(16, 50, 6, 200_000, 9, 1.5, O.GENZ_DISCONTINUOUS, p16, n_skip=2, threads=8)
+    exact = W.closed_form(W.GENZ_DISCONTINUOUS, 16, p16)
+    assert abs(r["I"] - exact) < 5 * r["sigma"] and r["sigma"] / exact < 2e-2
+
+
 def test_c5_const():
     assert O.f(O.CONST, [0.1, 0.9], None) == 1.0
     assert O.n_params(O.GENZ_PRODUCT_PEAK, 12) == 24 and O.n_params(O.BW_POLY, 6) == 29

@@ -521,9 +521,17 @@ int vegas_accumulate(vegas_grid* g, uint64_t first_event, uint64_t count, uint64
         a.jac_scale = jac_scale_for(g, precision);
     }
     const uint64_t chunk = chunk_events ? chunk_events : count;
-    for (uint64_t done = 0; done < count; done += chunk) {
+    for (uint64_t done = 0, n_launch = 0; done < count; done += n_launch) {
+        n_launch = (count - done < chunk) ? count - done : chunk;
+        if (rot) {
+            // a fast-path launch never crosses a multiple of 2^32 in the global event index: the high counter word
+            // (C2) is then uniform over the launch and everything Philox derives from it alone is loop-invariant
+            const uint64_t to_boundary = 0x100000000ull - ((first_event + done) & 0xFFFFFFFFull);
+            if (n_launch > to_boundary) n_launch = to_boundary;
+            if (n_launch > 0xFFF00000ull) n_launch = 0xFFF00000ull;     // the kernel's 32-bit event offset (+ one padded pass)
+        }
         a.first_event = ra.first_event = first_event + done;
-        a.count = ra.count = (count - done < chunk) ? count - done : chunk;
+        a.count = ra.count = n_launch;
         cudaEvent_t e0 = nullptr, e1 = nullptr;
         if (g->profiling) {
             if (g->events_used + 2 > g->events.size()) {

@@ -301,13 +301,12 @@ __device__ __forceinline__ void philox4x32_10_args(uint32_t c0, uint32_t c1, uin
 // table address of every (block, sub-step) in taddr (the histogram update derives its addresses from them).
 template <int FID, typename T, int DIM>
 __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, DIM>& L,
-                                            const RotCtx<FID, T, (DIM + 3) / 4>& ctx, unsigned long long ev, bool live,
-                                            T fin0, uint32_t (&taddr)[(DIM + 3) / 4][4]) {
+                                            const RotCtx<FID, T, (DIM + 3) / 4>& ctx, uint32_t e_lo, uint32_t e_hi,
+                                            bool live, T fin0, uint32_t (&taddr)[(DIM + 3) / 4][4]) {
     using E = RotEntry<T>;
     using T2 = typename E::type;
     constexpr int NBLK = RotLane<T, DIM>::NBLK, R = RotLane<T, DIM>::R, GL = RotLane<T, DIM>::GL;
     const int nb = a.n_bins;
-    const uint32_t e_lo = (uint32_t)ev, e_hi = (uint32_t)(ev >> 32);
     constexpr int NCH = rot_chains(DIM);
     IntegrandU<FID, T, NCH> f;
     f.begin(ctx);
@@ -470,14 +469,19 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     double s1 = 0.0, s2 = 0.0;
     // every warp runs the same number of loop iterations (the ring hands the token on once per iteration);
     // events past the end of the range contribute v = 0
-    const unsigned long long nthr = (unsigned long long)gridDim.x * blockDim.x;
-    const unsigned long long n_iter = (a.count + nthr - 1) / nthr;
-    unsigned long long q = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    // The host never lets a launch cross a multiple of 2^32 in the global event index nor exceed 2^32 - 2^20
+    // events (vegas_accumulate), so the high counter word of C2 is uniform, the low one is first_lo + q without a
+    // carry, and q fits 32 bits even in the padded last pass.
+    const uint32_t nthr = gridDim.x * blockDim.x;
+    const uint32_t count = (uint32_t)a.count;
+    const uint32_t n_iter = (uint32_t)((a.count + nthr - 1) / nthr);
+    const uint32_t e_hi = (uint32_t)(a.first_event >> 32), first_lo = (uint32_t)a.first_event;
+    uint32_t q = blockIdx.x * blockDim.x + threadIdx.x;
     // (A software-pipelined variant -- histogram update of iteration it-1 after the per-event work of iteration
     // it -- removed the barrier stalls but cost 30 register moves per iteration and measured 2 % slower.)
-    for (unsigned long long it = 0; it < n_iter; ++it, q += nthr) {
+    for (uint32_t it = 0; it < n_iter; ++it, q += nthr) {
         uint32_t taddr[NBLK][4];
-        const double v = rot_event<FID, T, DIM>(a, L, ctx, a.first_event + q, q < a.count, fin0, taddr);
+        const double v = rot_event<FID, T, DIM>(a, L, ctx, first_lo + q, e_hi, q < count, fin0, taddr);
         const double v2 = v * v;
         s1 += v;
         s2 += v2;

@@ -275,6 +275,22 @@ def test_p6_event_range_sharding_matches_whole_iteration(B):
     oI, oS = O.estimate(S1, S2, n)
     assert I == pytest.approx(oI, rel=RTOL64) and s == pytest.approx(oS, rel=RTOL64)
     np.testing.assert_allclose(H, Ho.astype(np.float64), rtol=RTOL64)
+    # a range that CROSSES a multiple of 2^32: the fast path splits the launch there (its high counter word is
+    # uniform per launch), the generic kernel carries into the high word per event; with and without chunking
+    off = (2 << 32) - 77_777
+    n = 200_003
+    S1, S2, Ho = O.accumulate(edges, w.seed, 3, off, n, w.integrand_id, w.params)
+    oI, oS = O.estimate(S1, S2, n)
+    for pin_generic, chunk in ((False, 0), (False, 50_000), (True, 0)):
+        if pin_generic:
+            g.set_launch(0, 0, 2, 8)
+        assert g.get_launch(w.integrand_id, 64)["path"] == ("generic" if pin_generic else "rotated")
+        g.begin_iteration()
+        g.accumulate(off, n, w.seed, 3, w.integrand_id, 64, chunk_events=chunk)
+        g.reduce()
+        I, s, H, st = g.finalize(n)
+        assert I == pytest.approx(oI, rel=RTOL64) and s == pytest.approx(oS, rel=RTOL64)
+        np.testing.assert_allclose(H, Ho.astype(np.float64), rtol=RTOL64)
     g.close()
 
 

@@ -423,19 +423,26 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     unsigned char* hist = smem_rot + (size_t)rows * 128;       // NG x rows x 256 B
     dd* red = reinterpret_cast<dd*>(hist + (size_t)NG * rows * 256);
 
-    // ---- prologue: table from the master grid, zero histograms
-    for (int idx = threadIdx.x; idx < rows * (128 / ENTRY); idx += blockDim.x) {
-        const int row = idx / (128 / ENTRY), e = idx - row * (128 / ENTRY);   // entry e of the row
-        const int blk = row / nb, b = row - blk * nb;
-        const int G = (blk < NBLK - 1) ? 4 : GL;
-        const int slot = e / ((128 / ENTRY) / G);
-        const int j = 4 * blk + slot;
-        T2 ent = T2{};
-        if (j < DIM) {
-            const double* X = a.edges + (size_t)j * (nb + 1);
-            ent = E::make(X[b], X[b + 1], a.shift[j], a.scale[j]);
+    // ---- prologue: the master grid is staged in shared memory with one coalesced pass (in the histogram region,
+    // zeroed afterwards), the table is built from the staged copy, the histograms are zeroed
+    {
+        double* stage_e = reinterpret_cast<double*>(hist);         // DIM (nb+1) doubles <= one histogram copy
+        for (int idx = threadIdx.x; idx < DIM * (nb + 1); idx += blockDim.x) stage_e[idx] = a.edges[idx];
+        __syncthreads();
+        for (int idx = threadIdx.x; idx < rows * (128 / ENTRY); idx += blockDim.x) {
+            const int row = idx / (128 / ENTRY), e = idx - row * (128 / ENTRY);   // entry e of the row
+            const int blk = row / nb, b = row - blk * nb;
+            const int G = (blk < NBLK - 1) ? 4 : GL;
+            const int slot = e / ((128 / ENTRY) / G);
+            const int j = 4 * blk + slot;
+            T2 ent = T2{};
+            if (j < DIM) {
+                const double* X = stage_e + j * (nb + 1);
+                ent = E::make(X[b], X[b + 1], a.shift[j], a.scale[j]);
+            }
+            reinterpret_cast<T2*>(table)[idx] = ent;
         }
-        reinterpret_cast<T2*>(table)[idx] = ent;
+        __syncthreads();
     }
     for (int idx = threadIdx.x; idx < NG * rows * 32; idx += blockDim.x) reinterpret_cast<double*>(hist)[idx] = 0.0;
     __syncthreads();
@@ -492,12 +499,28 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     if (S > 1 && pos == 0 && n_iter > 0) token_wait(my_token);   // absorbs the ring's last hand-off
 
     // ---- S5: warp shuffle -> CTA -> this CTA's partial (accumulated over the launches of an iteration)
-    dd t1 = dd_warp_sum(dd{s1, 0.0});
-    dd t2 = dd_warp_sum(dd{s2, 0.0});
+    // (the 32 per-thread sums of a warp are added by a plain fp64 shuffle tree, like the per-thread sums
+    // themselves; warps, launches and CTAs -- where thousands of terms meet -- are added in double-double)
+#pragma unroll
+    for (int m = 16; m > 0; m >>= 1) {
+        s1 += __shfl_xor_sync(0xffffffffu, s1, m);
+        s2 += __shfl_xor_sync(0xffffffffu, s2, m);
+    }
+    dd t1{s1, 0.0}, t2{s2, 0.0};
     const int nwarps = (blockDim.x + 31) >> 5;
     if (lane == 0) { red[2 * warp] = t1; red[2 * warp + 1] = t2; }
-    __syncthreads();
     double* part = a.partials + (size_t)blockIdx.x * (4 + DIM * nb);
+    // this thread's words of the CTA's partial row: loaded now, used after the merge (hides the global latency)
+    // (the first 4 words per thread; a shape with more than 4 blockDim.x bins reads the rest in the last pass)
+    double own[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int idx = threadIdx.x + k * blockDim.x;
+        own[k] = (idx < DIM * nb) ? part[4 + idx] : 0.0;
+    }
+    __syncthreads();
+    // warp 0 adds the warps' sums (latency-bound double-double chains) while the other warps merge the histograms
+    // (shared-memory-bandwidth-bound); with a single warp it does both
     if (warp == 0) {
         t1 = (lane < nwarps) ? red[2 * lane] : dd{0.0, 0.0};
         t2 = (lane < nwarps) ? red[2 * lane + 1] : dd{0.0, 0.0};
@@ -509,20 +532,52 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
             part[0] = t1.hi; part[1] = t1.lo; part[2] = t2.hi; part[3] = t2.lo;
         }
     }
-    // ---- S6: merge the copies of every (dimension, bin) in fixed order, one pass per CTA
-    for (int idx = threadIdx.x; idx < DIM * nb; idx += blockDim.x) {
-        const int j = idx / nb, b = idx - j * nb;
-        const int blk = j >> 2, slot = j & 3;
-        const int G = (blk < NBLK - 1) ? 4 : GL;
-        const int per = 16 / G;                                   // copies per half-warp row half
-        double h = 0.0;
+    const int mwarps = nwarps > 1 ? nwarps - 1 : 1, mwarp = nwarps > 1 ? warp - 1 : 0;   // merging warps, my rank
+    // ---- S6: merge the copies of every (dimension, bin) in fixed order, one pass per CTA.  One warp per
+    // histogram row, lane l reads word l of the row (conflict-free; a thread-per-bin loop here put all lanes of
+    // a warp on one bank), sums it over the copies, and the words of one dimension slot -- lanes that differ in
+    // the half-warp bit and the copy bits -- are added by a fixed xor-shuffle tree.  The row sums are staged in
+    // the table's shared memory (dead after the event loop; the barrier above orders it), then added to this
+    // CTA's partial row in one coalesced pass.
+    double* stage = reinterpret_cast<double*>(table);
+    constexpr int LGPL = (GL == 4) ? 2 : (GL == 2) ? 3 : 4;           // log2(copies per slot per half-warp), last block
+    const double* hw = reinterpret_cast<const double*>(hist) + lane;
+    for (int row0 = mwarp; row0 < rows && mwarp >= 0; row0 += 4 * mwarps) {   // 4 rows in flight per warp
+        double h[4] = {0.0, 0.0, 0.0, 0.0};
         for (int g = 0; g < NG; ++g) {
-            const double* row = reinterpret_cast<const double*>(hist + ((size_t)g * rows + (size_t)(blk * nb + b)) * 256);
-            for (int half = 0; half < 2; ++half)
-                for (int c = 0; c < per; ++c) h += row[half * 16 + slot * per + c];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int row = row0 + u * mwarps;
+                if (row < rows) h[u] += hw[((size_t)g * rows + (size_t)row) * 32];
+            }
         }
-        part[4 + idx] += h;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            h[u] += __shfl_xor_sync(0xffffffffu, h[u], 16);
+            h[u] += __shfl_xor_sync(0xffffffffu, h[u], 1);
+            h[u] += __shfl_xor_sync(0xffffffffu, h[u], 2);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int row = row0 + u * mwarps;
+            if (row >= rows) continue;                                // warp-uniform
+            const bool last = row >= (NBLK - 1) * nb;
+            const int lgp = last ? LGPL : 2;
+            if (lgp >= 3) h[u] += __shfl_xor_sync(0xffffffffu, h[u], 4);
+            if (lgp >= 4) h[u] += __shfl_xor_sync(0xffffffffu, h[u], 8);
+            const int blk = last ? NBLK - 1 : row / nb, b = row - blk * nb;
+            const int slot = (lane & 15) >> lgp, c = lane & ((1 << lgp) - 1);
+            const int j = 4 * blk + slot;
+            if (lane < 16 && c == 0 && j < DIM) stage[j * nb + b] = h[u];
+        }
     }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int idx = threadIdx.x + k * blockDim.x;
+        if (idx < DIM * nb) part[4 + idx] = own[k] + stage[idx];
+    }
+    for (int idx = threadIdx.x + 4 * blockDim.x; idx < DIM * nb; idx += blockDim.x) part[4 + idx] += stage[idx];
 }
 
 #ifndef __CUDACC_RTC__

@@ -49,8 +49,9 @@ def n_wide(w):
 
 WIDE_EXTRA_SLOTS = 2.4
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE K1 launch, from the `ncu --set full` captures summarised in
-# profiles/r01_s13_fast_path.md (bench.py never runs under a profiler): (workload, precision) -> bytes per launch
-NCU_TRAFFIC_BYTES = {("cfg3_gauss_d20", 64): 1.24e6, ("cfg3_gauss_d20", 32): 1.23e6, ("cfg4_genz_pp_d12", 64): 1.47e6}
+# profiles/r01_s14_final.md (bench.py never runs under a profiler): (workload, precision) -> bytes per launch
+NCU_TRAFFIC_BYTES = {("cfg3_gauss_d20", 64): 1.24e6, ("cfg3_gauss_d20", 32): 1.24e6, ("cfg4_genz_pp_d12", 64): 1.48e6,
+                     ("cfg5_bw_poly_d6", 64): 0.40e6}
 
 
 def n_fp(w, precision):
@@ -329,7 +330,7 @@ def main():
                     "kernel_events_per_s": k1_rate, "kernel_ms_per_launch": k1_s * 1e3, "kernel_launches": int(k1_launches),
                     "kernel_share_of_step": k1_ms / k1_region_ms if world == 1 else None,
                     "traffic": NCU_TRAFFIC_BYTES.get((w.name, args.precision)),
-                    "traffic_note": "DRAM bytes per K1 launch (ncu, profiles/r01_s13_fast_path.md); algorithmic global bytes "
+                    "traffic_note": "DRAM bytes per K1 launch (ncu, profiles/r01_s14_final.md); algorithmic global bytes "
                                     "per launch = grid read + partial row read/write per CTA = %d" % (
                                         shape["blocks"] * 8 * (w.dim * (w.n_bins + 1) + 2 * (4 + w.dim * w.n_bins)))}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

@@ -294,6 +294,21 @@ def test_p6_event_range_sharding_matches_whole_iteration(B):
     g.close()
 
 
+def test_plain_mc_mode_is_alpha_zero(B):
+    """The paper's "Plain MC" column = the same iteration with the refinement switched off:
+    alpha = 0 leaves the grid where it is (C8 fixed point), so every iteration samples the uniform grid."""
+    w = W.config(1)
+    g = _grid(B, w)
+    r = g.integrate(4, w.n_events, w.seed, 0.0, w.integrand_id, 64)
+    o = O.integrate(w.dim, w.n_bins, 4, w.n_events, w.seed, 0.0, w.integrand_id, w.params, threads=THREADS)
+    np.testing.assert_allclose(g.get_edges(), O.uniform_edges(w.dim, w.n_bins), rtol=0, atol=1e-15)
+    np.testing.assert_allclose(r["per_iter"], o["per_iter"], rtol=RTOL64)
+    assert r["I"] == pytest.approx(o["I"], rel=RTOL64) and r["sigma"] == pytest.approx(o["sigma"], rel=RTOL64)
+    # without adaptation the error stays at its first-iteration size (the adaptive chain shrinks it ~30x, cfg1)
+    assert r["per_iter"][3, 1] > 0.5 * r["per_iter"][0, 1]
+    g.close()
+
+
 # ------------------------------------------------------------------ P7: 5 sigma, control, fixed point
 def test_p7_constant_control_and_fixed_point(B):
     w = W.control_const(n_events=10_000_000)

@@ -171,9 +171,9 @@ double jac_scale_for(const vegas_grid* g, int precision) {
 bool use_rot_path(const vegas_grid* g, int fid, int precision) {
     if (fid == VEGAS_F_USER) return true;          // a user integrand exists only as a fast-path kernel
     if (g->cfg_ct > 0 || g->cfg_ch > 0) return false;
-    const bool kind = fid == VEGAS_F_CONST || fid == VEGAS_F_GAUSS ||
-                      (fid == VEGAS_F_GENZ_PRODUCT_PEAK && precision == VEGAS_FP64) ||
-                      (fid == VEGAS_F_BW_POLY && precision == VEGAS_FP64 && g->dim <= vegas::kRotBwMaxDim);
+    (void)precision;
+    const bool kind = fid == VEGAS_F_CONST || fid == VEGAS_F_GAUSS || fid == VEGAS_F_GENZ_PRODUCT_PEAK ||
+                      (fid == VEGAS_F_BW_POLY && g->dim <= vegas::kRotBwMaxDim);
     if (!kind) return false;
     if (g->cfg_threads > vegas::rot_max_threads(fid)) return false;
     return vegas::rot_shared_bytes(g->dim, g->n_bins, 1) <= g->smem_optin;
@@ -285,6 +285,10 @@ cudaError_t launch_rot(vegas_grid* g, int fid, int precision, int dim, const veg
         switch (fid) {
         case VEGAS_F_CONST: return vegas::launch_iterate_rot<VEGAS_F_CONST, float>(dim, a, s.blocks, s.threads, s.shmem, st);
         case VEGAS_F_GAUSS: return vegas::launch_iterate_rot<VEGAS_F_GAUSS, float>(dim, a, s.blocks, s.threads, s.shmem, st);
+        case VEGAS_F_GENZ_PRODUCT_PEAK:
+            return vegas::launch_iterate_rot<VEGAS_F_GENZ_PRODUCT_PEAK, float>(dim, a, s.blocks, s.threads, s.shmem, st);
+        case VEGAS_F_BW_POLY:
+            return vegas::launch_iterate_rot<VEGAS_F_BW_POLY, float>(dim, a, s.blocks, s.threads, s.shmem, st);
         }
     }
     return cudaErrorInvalidValue;

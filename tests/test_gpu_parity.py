@@ -122,6 +122,7 @@ def test_p3_iterate_on_oracle_grids_fp32(B, chains, cfg, path):
     g = _grid(B, w)
     if path == "generic":
         g.set_launch(0, 0, 4, 8)
+    assert g.get_launch(w.integrand_id, 32)["path"] == ("generic" if path == "generic" else "rotated")
     for k in range(w.n_iter):
         g.set_edges(ch["edges_trace"][k])
         I, s, H, st = g.iterate(w.n_events, w.seed, k, w.integrand_id, 32, chunk_events=w.chunk_events)

@@ -228,6 +228,11 @@ def main():
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
 
     def step(k):
+        if world == 1:
+            # one iteration + refinement enqueued back to back, one synchronisation (vegas_integrate_from, n_iter = 1)
+            r = g.integrate(1, n_step, w.seed, w.alpha, fid, args.precision, chunk_events=w.chunk_events,
+                            first_iteration=k)
+            return r["I"], r["sigma"]
         I, s, _, st = D.iterate_sharded(g, n_step, w.seed, k, fid, args.precision, w.chunk_events,
                                         rank, world, want_hist=False)
         g.refine(w.alpha)

@@ -176,6 +176,15 @@ int vegas_integrate(vegas_grid* g, int n_iter, int n_skip, uint64_t n_events, ui
                     uint64_t seed, double alpha, int integrand_id, int precision, void* cuda_stream,
                     double* I, double* sigma, double* chi2_dof, double* per_iter_host);
 
+/* The same, continuing a run: the n_iter iterations carry the indices first_iteration .. first_iteration+n_iter-1
+ * in the RNG counter (C2) and start from the grid as it stands.  With the grid (vegas_get_edges / vegas_set_edges),
+ * the seed and the next iteration index saved, a run is resumed bit for bit: the RNG is counter-based, nothing else
+ * is state.  n_skip counts from first_iteration.  vegas_integrate(...) = vegas_integrate_from(g, 0, ...).
+ * Additional error: VEGAS_EINVAL if first_iteration + n_iter exceeds 0xFFFFFFFF (reserved, reading C10). */
+int vegas_integrate_from(vegas_grid* g, uint32_t first_iteration, int n_iter, int n_skip, uint64_t n_events,
+                         uint64_t chunk_events, uint64_t seed, double alpha, int integrand_id, int precision,
+                         void* cuda_stream, double* I, double* sigma, double* chi2_dof, double* per_iter_host);
+
 /* Step S9 alone on host arrays (no device work). */
 int vegas_combine(int n_iter, int n_skip, const double* I_k, const double* sigma_k, double* I,
                   double* sigma, double* chi2_dof);

@@ -51,6 +51,8 @@ SIGNATURES = {
     "vegas_refine": (C.c_int, [_vp, _f64p, C.c_double, _vp]),
     "vegas_integrate": (C.c_int, [_vp, C.c_int, C.c_int, _u64, _u64, _u64, C.c_double, C.c_int, C.c_int, _vp,
                                   _f64p, _f64p, _f64p, _f64p]),
+    "vegas_integrate_from": (C.c_int, [_vp, C.c_uint32, C.c_int, C.c_int, _u64, _u64, _u64, C.c_double, C.c_int, C.c_int,
+                                       _vp, _f64p, _f64p, _f64p, _f64p]),
     "vegas_combine": (C.c_int, [C.c_int, C.c_int, _f64p, _f64p, _f64p, _f64p, _f64p]),
     "vegas_debug_scratch_bytes": (C.c_size_t, [C.c_int, C.c_uint32]),
     "vegas_debug_sample": (C.c_int, [_vp, _u64, C.c_uint32, _u64, C.c_uint32, C.c_int, C.c_int, _vp, _vp,
@@ -235,13 +237,13 @@ class VegasGrid:
         return self._check(lib.vegas_refine(self._h, _ptr(h), float(alpha), _stream(stream)), allow_numeric=True)
 
     def integrate(self, n_iter, n_events, seed, alpha, integrand_id, precision=VEGAS_FP64, n_skip=0,
-                  chunk_events=0, stream=None):
-        """-> dict(I, sigma, chi2_dof, per_iter [n_iter,2], status)"""
+                  chunk_events=0, stream=None, first_iteration=0):
+        """-> dict(I, sigma, chi2_dof, per_iter [n_iter,2], status); first_iteration > 0 continues a run"""
         I, s, c = C.c_double(), C.c_double(), C.c_double()
         per = np.zeros((max(int(n_iter), 1), 2))
-        rc = lib.vegas_integrate(self._h, int(n_iter), int(n_skip), int(n_events), int(chunk_events), int(seed),
-                                 float(alpha), integrand_id, precision, _stream(stream), C.byref(I), C.byref(s),
-                                 C.byref(c), _ptr(per))
+        rc = lib.vegas_integrate_from(self._h, int(first_iteration), int(n_iter), int(n_skip), int(n_events),
+                                      int(chunk_events), int(seed), float(alpha), integrand_id, precision,
+                                      _stream(stream), C.byref(I), C.byref(s), C.byref(c), _ptr(per))
         self._check(rc, allow_numeric=True)
         return dict(I=I.value, sigma=s.value, chi2_dof=c.value, per_iter=per, status=rc)
 

@@ -651,7 +651,15 @@ int vegas_combine(int n_iter, int n_skip, const double* I_k, const double* sigma
 int vegas_integrate(vegas_grid* g, int n_iter, int n_skip, uint64_t n_events, uint64_t chunk_events, uint64_t seed,
                     double alpha, int fid, int precision, void* cuda_stream, double* I, double* sigma,
                     double* chi2_dof, double* per_iter_host) {
+    return vegas_integrate_from(g, 0, n_iter, n_skip, n_events, chunk_events, seed, alpha, fid, precision, cuda_stream,
+                                I, sigma, chi2_dof, per_iter_host);
+}
+
+int vegas_integrate_from(vegas_grid* g, uint32_t first_iteration, int n_iter, int n_skip, uint64_t n_events,
+                         uint64_t chunk_events, uint64_t seed, double alpha, int fid, int precision, void* cuda_stream,
+                         double* I, double* sigma, double* chi2_dof, double* per_iter_host) {
     if (!check_call(g, fid, precision) || n_events < 2) return VEGAS_EINVAL;
+    if ((uint64_t)first_iteration + (uint64_t)(n_iter > 0 ? n_iter : 0) > 0xFFFFFFFFull) return VEGAS_EINVAL;   // C2: 0xFFFFFFFF is reserved
     if (n_iter < 1 || n_iter > kMaxIter || n_skip < 0 || n_skip >= n_iter || !I || !sigma || !chi2_dof)
         return VEGAS_EINVAL;
     if (alpha != alpha || std::isinf(alpha)) return VEGAS_EINVAL;
@@ -661,7 +669,8 @@ int vegas_integrate(vegas_grid* g, int n_iter, int n_skip, uint64_t n_events, ui
     for (int k = 0; k < n_iter; ++k) {
         int rc = vegas_begin_iteration(g, cuda_stream);
         if (rc) return rc;
-        rc = vegas_accumulate(g, 0, n_events, chunk_events, seed, (uint32_t)k, fid, precision, cuda_stream);
+        rc = vegas_accumulate(g, 0, n_events, chunk_events, seed, first_iteration + (uint32_t)k, fid, precision,
+                              cuda_stream);
         if (rc) return rc;
         rc = vegas_reduce(g, cuda_stream);
         if (rc) return rc;

@@ -159,12 +159,13 @@ k_iterate(const IterArgs a, const __grid_constant__ FParams<T> fp) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// K2: totals[i] = sum over CTAs, in CTA order, of partials[cta][i]  (i >= 4: histogram, plain fp64, one thread
-// each; i < 4: the two double-double sums, one warp each).
+// K2: totals[i] = sum over CTAs of partials[cta][i] in a fixed association (i >= 4: histogram, plain fp64, 8 strided
+// slices of the CTAs then the slices in order; i < 4: the two double-double sums, one warp each).
 // ---------------------------------------------------------------------------------------------
 __global__ void k_reduce(const double* __restrict__ partials, int n_parts, int n_tot, double* __restrict__ totals) {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t < 64) {
+    if (blockIdx.x == 0) {
+        if (t >= 64) return;
         // S1 (warp 0) and S2 (warp 1): lane l adds the partials of CTAs l, l+32, ... in that order, then a fixed
         // shuffle tree -- the same association for every run of a given launch shape
         const int i = 2 * (t >> 5), lane = t & 31;
@@ -175,19 +176,29 @@ __global__ void k_reduce(const double* __restrict__ partials, int n_parts, int n
         if (lane == 0) { totals[i] = s.hi; totals[i + 1] = s.lo; }
         return;
     }
-    const int i = 4 + (t - 64);
-    if (i >= n_tot) return;
+    // histogram totals: block b > 0 owns 32 consecutive totals; its 8 warps each add every 8th CTA's partial
+    // (4 loads in flight), and warp 0 adds the 8 slice sums in slice order -- a fixed association
+    __shared__ double slice[8][32];
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int i = 4 + ((int)blockIdx.x - 1) * 32 + lane;
     double h = 0.0;
-    int p = 0;
-    for (; p + 8 <= n_parts; p += 8) {           // 8 loads in flight; the additions stay in CTA order
-        double v[8];
-#pragma unroll
-        for (int u = 0; u < 8; ++u) v[u] = partials[(size_t)(p + u) * n_tot + i];
-#pragma unroll
-        for (int u = 0; u < 8; ++u) h += v[u];
+    if (i < n_tot) {
+        int p = w;
+        for (; p + 24 < n_parts; p += 32) {
+            const double v0 = partials[(size_t)p * n_tot + i], v1 = partials[(size_t)(p + 8) * n_tot + i];
+            const double v2 = partials[(size_t)(p + 16) * n_tot + i], v3 = partials[(size_t)(p + 24) * n_tot + i];
+            h += v0; h += v1; h += v2; h += v3;
+        }
+        for (; p < n_parts; p += 8) h += partials[(size_t)p * n_tot + i];
     }
-    for (; p < n_parts; ++p) h += partials[(size_t)p * n_tot + i];
-    totals[i] = h;
+    slice[w][lane] = h;
+    __syncthreads();
+    if (w == 0 && i < n_tot) {
+        double t = slice[0][lane];
+#pragma unroll
+        for (int k = 1; k < 8; ++k) t += slice[k][lane];
+        totals[i] = t;
+    }
 }
 
 // S7 (C7): I = S1/n; Var = (S2/n - I^2)/(n-1); sigma = sqrt(max(Var, 0)).
@@ -408,8 +419,8 @@ size_t iterate_shared_bytes(int dim, int n_bins, int precision, int table_copies
 }
 
 cudaError_t launch_reduce(const double* partials, int n_parts, int n_tot, double* totals, cudaStream_t st) {
-    const int threads = 128;
-    k_reduce<<<(n_tot - 4 + 64 + threads - 1) / threads, threads, 0, st>>>(partials, n_parts, n_tot, totals);
+    const int threads = 256;                                  // k_reduce: 8 warps = 8 slices of the CTA partials
+    k_reduce<<<1 + (n_tot - 4 + 31) / 32, threads, 0, st>>>(partials, n_parts, n_tot, totals);
     return cudaGetLastError();
 }
 

@@ -295,6 +295,27 @@ def test_p6_event_range_sharding_matches_whole_iteration(B):
     g.close()
 
 
+def test_integrate_from_resumes_bit_for_bit(B):
+    """Checkpoint / resume: (grid, seed, next iteration index) is the whole state (counter-based RNG)."""
+    w = _small(4)
+    g = _grid(B, w)
+    whole = g.integrate(4, w.n_events, w.seed, w.alpha, w.integrand_id, 64)
+    edges_whole = g.get_edges()
+    g2 = _grid(B, w)
+    a = g2.integrate(2, w.n_events, w.seed, w.alpha, w.integrand_id, 64)
+    saved = g2.get_edges()
+    g2.close()
+    g3 = _grid(B, w, saved)                                  # a fresh grid object restored from the checkpoint
+    b = g3.integrate(2, w.n_events, w.seed, w.alpha, w.integrand_id, 64, first_iteration=2)
+    assert np.array_equal(np.vstack([a["per_iter"], b["per_iter"]]), whole["per_iter"])
+    assert np.array_equal(g3.get_edges(), edges_whole)
+    I, s, chi2 = B.vegas_combine(np.r_[a["per_iter"][:, 0], b["per_iter"][:, 0]], np.r_[a["per_iter"][:, 1], b["per_iter"][:, 1]])
+    assert I == whole["I"] and s == whole["sigma"]
+    with pytest.raises(B.VegasError):
+        g3.integrate(2, w.n_events, w.seed, w.alpha, w.integrand_id, 64, first_iteration=0xFFFFFFFE)
+    g.close(); g3.close()
+
+
 def test_plain_mc_mode_is_alpha_zero(B):
     """The paper's "Plain MC" column = the same iteration with the refinement switched off:
     alpha = 0 leaves the grid where it is (C8 fixed point), so every iteration samples the uniform grid."""

@@ -502,3 +502,42 @@ def test_full_size_iteration_in_bench_configuration(B, chains, cfg, precision):
     _assert_hist(H, oH, precision)
     assert abs(I - w.closed_form) < 5 * s
     g.close()
+
+
+# ------------------------------------------------------------------ full-size free-running chains vs the survey's probe
+@pytest.mark.parametrize("cfg", [2, 3, 4, 5])
+def test_full_size_chains_match_the_survey_probe(B, probe, cfg):
+    """The four large configs at their full BASELINE.json sizes, free-running (vegas_integrate), against the values an
+    independently written program produced during the survey (tests/golden/survey_probe.txt).
+    First iteration: same sample, same uniform grid -> agreement to rounding.  Combined results: the adaptive chain
+    amplifies rounding (finding F2) -> the printed digits (P5 gate 1e-8 on I)."""
+    w = W.config(cfg)
+    g = _grid(B, w)
+    r = g.integrate(w.n_iter, w.n_events, w.seed, w.alpha, w.integrand_id, 64, chunk_events=w.chunk_events)
+    flt = lambda key: [float(t) for t in probe[key]]
+    names = {2: ("cfg2.iter0", "cfg2.combined_all10"), 3: ("cfg3.iter0", "cfg3.combined_all10"),
+             4: ("cfg4.iter0", "cfg4.combined_all15"), 5: ("cfg5.iter0", "cfg5.combined_all20")}[cfg]
+    i0, comb = flt(names[0]), flt(names[1])
+    assert r["per_iter"][0, 0] == pytest.approx(i0[0], rel=1e-10)
+    assert r["per_iter"][0, 1] == pytest.approx(i0[1], rel=2e-3 if cfg == 3 else 1e-5)     # sigma_0 printed to 3-6 digits
+    assert r["I"] == pytest.approx(comb[0], rel=1e-8)
+    assert r["sigma"] == pytest.approx(comb[1], rel=1e-2 if cfg == 3 else 2e-5)
+    if len(comb) > 2:
+        assert r["chi2_dof"] == pytest.approx(comb[2], abs=0.006)
+    if cfg == 2:
+        assert r["per_iter"][1] == pytest.approx(flt("cfg2.iter1"), rel=1e-5)
+        assert r["per_iter"][1, 0] == pytest.approx(flt("cfg2.iter1")[0], rel=1e-10)
+    if cfg == 3:
+        i9, from1 = flt("cfg3.iter9"), flt("cfg3.combined_from1")
+        assert r["per_iter"][9, 0] == pytest.approx(i9[0], rel=1e-8) and r["per_iter"][9, 1] == pytest.approx(i9[1], rel=1e-4)
+        I, s, chi2 = B.vegas_combine(r["per_iter"][:, 0], r["per_iter"][:, 1], n_skip=1)
+        assert I == pytest.approx(from1[0], rel=1e-8) and s == pytest.approx(from1[1], rel=2e-3)
+        assert chi2 == pytest.approx(from1[2], abs=0.006)
+        # finding F1: the first iterations at d = 20 are far off for any correct implementation; from k = 3 on every
+        # estimate is within 5 sigma of the closed form
+        assert abs(r["per_iter"][0, 0] - w.closed_form) > 1000 * r["per_iter"][0, 1]
+        for k in range(3, 10):
+            assert abs(r["per_iter"][k, 0] - w.closed_form) < 5 * r["per_iter"][k, 1]
+    else:
+        assert abs(r["I"] - w.closed_form) < 5 * r["sigma"]
+    g.close()

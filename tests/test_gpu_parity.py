@@ -541,3 +541,25 @@ def test_full_size_chains_match_the_survey_probe(B, probe, cfg):
     else:
         assert abs(r["I"] - w.closed_form) < 5 * r["sigma"]
     g.close()
+
+
+def test_genz_product_peak_at_the_papers_16_dimensions(B):
+    """PAPER.md:86 (Table 1, "Genz Eq.(3) 16-d"): the product peak at the paper's dimension count, teacher-forced on
+    oracle grids (P3/P4) and free-running against the arctan closed form (5 sigma)."""
+    dim, nb, n, seed = 16, 50, 400_003, 16
+    p = W.genz_params(dim, seed)
+    ch = O.integrate(dim, nb, 3, n, seed, 1.5, O.GENZ_PRODUCT_PEAK, p, threads=THREADS)
+    g = B.VegasGrid(dim, nb)
+    g.set_params(B.VEGAS_F_GENZ_PRODUCT_PEAK, p)
+    for prec, tol in ((64, RTOL64), (32, RTOL32)):
+        for k in range(3):
+            g.set_edges(ch["edges_trace"][k])
+            I, s, H, st = g.iterate(n, seed, k, B.VEGAS_F_GENZ_PRODUCT_PEAK, prec)
+            assert st == 0 and I == pytest.approx(ch["per_iter"][k, 0], rel=tol)
+            assert s == pytest.approx(ch["per_iter"][k, 1], rel=tol if prec == 64 else 1e-4)
+            _assert_hist(H, ch["hist_trace"][k], prec)
+    g.set_edges(O.uniform_edges(dim, nb))
+    r = g.integrate(8, 4_000_000, seed, 1.5, B.VEGAS_F_GENZ_PRODUCT_PEAK, 64, n_skip=3)
+    exact = W.closed_form(W.GENZ_PRODUCT_PEAK, dim, p)
+    assert abs(r["I"] - exact) < 5 * r["sigma"] and r["sigma"] / exact < 1e-2
+    g.close()

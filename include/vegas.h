@@ -122,6 +122,23 @@ int vegas_set_params(vegas_grid* g, int integrand_id, const double* params_host,
 int vegas_set_user_integrand(vegas_grid* g, const char* cuda_source, const double* params_host, int n_params,
                              char* log, size_t log_bytes);
 
+/* Host-callback integrands (integrands written "in Fortran, C/C++" reach the paper's library through
+ * CFFI, second half).  One iteration like vegas_iterate(), but f is evaluated by a HOST function
+ * on batches of points: per batch of at most batch_events events the library samples x on the device (S1-S3), copies
+ * x [n][dim] (row-major fp64) to the host, calls fn(x, n, dim, f, user) -- which must fill f[0..n-1] -- copies f back
+ * and accumulates S1, S2 and the histogram on the device (S5-S6).  Same sample, same sums as a device integrand with
+ * the same f; fp64; this is a convenience path bound by the host function and the PCIe copies, not the hot path.
+ * dev_scratch: device memory, 256-byte aligned, at least vegas_callback_scratch_bytes(dim, batch_events) bytes
+ * (caller-owned; about batch_events * (20 dim + 16) bytes).  The callback runs on the calling thread, between stream
+ * synchronisations; it must not call into this grid.
+ * Errors: VEGAS_EINVAL (NULL fn / scratch, n_events < 2, batch_events = 0, scratch too small or misaligned),
+ * VEGAS_ECUDA, VEGAS_ENUMERIC (a non-finite f makes the sums non-finite; I, sigma are still written). */
+typedef void (*vegas_host_integrand)(const double* x, uint64_t n, int dim, double* f, void* user);
+size_t vegas_callback_scratch_bytes(int dim, uint32_t batch_events);
+int vegas_iterate_callback(vegas_grid* g, uint64_t n_events, uint32_t batch_events, uint64_t seed, uint32_t iteration,
+                           vegas_host_integrand fn, void* user, void* dev_scratch, size_t scratch_bytes,
+                           void* cuda_stream, double* I, double* sigma, double* hist_host);
+
 /* Inject / read the master grid: edges_host is [dim][n_bins+1] fp64, every row strictly increasing
  * with first element 0 and last element 1 (checked -> VEGAS_EINVAL).  Synchronous on `stream`. */
 int vegas_set_edges(vegas_grid* g, const double* edges_host, void* cuda_stream);

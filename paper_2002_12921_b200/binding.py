@@ -38,6 +38,9 @@ SIGNATURES = {
     "vegas_destroy": (C.c_int, [_vp]),
     "vegas_set_params": (C.c_int, [_vp, C.c_int, _f64p, C.c_int]),
     "vegas_set_user_integrand": (C.c_int, [_vp, C.c_char_p, _f64p, C.c_int, C.c_char_p, C.c_size_t]),
+    "vegas_callback_scratch_bytes": (C.c_size_t, [C.c_int, C.c_uint32]),
+    "vegas_iterate_callback": (C.c_int, [_vp, _u64, C.c_uint32, _u64, C.c_uint32, _vp, _vp, _vp, C.c_size_t, _vp,
+                                         _f64p, _f64p, _f64p]),
     "vegas_set_edges": (C.c_int, [_vp, _f64p, _vp]),
     "vegas_get_edges": (C.c_int, [_vp, _f64p, _vp]),
     "vegas_get_hist": (C.c_int, [_vp, _f64p, _vp]),
@@ -72,6 +75,9 @@ for _name, (_res, _args) in SIGNATURES.items():
     _fn = getattr(lib, _name)          # AttributeError here = the library does not export it
     _fn.restype = _res
     _fn.argtypes = _args
+
+
+HOST_INTEGRAND = C.CFUNCTYPE(None, _f64p, _u64, C.c_int, _f64p, _vp)
 
 
 class VegasError(RuntimeError):
@@ -202,6 +208,30 @@ class VegasGrid:
         rc = lib.vegas_iterate(self._h, int(n_events), int(chunk_events), int(seed), int(iteration), integrand_id,
                                precision, _stream(stream), C.byref(I), C.byref(s), _ptr(h))
         return I.value, s.value, h, self._check(rc, allow_numeric=True)
+
+    def iterate_callback(self, fn, n_events, seed, iteration, batch_events=1 << 18, want_hist=True, stream=None):
+        """One iteration with a HOST integrand: fn(x) takes a float64 array [n, dim] and returns n values.
+        -> (I, sigma, hist or None, status)"""
+        import torch
+        n_batch = int(min(batch_events, n_events))
+        nbytes = lib.vegas_callback_scratch_bytes(self.dim, n_batch)
+        scratch = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        ptr = (scratch.data_ptr() + 255) // 256 * 256
+        dim = self.dim
+
+        @HOST_INTEGRAND
+        def _cb(x, n, d, f, user):
+            xs = np.ctypeslib.as_array(x, shape=(n, d))
+            out = np.ctypeslib.as_array(f, shape=(n,))
+            out[:] = np.asarray(fn(xs), dtype=np.float64)
+
+        I, s = C.c_double(), C.c_double()
+        H = np.zeros((self.dim, self.n_bins)) if want_hist else None
+        rc = lib.vegas_iterate_callback(self._h, int(n_events), n_batch, int(seed), int(iteration),
+                                        C.cast(_cb, _vp), None, _vp(ptr), nbytes, _stream(stream),
+                                        C.byref(I), C.byref(s), _ptr(H) if want_hist else None)
+        self._check(rc, allow_numeric=True)
+        return I.value, s.value, H, rc
 
     def begin_iteration(self, stream=None):
         self._check(lib.vegas_begin_iteration(self._h, _stream(stream)))

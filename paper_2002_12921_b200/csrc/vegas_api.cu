@@ -739,6 +739,58 @@ int vegas_debug_sample(vegas_grid* g, uint64_t first_event, uint32_t count, uint
     return VEGAS_OK;
 }
 
+size_t vegas_callback_scratch_bytes(int dim, uint32_t batch_events) {
+    if (dim < 1 || dim > VEGAS_MAX_DIM || batch_events == 0) return 0;
+    return vegas_debug_scratch_bytes(dim, batch_events) + align_up((size_t)batch_events * 8);
+}
+
+int vegas_iterate_callback(vegas_grid* g, uint64_t n_events, uint32_t batch_events, uint64_t seed, uint32_t iteration,
+                           vegas_host_integrand fn, void* user, void* dev_scratch, size_t scratch_bytes,
+                           void* cuda_stream, double* I, double* sigma, double* hist_host) {
+    if (!g || !fn || !dev_scratch || n_events < 2 || batch_events == 0) return VEGAS_EINVAL;
+    if (((uintptr_t)dev_scratch) % kAlign) return VEGAS_EINVAL;
+    if (scratch_bytes < vegas_callback_scratch_bytes(g->dim, batch_events)) return VEGAS_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = vegas_begin_iteration(g, cuda_stream);
+    if (rc) return rc;
+    const int dim = g->dim;
+    const size_t per_dim = (size_t)batch_events * dim;
+    unsigned char* base = (unsigned char*)dev_scratch;
+    vegas::DebugArgs a{};
+    a.edges = g->d_edges;
+    a.key0 = (uint32_t)(seed & 0xFFFFFFFFu);
+    a.key1 = (uint32_t)(seed >> 32);
+    a.iteration = iteration;
+    a.dim = dim;
+    a.n_bins = g->n_bins;
+    a.jac_scale = jac_scale_for(g, VEGAS_FP64);
+    a.words = (uint32_t*)base;                 base += align_up(per_dim * 4);
+    a.bins = (int32_t*)base;                   base += align_up(per_dim * 4);
+    a.x = (double*)base;                       base += align_up(per_dim * 8);
+    a.fJ = (double*)base;                      base += align_up((size_t)batch_events * 8);
+    double* d_f = (double*)base;
+    std::vector<double> x_host(per_dim), f_host(batch_events);
+    const int blocks = g->active_blocks < g->sm_count ? g->active_blocks : g->sm_count;
+    for (uint64_t done = 0; done < n_events; done += batch_events) {
+        const uint32_t n = (uint32_t)((n_events - done < batch_events) ? n_events - done : batch_events);
+        a.first_event = done;
+        a.count = n;
+        // S1-S3 for the batch with f = 1: x, bins and J = prod n_bins Delta go to the scratch (the only place in the
+        // library where per-event arrays exist)
+        CUDA_TRY(g, vegas::launch_debug(VEGAS_F_CONST, VEGAS_FP64, false, a, g->derived[VEGAS_F_CONST], st));
+        CUDA_TRY(g, cudaMemcpyAsync(x_host.data(), a.x, sizeof(double) * (size_t)n * dim, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(g, cudaStreamSynchronize(st));
+        fn(x_host.data(), (uint64_t)n, dim, f_host.data(), user);                    // S4 on the host
+        CUDA_TRY(g, cudaMemcpyAsync(d_f, f_host.data(), sizeof(double) * n, cudaMemcpyHostToDevice, st));
+        CUDA_TRY(g, vegas::launch_accumulate_batch(d_f, a.fJ, a.bins, n, dim, g->n_bins, g->d_partials, blocks, st));
+        CUDA_TRY(g, cudaStreamSynchronize(st));                                       // f_host is reused by the next batch
+        g->launches += 2;
+    }
+    rc = vegas_reduce(g, cuda_stream);
+    if (rc) return rc;
+    return finish_iteration(g, n_events, st, I, sigma, hist_host);
+}
+
 int vegas_set_launch(vegas_grid* g, int blocks, int threads, int table_copies, int hist_copies) {
     if (!g || blocks < 0 || threads < 0 || table_copies < 0 || hist_copies < 0) return VEGAS_EINVAL;
     auto pow2 = [](int v) { return v == 0 || (v & (v - 1)) == 0; };

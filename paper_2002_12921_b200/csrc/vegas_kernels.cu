@@ -314,6 +314,50 @@ __global__ void k_debug(const DebugArgs a, const __grid_constant__ FParams<T> fp
     a.fJ[q] = (double)(f.finish(fp) * jac) * a.jac_scale;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Host-callback path (vegas_iterate_callback: integrands written in C or Fortran):
+// the batch's points were produced by k_debug<CONST> (x, bins, J), the caller's host function supplied f; this kernel
+// is steps S5/S6 on the stored batch.  Not the hot path: it exists so that a host integrand can be used at all.
+// Shared memory: one fp64 histogram of dim*n_bins words, then the block-reduction scratch.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_accumulate_batch(const double* __restrict__ f, const double* __restrict__ J, const int32_t* __restrict__ bins,
+                   uint32_t count, int dim, int nb, double* __restrict__ partials) {
+    extern __shared__ __align__(16) unsigned char smem_cb[];
+    const int nent = dim * nb;
+    double* hist = reinterpret_cast<double*>(smem_cb);
+    dd* red = reinterpret_cast<dd*>(smem_cb + sizeof(double) * nent);
+    for (int i = threadIdx.x; i < nent; i += blockDim.x) hist[i] = 0.0;
+    __syncthreads();
+    double s1 = 0.0, c1 = 0.0, s2 = 0.0, c2 = 0.0;
+    for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < count; e += gridDim.x * blockDim.x) {
+        const double v = f[e] * J[e];                       // C6: v = f J
+        const double v2 = v * v;
+        kahan_add(s1, c1, v);
+        kahan_add(s2, c2, v2);
+        const int32_t* b = bins + (size_t)e * dim;
+        for (int j = 0; j < dim; ++j) atomicAdd(hist + j * nb + b[j], v2);
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = (blockDim.x + 31) >> 5;
+    dd t1 = dd_warp_sum(fast_two_sum(s1, -c1));
+    dd t2 = dd_warp_sum(fast_two_sum(s2, -c2));
+    if (lane == 0) { red[2 * warp] = t1; red[2 * warp + 1] = t2; }
+    __syncthreads();
+    double* part = partials + (size_t)blockIdx.x * (4 + nent);
+    if (warp == 0) {
+        t1 = (lane < nwarps) ? red[2 * lane] : dd{0.0, 0.0};
+        t2 = (lane < nwarps) ? red[2 * lane + 1] : dd{0.0, 0.0};
+        t1 = dd_warp_sum(t1);
+        t2 = dd_warp_sum(t2);
+        if (lane == 0) {
+            t1 = dd_add(t1, dd{part[0], part[1]});
+            t2 = dd_add(t2, dd{part[2], part[3]});
+            part[0] = t1.hi; part[1] = t1.lo; part[2] = t2.hi; part[3] = t2.lo;
+        }
+    }
+    for (int i = threadIdx.x; i < nent; i += blockDim.x) part[4 + i] += hist[i];
+}
+
 // K4 for the fast path: u_j and f*J through the device functions of k_iterate_rot (RotEntry,
 // IntegrandU); x_j, which that kernel never forms, is reported from the plain map (C4).
 template <int FID, typename T>
@@ -461,6 +505,19 @@ static cudaError_t launch_debug_rot_t(int fid, const DebugArgs& a, cudaStream_t 
     case VEGAS_F_BW_POLY: k_debug_rot<VEGAS_F_BW_POLY, T><<<blocks, threads, 0, st>>>(a); break;
     default: return cudaErrorInvalidValue;
     }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_accumulate_batch(const double* f, const double* J, const int32_t* bins, uint32_t count, int dim,
+                                    int n_bins, double* partials, int blocks, cudaStream_t st) {
+    const size_t shmem = sizeof(double) * (size_t)dim * n_bins + 2 * sizeof(dd) * 8;
+    static size_t configured = 0;
+    if (shmem > configured) {
+        cudaError_t e = cudaFuncSetAttribute(k_accumulate_batch, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem);
+        if (e != cudaSuccess) return e;
+        configured = shmem;
+    }
+    k_accumulate_batch<<<blocks, 256, shmem, st>>>(f, J, bins, count, dim, n_bins, partials);
     return cudaGetLastError();
 }
 

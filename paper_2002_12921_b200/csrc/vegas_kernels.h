@@ -54,6 +54,8 @@ cudaError_t launch_reduce(const double* partials, int n_parts, int n_tot, double
 cudaError_t launch_finalize(const double* totals, double n_events, double* result, cudaStream_t st);
 cudaError_t launch_refine(double* edges, const double* hist, int dim, int n_bins, double alpha, int* status,
                           cudaStream_t st);
+cudaError_t launch_accumulate_batch(const double* f, const double* J, const int32_t* bins, uint32_t count, int dim,
+                                    int n_bins, double* partials, int blocks, cudaStream_t st);
 cudaError_t launch_debug(int fid, int precision, bool rot_path, const DebugArgs& a, const double* derived_params,
                          cudaStream_t st);
 

@@ -115,3 +115,38 @@ def test_user_integrand_parameters_and_errors(B):
     oI3, _, _ = O.iterate(edges, 100_003, 5, 0, O.GENZ_PRODUCT_PEAK, W.genz_params(6, 8))
     assert I3 == pytest.approx(oI3, rel=RTOL64)
     g.close()
+
+
+def test_host_callback_integrand_matches_the_oracle(B):
+    """vegas_iterate_callback (second half): f evaluated by a HOST function on batches of points
+    sampled on the device; same sample and sums as the oracle's iteration with the same f (fp64 tolerances)."""
+    dim, nb, n, seed = 7, 40, 250_003, 31
+    p = W.genz_params(dim, 5)
+    c, wv = p[:dim], p[dim:]
+    edges = W.adapted_edges(dim, nb, seed=3)
+    calls = []
+
+    def f_host(x):                                   # numpy restatement of Eq.(3): the "user's C/Fortran function"
+        calls.append(x.shape[0])
+        assert x.shape[1] == dim and np.all((x > 0) & (x < 1))
+        return 1.0 / np.prod(1.0 / (c * c) + (x - wv) ** 2, axis=1)
+
+    g = B.VegasGrid(dim, nb)
+    g.set_edges(edges)
+    I, s, H, st = g.iterate_callback(f_host, n, seed, 2, batch_events=100_000)
+    assert st == 0 and calls == [100_000, 100_000, 50_003]
+    oI, oS, oH = O.iterate(edges, n, seed, 2, O.GENZ_PRODUCT_PEAK, p)
+    assert I == pytest.approx(oI, rel=RTOL64) and s == pytest.approx(oS, rel=RTOL64)
+    _hist_ok(H, oH)
+    # the device integrand on the same grid object gives the same iteration
+    g.set_params(B.VEGAS_F_GENZ_PRODUCT_PEAK, p)
+    Id, sd, Hd, _ = g.iterate(n, seed, 2, B.VEGAS_F_GENZ_PRODUCT_PEAK, 64)
+    assert I == pytest.approx(Id, rel=1e-12) and s == pytest.approx(sd, rel=1e-11)
+    # refinement from the callback iteration's histogram
+    assert g.refine(1.5) == 0
+    want, _ = O.refine(edges, oH, 1.5)
+    np.testing.assert_allclose(g.get_edges(), want, rtol=0, atol=1e-10)
+    # a non-finite f is reported, not hidden
+    I2, s2, _, st2 = g.iterate_callback(lambda x: np.full(x.shape[0], np.inf), 1000, seed, 0, batch_events=512)
+    assert st2 == B.VEGAS_ENUMERIC
+    g.close()

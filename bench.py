@@ -199,6 +199,14 @@ def main():
     import numpy as np
     import torch
     import torch.distributed as dist
+    if local_rank == 0:
+        from paper_2002_12921_b200 import build as lib_build
+        lib_build.build()                                         # no-op when libvegas_b200.so is up to date
+    if world > 1:
+        import time as _t
+        from paper_2002_12921_b200.build import LIB as _lib_path
+        while not os.path.exists(_lib_path):                      # other ranks wait for rank 0's build
+            _t.sleep(0.5)
     from paper_2002_12921_b200 import binding as B
     from paper_2002_12921_b200 import distributed as D
 

@@ -22,6 +22,8 @@ def B():
     import torch
     if not torch.cuda.is_available():
         pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
+    from paper_2002_12921_b200 import build
+    build.build()                                   # no-op when libvegas_b200.so is up to date
     from paper_2002_12921_b200 import binding
     return binding
 

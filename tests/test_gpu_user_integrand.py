@@ -152,3 +152,33 @@ def test_host_callback_integrand_matches_the_oracle(B):
     I2, s2, _, st2 = g.iterate_callback(lambda x: np.full(x.shape[0], np.inf), 1000, seed, 0, batch_events=512)
     assert st2 == B.VEGAS_ENUMERIC
     g.close()
+
+
+def test_user_integrand_shape_limits_and_no_parameters(B):
+    # a shape whose table plus one histogram copy exceed the 227 KB of shared memory has no fast path: refused
+    g = B.VegasGrid(32, 256)
+    with pytest.raises(B.VegasError) as ei:
+        g.set_user_integrand(U.GAUSS, [0.1])
+    assert ei.value.code == B.VEGAS_EINVAL
+    g.close()
+    # an integrand without parameters: f = prod_j 2 x_j integrates to 1
+    src = """
+    struct vegas_user_integrand {
+        double prod;
+        __device__ void begin(int dim, const double* p) { prod = 1.0; }
+        __device__ void dim(int j, double x, const double* p) { prod *= 2.0 * x; }
+        __device__ double finish(const double* p) { return prod; }
+    };"""
+    g = B.VegasGrid(3, 16)
+    g.set_user_integrand(src)
+    r = g.integrate(5, 1_000_000, 7, 1.5, B.VEGAS_F_USER, 64, n_skip=1)
+    assert abs(r["I"] - 1.0) < 5 * r["sigma"] and r["sigma"] < 1e-3
+    # host callback with a batch larger than the iteration, and the same f: same sample -> same first iteration
+    g2 = B.VegasGrid(3, 16)
+    I, s, H, st = g2.iterate_callback(lambda x: np.prod(2.0 * x, axis=1), 1_000_000, 7, 0, batch_events=1 << 21)
+    g3 = B.VegasGrid(3, 16)
+    g3.set_user_integrand(src)
+    Iu, su, Hu, _ = g3.iterate(1_000_000, 7, 0, B.VEGAS_F_USER, 64)
+    assert I == pytest.approx(Iu, rel=1e-12) and s == pytest.approx(su, rel=1e-11)
+    np.testing.assert_allclose(H, Hu, rtol=1e-11)
+    g.close(); g2.close(); g3.close()

@@ -177,6 +177,9 @@ def main():
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32])
     ap.add_argument("--n-events", type=int, default=0, help="override events per step per GPU")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--alpha", type=float, default=None,
+                    help="override the damping exponent (0 = plain MC: the grid stays uniform; SURVEY.md 8(d) asks for "
+                         "one timing on the uniform grid)")
     ap.add_argument("--user-integrand", action="store_true",
                     help="run the workload's integrand as a run-time compiled user integrand (VEGAS_F_USER; gauss / genz only)")
     ap.add_argument("--launch", default="", help="blocks,threads,table_copies,hist_copies (0 = auto)")
@@ -187,6 +190,9 @@ def main():
     w = W.config(int(args.workload.replace("cfg", "")))
     if args.n_events:
         w = w.scaled(args.n_events)
+    if args.alpha is not None:
+        import dataclasses
+        w = dataclasses.replace(w, alpha=args.alpha)
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -353,7 +359,7 @@ def main():
                            "n_events_per_gpu_per_step": w.n_events, "chunk_events": w.chunk_events, "alpha": w.alpha,
                            "seed": w.seed, "launch": shape, "l2": "256 MiB memset between timed steps, outside the event brackets "
                            "(the path reads ~10 KB of global memory per launch)",
-                           "grid": "adapted by the %d warm-up iterations" % args.warmup},
+                           "grid": ("uniform (alpha = 0)" if w.alpha == 0 else "adapted by the %d warm-up iterations" % args.warmup)},
                 "clocks": clocks, "wall_s_timed_region": t_wall,
                 "e2e": {"value": n_step * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
                 "gpu_launches": int(launches),

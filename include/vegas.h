@@ -149,7 +149,8 @@ int vegas_get_hist(vegas_grid* g, double* hist_host, void* cuda_stream);
 /* One Vegas iteration (steps S1-S7 of SURVEY.md 8(a)): n_events events with global indices
  * 0..n_events-1 of iteration `iteration`, processed in launches of at most chunk_events events
  * (0 = a single launch; the result does not depend on it beyond summation order, every event's RNG
- * counter is its global index, C2).  Writes I and sigma (host doubles, C7) and, if hist_host is not
+ * counter is its global index, C2; the fast path additionally splits a launch at multiples of 2^32 of
+ * the event index).  Writes I and sigma (host doubles, C7) and, if hist_host is not
  * NULL, the histogram [dim][n_bins] (host); the histogram also stays on the device for
  * vegas_refine(g, NULL, ...).  Synchronises `stream` before returning.
  * Errors: VEGAS_EINVAL (n_events < 2, unknown id/precision, params not set), VEGAS_ECUDA,
@@ -217,10 +218,11 @@ int vegas_debug_sample(vegas_grid* g, uint64_t first_event, uint32_t count, uint
                        void* cuda_stream, uint32_t* words, int32_t* bins, double* x, double* fJ);
 
 /* Launch shape of the fused kernel.  0 = automatic for any field.  blocks: CTAs per launch (default:
- * one or two per SM); threads: per CTA (multiple of 32, <= 512).  The library has two fused kernels
+ * one per SM); threads: per CTA (multiple of 32, <= 512).  The library has two fused kernels
  * (DESIGN.md "Kernels"): the fast path (path 1: compile-time dimension, affine pre-composed table, bank
- * rotation; CONST and GAUSS in both precisions, GENZ product peak in fp64, when its shared memory fits)
- * and the generic path (path 0: every integrand, any shape).  table_copies / hist_copies are the
+ * rotation, exclusive-owner histograms; every built-in integrand in both precisions -- BW_POLY up to 8 dimensions --
+ * and user integrands, when the table plus one histogram copy fit the shared memory)
+ * and the generic path (path 0: every built-in integrand, any shape).  table_copies / hist_copies are the
  * bank-interleaved replicas of the grid table / histogram of the GENERIC kernel (powers of two, <= 32);
  * setting either to a non-zero value pins the generic path.  VEGAS_EINVAL if the combination does not fit
  * the device's shared memory.  vegas_get_launch reports what a call with (integrand_id, precision) will use. */

@@ -122,6 +122,18 @@ int vegas_set_params(vegas_grid* g, int integrand_id, const double* params_host,
 int vegas_set_user_integrand(vegas_grid* g, const char* cuda_source, const double* params_host, int n_params,
                              char* log, size_t log_bytes);
 
+/* Histogram of an observable during the integration ("exporting histograms during integration").
+ * If the user integrand's struct also defines
+ *         __device__ double observable(const double* p);     // called after finish(), same event
+ * and vegas_set_observable(g, lo, hi, n_obs_bins) was called with 1 <= n_obs_bins <= 128, every iteration with
+ * VEGAS_F_USER also accumulates  O[k] += v  (v = f*J of the event) for k = floor((observable - lo) / (hi - lo) *
+ * n_obs_bins) in [0, n_obs_bins); events outside [lo, hi) are not counted.  vegas_get_observable_hist() copies the n_obs_bins
+ * sums of the LAST iteration to the host (divide by n_events and the bin width for dI/dO); one shared-memory add per
+ * event in the fused kernel and one global add per bin per CTA per launch, so the last bits depend on the CTA order.
+ * n_obs_bins = 0 switches it off.  Errors: VEGAS_EINVAL (hi <= lo, n_obs_bins out of range, nothing to get). */
+int vegas_set_observable(vegas_grid* g, double lo, double hi, int n_obs_bins);
+int vegas_get_observable_hist(vegas_grid* g, double* obs_hist_host, void* cuda_stream);
+
 /* Host-callback integrands (integrands written "in Fortran, C/C++" reach the paper's library through
  * CFFI, second half).  One iteration like vegas_iterate(), but f is evaluated by a HOST function
  * on batches of points: per batch of at most batch_events events the library samples x on the device (S1-S3), copies

@@ -38,6 +38,8 @@ SIGNATURES = {
     "vegas_destroy": (C.c_int, [_vp]),
     "vegas_set_params": (C.c_int, [_vp, C.c_int, _f64p, C.c_int]),
     "vegas_set_user_integrand": (C.c_int, [_vp, C.c_char_p, _f64p, C.c_int, C.c_char_p, C.c_size_t]),
+    "vegas_set_observable": (C.c_int, [_vp, C.c_double, C.c_double, C.c_int]),
+    "vegas_get_observable_hist": (C.c_int, [_vp, _f64p, _vp]),
     "vegas_callback_scratch_bytes": (C.c_size_t, [C.c_int, C.c_uint32]),
     "vegas_iterate_callback": (C.c_int, [_vp, _u64, C.c_uint32, _u64, C.c_uint32, _vp, _vp, _vp, C.c_size_t, _vp,
                                          _f64p, _f64p, _f64p]),
@@ -182,6 +184,15 @@ class VegasGrid:
         if rc != VEGAS_OK:
             raise VegasError(rc, text or lib.vegas_last_cuda_error(self._h).decode())
         return text
+
+    def set_observable(self, lo, hi, n_obs_bins):
+        self._check(lib.vegas_set_observable(self._h, float(lo), float(hi), int(n_obs_bins)))
+        self._n_obs = int(n_obs_bins)
+
+    def get_observable_hist(self, stream=None):
+        out = np.zeros(self._n_obs)
+        self._check(lib.vegas_get_observable_hist(self._h, _ptr(out), _stream(stream)))
+        return out
 
     def set_edges(self, edges, stream=None):
         e = np.ascontiguousarray(edges, dtype=np.float64)

@@ -26,7 +26,7 @@ constexpr size_t kAlign = 256;
 size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t edges, totals, result, status, hist_up, partials, total;
+    size_t edges, totals, result, status, hist_up, obs, partials, total;
 };
 
 Layout make_layout(int dim, int n_bins) {
@@ -38,6 +38,7 @@ Layout make_layout(int dim, int n_bins) {
     L.result = off;   off += align_up(sizeof(double) * kResultStride * kMaxIter);
     L.status = off;   off += align_up(sizeof(int) * 8);
     L.hist_up = off;  off += align_up(sizeof(double) * nent);
+    L.obs = off;      off += align_up(sizeof(double) * vegas::kRotMaxObsBins);
     L.partials = off; off += align_up(sizeof(double) * ntot * kMaxBlocks);
     L.total = off;
     return L;
@@ -70,6 +71,9 @@ struct vegas_grid {
     int* d_status = nullptr;
     double* d_hist_up = nullptr;
     double* d_partials = nullptr;
+    double* d_obs = nullptr;                     // observable histogram of a user integrand: sums of v per bin
+    int n_obs = 0;
+    double obs_lo = 0.0, obs_hi = 1.0;
     bool params_set[5] = {true, false, false, false, false};
     double derived[5][VEGAS_MAX_PARAMS] = {};
     double user[5][VEGAS_MAX_PARAMS] = {};       // the caller's arrays as given to vegas_set_params
@@ -344,6 +348,7 @@ int vegas_create(int dim, int n_bins, void* dev_workspace, size_t bytes, vegas_g
     g->d_status = (int*)(g->ws + L.status);
     g->d_hist_up = (double*)(g->ws + L.hist_up);
     g->d_partials = (double*)(g->ws + L.partials);
+    g->d_obs = (double*)(g->ws + L.obs);
     std::vector<double> edges((size_t)dim * (n_bins + 1));
     for (int j = 0; j < dim; ++j)
         for (int i = 0; i <= n_bins; ++i) edges[(size_t)j * (n_bins + 1) + i] = (double)i / (double)n_bins;
@@ -432,6 +437,24 @@ int vegas_set_user_integrand(vegas_grid* g, const char* cuda_source, const doubl
     return rc == -1 ? VEGAS_EINVAL : VEGAS_ECUDA;
 }
 
+int vegas_set_observable(vegas_grid* g, double lo, double hi, int n_obs_bins) {
+    if (!g || n_obs_bins < 0 || n_obs_bins > vegas::kRotMaxObsBins) return VEGAS_EINVAL;
+    if (n_obs_bins > 0 && (!(hi > lo) || !std::isfinite(lo) || !std::isfinite(hi))) return VEGAS_EINVAL;
+    g->n_obs = n_obs_bins;
+    g->obs_lo = lo;
+    g->obs_hi = hi;
+    return VEGAS_OK;
+}
+
+int vegas_get_observable_hist(vegas_grid* g, double* obs_hist_host, void* cuda_stream) {
+    if (!g || !obs_hist_host || g->n_obs <= 0) return VEGAS_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CUDA_TRY(g, cudaSetDevice(g->device));
+    CUDA_TRY(g, cudaMemcpyAsync(obs_hist_host, g->d_obs, sizeof(double) * g->n_obs, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(g, cudaStreamSynchronize(st));
+    return VEGAS_OK;
+}
+
 int vegas_set_edges(vegas_grid* g, const double* edges_host, void* cuda_stream) {
     if (!g || !edges_host) return VEGAS_EINVAL;
     const int nb = g->n_bins;
@@ -482,6 +505,7 @@ int vegas_begin_iteration(vegas_grid* g, void* cuda_stream) {
     g->active_blocks = blocks;
     const size_t ntot = 4 + (size_t)g->dim * g->n_bins;
     CUDA_TRY(g, cudaMemsetAsync(g->d_partials, 0, sizeof(double) * ntot * blocks, st));
+    if (g->n_obs > 0) CUDA_TRY(g, cudaMemsetAsync(g->d_obs, 0, sizeof(double) * vegas::kRotMaxObsBins, st));
     return VEGAS_OK;
 }
 
@@ -510,6 +534,12 @@ int vegas_accumulate(vegas_grid* g, uint64_t first_event, uint64_t count, uint64
         ra.n_groups = rs.n_groups;
         ra.ring = rs.ring;
         rot_constants(g, fid, precision, ra.shift, ra.scale, &ra.post_scale, &ra.fin0, &ra.jac_init, ra.fpar);
+        if (fid == VEGAS_F_USER && g->n_obs > 0) {
+            ra.obs = g->d_obs;
+            ra.n_obs = g->n_obs;
+            ra.obs_lo = g->obs_lo;
+            ra.obs_inv_width = (double)g->n_obs / (g->obs_hi - g->obs_lo);
+        }
     } else {
         if (resolve_launch(g, precision, &s)) return VEGAS_EINVAL;
         if (s.blocks > g->active_blocks) return VEGAS_EINVAL;

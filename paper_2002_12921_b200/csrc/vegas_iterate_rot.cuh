@@ -100,6 +100,7 @@ template <typename T, int NCH> struct IntegrandU<VEGAS_F_GENZ_PRODUCT_PEAK, T, N
 // f = [1/(1 + u_0^2)] * [sum_j a_j0 + sum_j u_j (a_j1 + u_j (a_j2 + u_j (a_j3 + u_j a_j4)))].
 // The lane that holds dimension 0 at sub-step i of block 0 runs the quartic with zero coefficients and keeps u.
 constexpr int kRotBwMaxDim = 8;    // 4 coefficient registers pairs per dimension per lane
+constexpr int kRotMaxObsBins = 128; // observable histogram of a user integrand (vegas_set_observable)
 constexpr int kRotParams = 64;     // doubles of integrand parameters carried in the kernel arguments (VEGAS_USER_MAX_PARAMS)
 template <typename T, int NCH> struct IntegrandU<VEGAS_F_BW_POLY, T, NCH> {
     T poly[NCH], u0;
@@ -184,6 +185,9 @@ struct RotArgs {
     double jac_init;                // start value of the running Jacobian product (a power of two, see RotEntry)
     double fin0;                    // integrand finish constant
     double shift[VEGAS_MAX_DIM], scale[VEGAS_MAX_DIM];
+    double* obs;                    // USER with an observable: device, [n_obs] sums of v per observable bin, or NULL
+    int n_obs;                      // 0 = no observable histogram
+    double obs_lo, obs_inv_width;   // bin k = floor((O - obs_lo) * obs_inv_width)
     double fpar[kRotParams];        // BW_POLY: a[j][k] at fpar[5 j + k], j = 1..dim-1 (row 0 unused); USER: the caller's array
 };
 
@@ -220,8 +224,18 @@ template <typename T, int NBLK> struct RotCtx<VEGAS_F_USER, T, NBLK> {
         p = r.fpar; gamma4 = g4; gammaL = gL; nblk = (d + 3) / 4; dim = d;
     }
 };
+template <class U> struct user_has_observable {
+    template <class V> static __device__ char test(decltype(&V::observable));
+    template <class V> static __device__ long test(...);
+    static constexpr bool value = sizeof(test<U>(0)) == sizeof(char);
+};
 template <typename T, int NCH> struct IntegrandU<VEGAS_F_USER, T, NCH> {
+    static constexpr bool kObservable = user_has_observable<vegas_user_integrand>::value;
     vegas_user_integrand f;
+    __device__ __forceinline__ double observable() {
+        if constexpr (kObservable) return f.observable(p);
+        else return 0.0;
+    }
     const double* p;
     template <class C> __device__ __forceinline__ void begin(const C& c) { p = c.p; f.begin(c.dim, p); }
     template <class C> __device__ __forceinline__ void dim(T u, int blk, int i, const C& c) {
@@ -302,7 +316,7 @@ __device__ __forceinline__ void philox4x32_10_args(uint32_t c0, uint32_t c1, uin
 template <int FID, typename T, int DIM>
 __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, DIM>& L,
                                             const RotCtx<FID, T, (DIM + 3) / 4>& ctx, uint32_t e_lo, uint32_t e_hi,
-                                            bool live, T fin0, uint32_t (&taddr)[(DIM + 3) / 4][4]) {
+                                            bool live, T fin0, uint32_t (&taddr)[(DIM + 3) / 4][4], double& obs_val) {
     using E = RotEntry<T>;
     using T2 = typename E::type;
     constexpr int NBLK = RotLane<T, DIM>::NBLK, R = RotLane<T, DIM>::R, GL = RotLane<T, DIM>::GL;
@@ -366,7 +380,11 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
     const T jall = chain_prod<NCH, T>(jac);
     if (sizeof(T) == 8) {
         const double wgt = live ? (double)jall * a.post_scale : 0.0;
-        return (double)f.finish(fin0) * wgt;
+        const double fv = (double)f.finish(fin0);
+#ifdef VEGAS_USER_INTEGRAND
+        if constexpr (FID == VEGAS_F_USER) obs_val = f.observable();     // after finish(): the user's state is complete
+#endif
+        return fv * wgt;
     }
     return (double)(f.finish(fin0) * jall) * (live ? a.post_scale : 0.0);      // C11: v formed in fp32, then widened
 }
@@ -422,6 +440,8 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     unsigned char* table = smem_rot;                           // rows x 128 B
     unsigned char* hist = smem_rot + (size_t)rows * 128;       // NG x rows x 256 B
     dd* red = reinterpret_cast<dd*>(hist + (size_t)NG * rows * 256);
+    double* obs_sh = reinterpret_cast<double*>(red + 2 * (kRotMaxThreads / 32));   // kRotMaxObsBins doubles
+    (void)obs_sh;
 
     // ---- prologue: the master grid is staged in shared memory with one coalesced pass (in the histogram region,
     // zeroed afterwards), the table is built from the staged copy, the histograms are zeroed
@@ -445,6 +465,7 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
         __syncthreads();
     }
     for (int idx = threadIdx.x; idx < NG * rows * 32; idx += blockDim.x) reinterpret_cast<double*>(hist)[idx] = 0.0;
+    if (FID == VEGAS_F_USER && threadIdx.x < kRotMaxObsBins) obs_sh[threadIdx.x] = 0.0;
     __syncthreads();
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -488,8 +509,18 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     // it -- removed the barrier stalls but cost 30 register moves per iteration and measured 2 % slower.)
     for (uint32_t it = 0; it < n_iter; ++it, q += nthr) {
         uint32_t taddr[NBLK][4];
-        const double v = rot_event<FID, T, DIM>(a, L, ctx, first_lo + q, e_hi, q < count, fin0, taddr);
+        double obs_val = 0.0;
+        const double v = rot_event<FID, T, DIM>(a, L, ctx, first_lo + q, e_hi, q < count, fin0, taddr, obs_val);
         const double v2 = v * v;
+#ifdef VEGAS_USER_INTEGRAND
+        if constexpr (FID == VEGAS_F_USER) {
+            // observable histogram: one shared-memory add of v per event; v = 0 for padded events
+            if (IntegrandU<FID, T, 1>::kObservable && a.n_obs > 0) {
+                const double t = (obs_val - a.obs_lo) * a.obs_inv_width;
+                if (t >= 0.0 && t < (double)a.n_obs && q < count) atomicAdd(obs_sh + (int)t, v);
+            }
+        }
+#endif
         s1 += v;
         s2 += v2;
         if (S > 1 && (pos != 0 || it != 0)) token_wait(my_token);
@@ -578,12 +609,15 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
         if (idx < DIM * nb) part[4 + idx] = own[k] + stage[idx];
     }
     for (int idx = threadIdx.x + 4 * blockDim.x; idx < DIM * nb; idx += blockDim.x) part[4 + idx] += stage[idx];
+    // observable bins: one global add per bin per CTA per launch (the order over CTAs is not fixed: 1e-16 effects)
+    if (FID == VEGAS_F_USER && a.obs != nullptr && (int)threadIdx.x < a.n_obs) atomicAdd(a.obs + threadIdx.x, obs_sh[threadIdx.x]);
 }
 
 #ifndef __CUDACC_RTC__
 inline size_t rot_shared_bytes(int dim, int n_bins, int n_groups) {
     const size_t rows = (size_t)((dim + 3) / 4) * n_bins;
-    return rows * (128 + 256 * (size_t)n_groups) + 2 * sizeof(dd) * (kRotMaxThreads / 32);
+    return rows * (128 + 256 * (size_t)n_groups) + 2 * sizeof(dd) * (kRotMaxThreads / 32) +
+           sizeof(double) * kRotMaxObsBins;
 }
 
 // one translation unit per (FID, T) instantiates DIM = 1..32 (vegas_rot_inst.cu)

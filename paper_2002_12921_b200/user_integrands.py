@@ -56,3 +56,20 @@ struct vegas_user_integrand {
     __device__ double finish(const double* p) { return 1.0; }
 };
 """
+
+# Eq.(3) again, with an observable (PAPER.md:57): the coordinate x_{d-1}, histogrammed with weight f*J during the
+# integration (vegas_set_observable / vegas_get_observable_hist)
+GENZ_PRODUCT_PEAK_WITH_OBSERVABLE = r"""
+struct vegas_user_integrand {
+    double prod, xlast;
+    int d;
+    __device__ void begin(int dim, const double* p) { prod = 1.0; d = dim; xlast = 0.0; }
+    __device__ void dim(int j, double x, const double* p) {
+        const double t = x - p[d + j];
+        prod *= 1.0 / (p[j] * p[j]) + t * t;
+        if (j == d - 1) xlast = x;
+    }
+    __device__ double finish(const double* p) { return 1.0 / prod; }
+    __device__ double observable(const double* p) { return xlast; }
+};
+"""

@@ -182,3 +182,39 @@ def test_user_integrand_shape_limits_and_no_parameters(B):
     assert I == pytest.approx(Iu, rel=1e-12) and s == pytest.approx(su, rel=1e-11)
     np.testing.assert_allclose(H, Hu, rtol=1e-11)
     g.close(); g2.close(); g3.close()
+
+
+def test_observable_histogram_during_integration(B):
+    """PAPER.md:57 ("exporting histograms during integration"): O[k] += f*J for the bin of the user's observable.
+    Expected values: numpy histogram of the oracle's per-event x and f*J (O.sample) over the same events."""
+    dim, nb, n, seed = 7, 40, 200_003, 12
+    p = W.genz_params(dim, 6)
+    edges = W.adapted_edges(dim, nb, seed=9)
+    g = B.VegasGrid(dim, nb)
+    g.set_edges(edges)
+    g.set_user_integrand(U.GENZ_PRODUCT_PEAK_WITH_OBSERVABLE, p)
+    lo, hi, nobs = 0.2, 0.9, 35
+    g.set_observable(lo, hi, nobs)
+    I, s, H, st = g.iterate(n, seed, 4, B.VEGAS_F_USER, 64, chunk_events=70_000)
+    got = g.get_observable_hist()
+    _, _, ox, of = O.sample(edges, seed, 4, 0, n, O.GENZ_PRODUCT_PEAK, p)
+    x = ox[:, dim - 1]
+    k = np.floor((x - lo) / (hi - lo) * nobs)
+    inside = (k >= 0) & (k < nobs)
+    want = np.bincount(k[inside].astype(int), weights=of[inside], minlength=nobs)
+    np.testing.assert_allclose(got, want, rtol=1e-10)
+    assert 0 < want.sum() < of.sum()                           # the window cuts events on both sides
+    oI, oS, oH = O.iterate(edges, n, seed, 4, O.GENZ_PRODUCT_PEAK, p)
+    assert I == pytest.approx(oI, rel=RTOL64) and s == pytest.approx(oS, rel=RTOL64)
+    _hist_ok(H, oH)
+    # it is the LAST iteration's histogram; an integrand without observable() leaves it at zero
+    g.iterate(1000, seed, 5, B.VEGAS_F_USER, 64)
+    assert g.get_observable_hist().sum() < 0.05 * want.sum()
+    g.set_user_integrand(U.GENZ_PRODUCT_PEAK, p)
+    g.iterate(n, seed, 4, B.VEGAS_F_USER, 64)
+    assert np.all(g.get_observable_hist() == 0.0)
+    with pytest.raises(B.VegasError):
+        g.set_observable(1.0, 1.0, 10)
+    with pytest.raises(B.VegasError):
+        g.set_observable(0.0, 1.0, 129)
+    g.close()

@@ -565,3 +565,25 @@ def test_genz_product_peak_at_the_papers_16_dimensions(B):
     exact = W.closed_form(W.GENZ_PRODUCT_PEAK, dim, p)
     assert abs(r["I"] - exact) < 5 * r["sigma"] and r["sigma"] / exact < 1e-2
     g.close()
+
+
+def test_more_than_2_to_the_32_events_in_one_iteration(B):
+    """5e9 events in one iteration (event indices beyond 2^32, launches split there by the fast path): the constant
+    control stays exactly 1, the Gaussian lands on the closed form, and two half-range accumulations equal the whole."""
+    n = 5_000_000_000
+    w = W.config(1)
+    g = _grid(B, w)
+    Ic, sc, _, st = g.iterate(n, 1, 0, B.VEGAS_F_CONST, 64, chunk_events=1_000_000_000)
+    assert st == 0 and abs(Ic - 1.0) <= 1e-12 and sc <= 1e-9                       # reading R9
+    g.set_edges(W.adapted_edges(w.dim, w.n_bins, seed=1))
+    I, s, H, st = g.iterate(n, w.seed, 3, w.integrand_id, 64)
+    assert st == 0 and abs(I - w.closed_form) < 5 * s and s / I < 1e-4
+    g.begin_iteration()
+    g.accumulate(0, n // 2, w.seed, 3, w.integrand_id, 64)
+    g.accumulate(n // 2, n - n // 2, w.seed, 3, w.integrand_id, 64, chunk_events=700_000_000)
+    g.reduce()
+    I2, s2, H2, _ = g.finalize(n)
+    assert I2 == pytest.approx(I, rel=1e-12) and s2 == pytest.approx(s, rel=1e-10)
+    np.testing.assert_allclose(H2, H, rtol=1e-11)
+    np.testing.assert_allclose(H.sum(axis=1), np.full(w.dim, H[0].sum()), rtol=1e-11)   # every dimension sums to S2
+    g.close()

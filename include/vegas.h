@@ -78,7 +78,9 @@ extern "C" {
 
 /* precision of the per-event arithmetic (reading C11): 64 = everything fp64; 32 = grid table, r, x,
  * J, f and v in fp32, v widened to fp64 before S1 += v, S2 += v^2, H += v^2.  Words, bins, the master
- * grid, the sums, the histogram and the refinement are identical / fp64 in both. */
+ * grid, the sums, the histogram and the refinement are identical / fp64 in both.  An integrand whose values leave
+ * the fp32 range (e.g. the un-normalised product peak beyond ~16 dimensions, f up to prod c_j^2) makes the sums
+ * non-finite in fp32: the iteration reports VEGAS_ENUMERIC, nothing is clamped. */
 #define VEGAS_FP64 64
 #define VEGAS_FP32 32
 

@@ -116,7 +116,8 @@ template <typename T, int NCH> struct IntegrandU<VEGAS_F_BW_POLY, T, NCH> {
         poly[i & (NCH - 1)] = t_fma(h, u, poly[i & (NCH - 1)]);
         if (blk == 0 && c.is0[i]) u0 = u;
     }
-    __device__ __forceinline__ T finish(T) const { return chain_sum<NCH, T>(poly) / t_fma(u0, u0, (T)1); }
+    // reciprocal first: it depends on u_0 alone, so it runs beside the polynomial chains; one multiply follows them
+    __device__ __forceinline__ T finish(T) const { return chain_sum<NCH, T>(poly) * ((T)1 / t_fma(u0, u0, (T)1)); }
 };
 
 // ---- table entry and u from the low product word ---------------------------------------------------

@@ -566,6 +566,7 @@ int vegas_accumulate(vegas_grid* g, uint64_t first_event, uint64_t count, uint64
         }
         a.first_event = ra.first_event = first_event + done;
         a.count = ra.count = n_launch;
+        ra.pdl = (done > 0 && !g->profiling) ? 1 : 0;   // chunk k > 0 follows chunk k-1 of this call directly in the stream
         cudaEvent_t e0 = nullptr, e1 = nullptr;
         if (g->profiling) {
             if (g->events_used + 2 > g->events.size()) {

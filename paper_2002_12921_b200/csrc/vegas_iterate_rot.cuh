@@ -186,6 +186,8 @@ struct RotArgs {
     double jac_init;                // start value of the running Jacobian product (a power of two, see RotEntry)
     double fin0;                    // integrand finish constant
     double shift[VEGAS_MAX_DIM], scale[VEGAS_MAX_DIM];
+    int pdl;                        // host side: launch with programmatic stream serialisation (the previous launch in
+                                    // the stream is a chunk of the same accumulate call); the kernel does not read it
     double* obs;                    // USER with an observable: device, [n_obs] sums of v per observable bin, or NULL
     int n_obs;                      // 0 = no observable histogram
     double obs_lo, obs_inv_width;   // bin k = floor((O - obs_lo) * obs_inv_width)
@@ -444,6 +446,10 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     double* obs_sh = reinterpret_cast<double*>(red + 2 * (kRotMaxThreads / 32));   // kRotMaxObsBins doubles
     (void)obs_sh;
 
+    // Programmatic dependent launch between the chunk launches of one accumulate call: the next chunk's CTAs may start
+    // (prologue, event loop) on SMs this grid has already left; they wait for this grid to complete before they touch
+    // the partial rows (griddepcontrol.wait below).  Both instructions are no-ops in an ordinary launch.
+    asm volatile("griddepcontrol.launch_dependents;");
     // ---- prologue: the master grid is staged in shared memory with one coalesced pass (in the histogram region,
     // zeroed afterwards), the table is built from the staged copy, the histograms are zeroed
     {
@@ -542,6 +548,7 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     const int nwarps = (blockDim.x + 31) >> 5;
     if (lane == 0) { red[2 * warp] = t1; red[2 * warp + 1] = t2; }
     double* part = a.partials + (size_t)blockIdx.x * (4 + DIM * nb);
+    asm volatile("griddepcontrol.wait;" ::: "memory");       // the previous chunk's partial rows are complete
     // this thread's words of the CTA's partial row: loaded now, used after the merge (hides the global latency)
     // (the first 4 words per thread; a shape with more than 4 blockDim.x bins reads the rest in the last pass)
     double own[4];

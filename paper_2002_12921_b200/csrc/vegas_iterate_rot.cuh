@@ -449,7 +449,10 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     // Programmatic dependent launch between the chunk launches of one accumulate call: the next chunk's CTAs may start
     // (prologue, event loop) on SMs this grid has already left; they wait for this grid to complete before they touch
     // the partial rows (griddepcontrol.wait below).  Both instructions are no-ops in an ordinary launch.
-    asm volatile("griddepcontrol.launch_dependents;");
+    // Where the trigger sits only matters through the code ptxas schedules around it (measured: cfg5 K1 8.72e10 with
+    // the trigger here against 8.49e10 after the loop; cfg4 5.15e10 here against 5.24e10 there; cfg3 the same).
+    constexpr bool kEarlyTrigger = (FID == VEGAS_F_BW_POLY);
+    if (kEarlyTrigger) asm volatile("griddepcontrol.launch_dependents;");
     // ---- prologue: the master grid is staged in shared memory with one coalesced pass (in the histogram region,
     // zeroed afterwards), the table is built from the staged copy, the histograms are zeroed
     {
@@ -535,6 +538,7 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
         if (S > 1) token_pass(next_token);
     }
     if (S > 1 && pos == 0 && n_iter > 0) token_wait(my_token);   // absorbs the ring's last hand-off
+    if (!kEarlyTrigger) asm volatile("griddepcontrol.launch_dependents;");
 
     // ---- S5: warp shuffle -> CTA -> this CTA's partial (accumulated over the launches of an iteration)
     // (the 32 per-thread sums of a warp are added by a plain fp64 shuffle tree, like the per-thread sums

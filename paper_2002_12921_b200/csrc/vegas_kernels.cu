@@ -12,6 +12,26 @@
 
 namespace vegas {
 
+// The small kernels that follow the fused kernel in the stream (K2, finalize, K3) are launched with programmatic
+// stream serialisation: their launch overlaps the tail of the kernel before them, and they wait here for it to
+// complete before they read anything.  A no-op when the kernel was launched the ordinary way.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t shmem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = shmem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
 template <typename T> struct Vec2;
 template <> struct Vec2<double> { using type = double2; };
 template <> struct Vec2<float> { using type = float2; };
@@ -163,6 +183,7 @@ k_iterate(const IterArgs a, const __grid_constant__ FParams<T> fp) {
 // slices of the CTAs then the slices in order; i < 4: the two double-double sums, one warp each).
 // ---------------------------------------------------------------------------------------------
 __global__ void k_reduce(const double* __restrict__ partials, int n_parts, int n_tot, double* __restrict__ totals) {
+    pdl_wait();
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (blockIdx.x == 0) {
         if (t >= 64) return;
@@ -204,6 +225,7 @@ __global__ void k_reduce(const double* __restrict__ partials, int n_parts, int n
 // S7 (C7): I = S1/n; Var = (S2/n - I^2)/(n-1); sigma = sqrt(max(Var, 0)).
 // result = { I, sigma, status } (status 0 or VEGAS_ENUMERIC as a double).
 __global__ void k_finalize(const double* __restrict__ totals, double n, double* __restrict__ result) {
+    pdl_wait();
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     const dd S1 = fast_two_sum(totals[0], totals[1]);
     const dd S2 = fast_two_sum(totals[2], totals[3]);
@@ -230,6 +252,7 @@ __global__ void __launch_bounds__(VEGAS_MAX_BINS)
 k_refine(double* __restrict__ edges, const double* __restrict__ hist, int n_bins, double alpha, int* status) {
     __shared__ double X[VEGAS_MAX_BINS + 1], m[VEGAS_MAX_BINS], cum[VEGAS_MAX_BINS + 1], s[VEGAS_MAX_BINS];
     __shared__ double total_s;
+    pdl_wait();
     const int j = blockIdx.x, nb = n_bins, i = threadIdx.x;
     double* Xg = edges + (size_t)j * (nb + 1);
     const double* h = hist + (size_t)j * nb;
@@ -464,20 +487,19 @@ size_t iterate_shared_bytes(int dim, int n_bins, int precision, int table_copies
 
 cudaError_t launch_reduce(const double* partials, int n_parts, int n_tot, double* totals, cudaStream_t st) {
     const int threads = 256;                                  // k_reduce: 8 warps = 8 slices of the CTA partials
+    // ordinary launch: launched early, its CTAs would sit beside the fused kernel's on SMs with shared memory to spare
     k_reduce<<<1 + (n_tot - 4 + 31) / 32, threads, 0, st>>>(partials, n_parts, n_tot, totals);
     return cudaGetLastError();
 }
 
 cudaError_t launch_finalize(const double* totals, double n_events, double* result, cudaStream_t st) {
-    k_finalize<<<1, 32, 0, st>>>(totals, n_events, result);
-    return cudaGetLastError();
+    return launch_pdl(k_finalize, dim3(1), dim3(32), 0, st, totals, n_events, result);
 }
 
 cudaError_t launch_refine(double* edges, const double* hist, int dim, int n_bins, double alpha, int* status,
                           cudaStream_t st) {
     const int threads = ((n_bins + 31) / 32) * 32;
-    k_refine<<<dim, threads, 0, st>>>(edges, hist, n_bins, alpha, status);
-    return cudaGetLastError();
+    return launch_pdl(k_refine, dim3(dim), dim3(threads), 0, st, edges, hist, n_bins, alpha, status);
 }
 
 template <typename T>

@@ -423,7 +423,10 @@ template <int FID, typename T, int NBLK>
 static cudaError_t launch_iterate_t(const IterArgs& a, const FParams<T>& fp, int blocks, int threads,
                                     size_t shmem, cudaStream_t st) {
     auto kern = k_iterate<FID, T, NBLK>;
-    static size_t configured = 0;   // per instantiation; attribute is sticky per context
+    static size_t configured_dev[kMaxDevices] = {};   // per instantiation and device: the attribute is per context
+    int dev_ = 0;
+    if (cudaGetDevice(&dev_) != cudaSuccess || dev_ < 0 || dev_ >= kMaxDevices) return cudaErrorInvalidDevice;
+    size_t& configured = configured_dev[dev_];
     if (shmem > configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem);
         if (e != cudaSuccess) return e;
@@ -533,7 +536,10 @@ static cudaError_t launch_debug_rot_t(int fid, const DebugArgs& a, cudaStream_t 
 cudaError_t launch_accumulate_batch(const double* f, const double* J, const int32_t* bins, uint32_t count, int dim,
                                     int n_bins, double* partials, int blocks, cudaStream_t st) {
     const size_t shmem = sizeof(double) * (size_t)dim * n_bins + 2 * sizeof(dd) * 8;
-    static size_t configured = 0;
+    static size_t configured_dev[kMaxDevices] = {};   // per device: the attribute is per context
+    int dev_ = 0;
+    if (cudaGetDevice(&dev_) != cudaSuccess || dev_ < 0 || dev_ >= kMaxDevices) return cudaErrorInvalidDevice;
+    size_t& configured = configured_dev[dev_];
     if (shmem > configured) {
         cudaError_t e = cudaFuncSetAttribute(k_accumulate_batch, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem);
         if (e != cudaSuccess) return e;

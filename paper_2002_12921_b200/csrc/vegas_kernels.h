@@ -14,6 +14,7 @@ namespace vegas {
 #ifndef VEGAS_ITER_MIN_BLOCKS
 #define VEGAS_ITER_MIN_BLOCKS 1
 #endif
+constexpr int kMaxDevices = 64;                          // per-device launch-attribute caches
 constexpr int kIterMaxThreads = VEGAS_ITER_MAX_THREADS;   // __launch_bounds__ of K1
 constexpr int kIterMinBlocks = VEGAS_ITER_MIN_BLOCKS;
 

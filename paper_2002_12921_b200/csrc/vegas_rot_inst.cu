@@ -17,7 +17,10 @@ using RT = float;
 template <int DIM>
 static cudaError_t go(const RotArgs& a, int blocks, int threads, size_t shmem, cudaStream_t st) {
     auto kern = k_iterate_rot<ROT_FID, RT, DIM>;
-    static size_t configured = 0;
+    static size_t configured_dev[kMaxDevices] = {};   // per device: the attribute is per context
+    int dev_ = 0;
+    if (cudaGetDevice(&dev_) != cudaSuccess || dev_ < 0 || dev_ >= kMaxDevices) return cudaErrorInvalidDevice;
+    size_t& configured = configured_dev[dev_];
     if (shmem > configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem);
         if (e != cudaSuccess) return e;

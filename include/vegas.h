@@ -80,7 +80,9 @@ extern "C" {
  * J, f and v in fp32, v widened to fp64 before S1 += v, S2 += v^2, H += v^2.  Words, bins, the master
  * grid, the sums, the histogram and the refinement are identical / fp64 in both.  An integrand whose values leave
  * the fp32 range (e.g. the un-normalised product peak beyond ~16 dimensions, f up to prod c_j^2) makes the sums
- * non-finite in fp32: the iteration reports VEGAS_ENUMERIC, nothing is clamped. */
+ * non-finite in fp32: the iteration reports VEGAS_ENUMERIC, nothing is clamped.  Values of f below the fp32 normal range
+ * (1.2e-38; e.g. exp(-E) with E > 87 everywhere, a narrow Gaussian sampled on an un-adapted grid in many dimensions)
+ * lose digits and then vanish: use VEGAS_FP64 until the grid has adapted. */
 #define VEGAS_FP64 64
 #define VEGAS_FP32 32
 

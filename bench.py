@@ -49,9 +49,9 @@ def n_wide(w):
 
 WIDE_EXTRA_SLOTS = 2.4
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE K1 launch, from the `ncu --set full` captures summarised in
-# profiles/r01_s14_final.md (bench.py never runs under a profiler): (workload, precision) -> bytes per launch
+# profiles/r01_s15_head.md and r01_s14_final.md (bench.py never runs under a profiler): (workload, precision) -> bytes per launch
 NCU_TRAFFIC_BYTES = {("cfg3_gauss_d20", 64): 1.24e6, ("cfg3_gauss_d20", 32): 1.24e6, ("cfg4_genz_pp_d12", 64): 1.48e6,
-                     ("cfg5_bw_poly_d6", 64): 0.40e6}
+                     ("cfg5_bw_poly_d6", 64): 0.41e6}
 
 
 def n_fp(w, precision):

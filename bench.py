@@ -331,7 +331,7 @@ def main():
         clk = float(clocks["sm_mhz"] or sm_max)
         ni, nf = n_issue(w, args.precision), n_fp(w, args.precision)
         k1_s = (k1_ms * 1e-3) / max(1, k1_launches)
-        events_per_launch = (w.n_events if not w.chunk_events else min(w.chunk_events, w.n_events))
+        events_per_launch = w.n_events * k1_steps / max(1, k1_launches)   # the fast path runs the chunk loop in the kernel
         k1_rate = events_per_launch / k1_s                         # events/s of the fused kernel alone
         peak_instr = SM_COUNT * ISSUE_LANES * sm_max * 1e6         # thread-instructions/s at max clock
         roofline = {"bound": "alu", "kernel": "k_iterate",

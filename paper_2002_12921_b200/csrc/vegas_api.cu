@@ -127,7 +127,8 @@ int resolve_launch(const vegas_grid* g, int precision, LaunchShape* out) {
     LaunchShape s;
     s.blocks = g->cfg_blocks > 0 ? g->cfg_blocks : g->sm_count;
     s.threads = g->cfg_threads > 0 ? g->cfg_threads : vegas::kIterMaxThreads;
-    if (s.blocks > kMaxBlocks || s.threads > vegas::kIterMaxThreads || s.threads % 32) return VEGAS_EINVAL;
+    if (s.blocks > kMaxBlocks || s.threads > 1024 || s.threads % 32) return VEGAS_EINVAL;
+    if (s.threads > vegas::kIterMaxThreads) s.threads = vegas::kIterMaxThreads;   // the generic kernel's launch bound
     const int max_ct = precision == VEGAS_FP64 ? 8 : 16;
     double best = 1e300;
     s.ct = s.ch = 0;
@@ -179,7 +180,7 @@ bool use_rot_path(const vegas_grid* g, int fid, int precision) {
     const bool kind = fid == VEGAS_F_CONST || fid == VEGAS_F_GAUSS || fid == VEGAS_F_GENZ_PRODUCT_PEAK ||
                       (fid == VEGAS_F_BW_POLY && g->dim <= vegas::kRotBwMaxDim);
     if (!kind) return false;
-    if (g->cfg_threads > vegas::rot_max_threads(fid)) return false;
+    if (g->cfg_threads > vegas::rot_max_threads(fid, g->dim)) return false;
     return vegas::rot_shared_bytes(g->dim, g->n_bins, 1) <= g->smem_optin;
 }
 
@@ -237,11 +238,11 @@ struct RotShape {
     size_t shmem;
 };
 
-// One CTA per SM, up to 128 registers per thread.  n_groups = histogram copies in the CTA (as many as fit next
-// to the table, a divisor of the warp count W), ring = W / n_groups warps share a copy (1 = no token passing).
-// W: 16 when every warp gets its own copy; otherwise the largest of 15..12 (token barriers 1..15) that keeps more
-// than half of the copies that fit -- measured on B200 (profiles/r01_s13_fast_path.md): 15 warps beat 12 by 4-5 %
-// on cfg2/cfg3 (more warps hide the Philox chain), but 15 warps on 1 copy lose 30 % to 14 warps on 2 (cfg4).
+// One CTA per SM.  n_groups = histogram copies in the CTA (as many as fit next to the table, a divisor of the warp
+// count W), ring = W / n_groups warps share a copy (1 = no token passing).  W is the caller's choice (vegas_set_launch),
+// else: with mbarrier tokens (24-warp kernels) the warp count among the four largest that gives the most copies; with
+// named-barrier tokens (16-warp kernels) 16 when every warp can own a copy, otherwise the largest of 15..12 that keeps
+// more than half of the copies that fit (measured on B200, profiles/r01_s13_fast_path.md).
 static int rot_divisor(int W, int fit) {
     int ng = fit < W ? fit : W;
     while (W % ng) --ng;
@@ -252,16 +253,22 @@ RotShape rot_shape(const vegas_grid* g, int fid) {
     const size_t one = vegas::rot_shared_bytes(g->dim, g->n_bins, 1), base = vegas::rot_shared_bytes(g->dim, g->n_bins, 0);
     int fit = (int)((g->smem_optin - base) / (one - base));
     if (fit < 1) fit = 1;
-    int W;
+    const int wmax = vegas::rot_max_warps(fid, g->dim);
+    const bool mbar = vegas::rot_mbar_tokens(fid, g->dim);
+    int W = wmax;
     if (g->cfg_threads > 0) {
         W = (g->cfg_threads + 31) / 32;
-        if (fit < W && W > vegas::kRotMaxRingWarps) W = vegas::kRotMaxRingWarps;
-    } else if (fit >= vegas::rot_max_threads(fid) / 32) {
-        W = vegas::rot_max_threads(fid) / 32;
-    } else {
-        W = vegas::kRotDefaultWarps;
-        const int wmax = vegas::rot_max_threads(fid) / 32 - 1;
-        for (int w = wmax < vegas::kRotMaxRingWarps ? wmax : vegas::kRotMaxRingWarps; w > vegas::kRotDefaultWarps; --w)
+        if (!mbar && fit < W && W > vegas::kRotMaxNamedRingWarps) W = vegas::kRotMaxNamedRingWarps;
+    } else if (mbar) {
+        int best = 0;
+        for (int w = wmax; w > wmax - 4 && w >= 1; --w) {
+            const int ng = rot_divisor(w, fit);
+            if (ng > best) { best = ng; W = w; }
+        }
+    } else if (fit < wmax) {
+        W = vegas::kRotNamedDefaultWarps < wmax ? vegas::kRotNamedDefaultWarps : wmax;
+        const int top = wmax - 1 < vegas::kRotMaxNamedRingWarps ? wmax - 1 : vegas::kRotMaxNamedRingWarps;
+        for (int w = top; w > W; --w)
             if (2 * rot_divisor(w, fit) > fit) { W = w; break; }
     }
     const int ng = rot_divisor(W, fit);
@@ -554,7 +561,10 @@ int vegas_accumulate(vegas_grid* g, uint64_t first_event, uint64_t count, uint64
         a.log_ch = ilog2(s.ch);
         a.jac_scale = jac_scale_for(g, precision);
     }
-    const uint64_t chunk = chunk_events ? chunk_events : count;
+    // The fast path runs the chunk loop inside the kernel (one launch per accumulate call: the grid finishes a chunk
+    // before it starts the next); the generic kernel is launched once per chunk.
+    const uint64_t chunk = (chunk_events && !rot) ? chunk_events : count;
+    ra.chunk = chunk_events;
     for (uint64_t done = 0, n_launch = 0; done < count; done += n_launch) {
         n_launch = (count - done < chunk) ? count - done : chunk;
         if (rot) {

@@ -170,14 +170,39 @@ __device__ __forceinline__ double lds_f64(uint32_t addr) {
 __device__ __forceinline__ void sts_f64(uint32_t addr, double v) {
     asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory");
 }
-// named barriers 1..15 on 64 threads: the waiting warp syncs, the signalling warp arrives
-__device__ __forceinline__ void token_wait(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
-__device__ __forceinline__ void token_pass(int id) { asm volatile("bar.arrive %0, 64;" ::"r"(id) : "memory"); }
+// Token passing between the warps that share a histogram copy: one mbarrier (arrival count 1) per warp and section
+// in shared memory.  The holder's predecessor arrives (release), the waiting warp spins on try_wait (acquire; the
+// hardware suspends the warp for a bounded time per attempt, so a waiting warp takes no issue slots to speak of).
+// Measured on B200 (profiles/r02_ubench_tokens.md): 78 clk per hand-off against 42 for bar.sync/bar.arrive, but the
+// 16 named barriers of a CTA cap a ring scheme at 15 warps, and more warps are worth more than the 36 clk.
+__device__ __forceinline__ void token_init(uint32_t bar) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar) : "memory");
+}
+// try_wait returns after ~12 clk on sm_100a whether or not the phase has completed (a suspend-time hint, nanosleep
+// between attempts, or an L2 round trip between attempts all measured the same or slower: profiles/r02_k1_steps.md),
+// so this is a spin; a waiting warp issues ~3 instructions per 12 clk.
+__device__ __forceinline__ void token_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "TOK_WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@!p bra TOK_WAIT_%=;\n"
+        "}" ::"r"(bar), "r"(parity) : "memory");
+}
+// named barriers 1..15 on 64 threads (rings of up to 15 warps): the waiting warp syncs, the signalling warp arrives
+__device__ __forceinline__ void token_wait_named(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
+__device__ __forceinline__ void token_pass_named(int id) { asm volatile("bar.arrive %0, 64;" ::"r"(id) : "memory"); }
+__device__ __forceinline__ void token_pass(uint32_t bar) {          // one lane, after __syncwarp()
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
 
 struct RotArgs {
     const double* edges;            // device, [DIM][n_bins+1]
     double* partials;               // device, [gridDim.x][4 + DIM*n_bins]
     unsigned long long first_event, count;
+    unsigned long long chunk;       // events per chunk inside this launch (0 = one chunk): the grid finishes a chunk before
+                                    // it starts the next, per-thread sums are folded into double-double at chunk ends
     uint32_t iteration;
     uint32_t k0[10], k1[10];        // Philox key schedule (C1), built on the host: LOP3 reads it from the constant bank
     int n_bins;
@@ -248,15 +273,38 @@ template <typename T, int NCH> struct IntegrandU<VEGAS_F_USER, T, NCH> {
 };
 #endif
 
-constexpr int kRotMaxThreads = 512;    // one CTA per SM: up to 16 warps, 128 registers per thread
-// BW_POLY keeps 4 coefficients per dimension per lane in registers: 12 warps, up to 168 registers
-// (and so does a user integrand, whose register needs are unknown)
-__host__ __device__ constexpr int rot_max_threads(int fid) {
-    return (fid == VEGAS_F_BW_POLY || fid == VEGAS_F_USER) ? 384 : kRotMaxThreads;
+// One CTA per SM.  Warps per CTA (= __launch_bounds__, i.e. the register budget ptxas works to):
+//  * 4 or 5 Philox blocks (dim >= 13): 24 warps at <= 85 registers.  ptxas fits the event loop of every instantiation
+//    into 72..80 registers without spills, and the per-event latencies (10 dependent Philox rounds, the exp tail, the
+//    histogram round trips) want more warps than the 15 the named-barrier ring allows: cfg3 3.98e10 -> 4.17e10
+//    events/s (profiles/r02_k1_steps.md; 27, 30 and 32 warps measured slower again).  Tokens are mbarriers.
+//  * up to 3 Philox blocks: 16 warps at <= 128 registers, tokens over named barriers (42 clk per hand-off against 78):
+//    most of these shapes give every warp or every other warp its own histogram copy, and measured 3..15 % faster
+//    this way (cfg1, cfg2, cfg5).
+//  * BW_POLY keeps 4 coefficients per dimension per lane in registers, and a user integrand's register needs are
+//    unknown: 12 warps, up to 168 registers.
+#ifndef VEGAS_ROT_WIDE_MIN_DIM
+#define VEGAS_ROT_WIDE_MIN_DIM 13
+#endif
+__host__ __device__ constexpr int rot_max_warps(int fid, int dim) {
+    return (fid == VEGAS_F_BW_POLY || fid == VEGAS_F_USER) ? 12 : (dim >= VEGAS_ROT_WIDE_MIN_DIM ? 24 : 16);
 }
-constexpr int kRotDefaultWarps = 12;
-constexpr int kRotMaxRingWarps = 15;   // token barriers 1..15 (barrier 0 is __syncthreads)
-
+__host__ __device__ constexpr int rot_max_threads(int fid, int dim) { return 32 * rot_max_warps(fid, dim); }
+__host__ __device__ constexpr bool rot_mbar_tokens(int fid, int dim) { return rot_max_warps(fid, dim) > 16; }
+constexpr int kRotMaxNamedRingWarps = 15;   // named barriers 1..15 carry the tokens (barrier 0 is __syncthreads)
+constexpr int kRotNamedDefaultWarps = 12;
+// Sections of a histogram copy: the rows of different Philox blocks are disjoint, so a copy shared by a ring of warps
+// is guarded by one token per section (a run of blocks) and the ring is pipelined: while one warp updates the rows of
+// blocks 3..4 the next already updates those of blocks 0..2.  Needs one token per warp and section: mbarriers only.
+#ifndef VEGAS_ROT_NSEC
+#define VEGAS_ROT_NSEC 2
+#endif
+__host__ __device__ constexpr int rot_sections(int fid, int dim) {
+    return !rot_mbar_tokens(fid, dim) ? 1 : ((dim + 3) / 4 < VEGAS_ROT_NSEC ? (dim + 3) / 4 : VEGAS_ROT_NSEC);
+}
+__host__ __device__ constexpr int rot_section_begin(int nblk, int nsec, int s) { return (s * nblk + nsec - 1) / nsec; }
+constexpr int kRotMaxSections = 8;
+constexpr int kRotScratchWarps = 32;   // sizing of the per-warp scratch (reduction slots, tokens): any CTA has <= 32 warps
 __host__ __device__ constexpr int rot_groups(int r) { return r >= 3 ? 4 : r; }   // dims in block -> lane groups
 
 // byte offset of (slot 0, this lane's copy) inside a table row, for a block with G lane groups;
@@ -315,11 +363,11 @@ __device__ __forceinline__ void philox4x32_10_args(uint32_t c0, uint32_t c1, uin
 }
 
 // S1..S5 for one event: Philox -> split -> table -> u -> integrand; returns v = f J and leaves the
-// table address of every (block, sub-step) in taddr (the histogram update derives its addresses from them).
+// histogram address of every (block, sub-step) in haddr (one LEA from the table address, outside the critical section).
 template <int FID, typename T, int DIM>
 __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, DIM>& L,
                                             const RotCtx<FID, T, (DIM + 3) / 4>& ctx, uint32_t e_lo, uint32_t e_hi,
-                                            bool live, T fin0, uint32_t (&taddr)[(DIM + 3) / 4][4], double& obs_val) {
+                                            bool live, T fin0, uint32_t (&haddr)[(DIM + 3) / 4][4], double& obs_val) {
     using E = RotEntry<T>;
     using T2 = typename E::type;
     constexpr int NBLK = RotLane<T, DIM>::NBLK, R = RotLane<T, DIM>::R, GL = RotLane<T, DIM>::GL;
@@ -354,7 +402,7 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
         T2 ent[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-            taddr[blk][i] = 0;
+            haddr[blk][i] = 0;
             if (i < NSUB) {
                 const bool active = !(last && R == 3) || ((gamma ^ i) < 3);
                 uint32_t b = 0;
@@ -364,8 +412,10 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
                     split_word(w[i], (uint32_t)nb, b, lo[i]);
                     // one multiply-add (ptxas: LEA/IMAD); written in C the compiler folds the shift into a
                     // 64-bit funnel shift of the product plus a mask plus an add
-                    asm("mad.lo.u32 %0, %1, 128, %2;" : "=r"(taddr[blk][i]) : "r"(b), "r"(tblk + (last ? L.txL[i] : L.tx4[i])));
-                    ent[i] = lds_entry<T2>(taddr[blk][i]);
+                    uint32_t taddr;
+                    asm("mad.lo.u32 %0, %1, 128, %2;" : "=r"(taddr) : "r"(b), "r"(tblk + (last ? L.txL[i] : L.tx4[i])));
+                    ent[i] = lds_entry<T2>(taddr);
+                    haddr[blk][i] = 2u * taddr + (last ? L.hcL[i] : L.hc4[i]);
                 }
             }
         }
@@ -392,44 +442,60 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
     return (double)(f.finish(fin0) * jall) * (live ? a.post_scale : 0.0);      // C11: v formed in fp32, then widened
 }
 
-// S6 for one event, by the warp that holds its group's token: H[j][b_j] += v2 with plain loads and
-// stores.  Round i handles sub-step i of every Philox block: within a round the lanes of the warp touch
-// pairwise different words (different rows per block; inside a row each lane has its own column), so the
-// NBLK read-modify-writes of a round are independent and pipeline.  Consecutive rounds can touch the
-// same word from different lanes, hence the __syncwarp() (shared memory is processed in order per warp).
-template <typename T, int DIM>
-__device__ __forceinline__ void rot_hist_update(const RotLane<T, DIM>& L, const uint32_t (&taddr)[(DIM + 3) / 4][4],
-                                                double v2) {
+// S6 for one event and one section (blocks B0..B1-1), by the warp that holds the section's token: H[j][b_j] += v2 with
+// plain loads and stores.  Round i handles sub-step i of every Philox block of the section: within a round the lanes of
+// the warp touch pairwise different words (different rows per block; inside a row each lane has its own column), so
+// the read-modify-writes of a round are independent and pipeline.  Consecutive rounds can touch the same word from
+// different lanes, hence the __syncwarp() (shared memory is processed in order per warp).
+template <typename T, int DIM, int B0, int B1>
+__device__ __forceinline__ void rot_hist_update(const uint32_t (&haddr)[(DIM + 3) / 4][4], int gammaL, double v2) {
     constexpr int NBLK = RotLane<T, DIM>::NBLK, R = RotLane<T, DIM>::R;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        uint32_t addr[NBLK];
         double h[NBLK];
 #pragma unroll
-        for (int blk = 0; blk < NBLK; ++blk) {
+        for (int blk = B0; blk < B1; ++blk) {
             const bool last = (blk == NBLK - 1);
             const int NSUB = last ? ((R == 3) ? 4 : R) : 4;
-            const int gamma = last ? L.gammaL : L.gamma4;
-            const bool active = (i < NSUB) && (!(last && R == 3) || ((gamma ^ i) < 3));
-            if (active) {
-                addr[blk] = 2u * taddr[blk][i] + (last ? L.hcL[i] : L.hc4[i]);
-                h[blk] = lds_f64(addr[blk]);
-            }
+            const bool active = (i < NSUB) && (!(last && R == 3) || ((gammaL ^ i) < 3));
+            if (active) h[blk] = lds_f64(haddr[blk][i]);
         }
 #pragma unroll
-        for (int blk = 0; blk < NBLK; ++blk) {
+        for (int blk = B0; blk < B1; ++blk) {
             const bool last = (blk == NBLK - 1);
             const int NSUB = last ? ((R == 3) ? 4 : R) : 4;
-            const int gamma = last ? L.gammaL : L.gamma4;
-            const bool active = (i < NSUB) && (!(last && R == 3) || ((gamma ^ i) < 3));
-            if (active) sts_f64(addr[blk], h[blk] + v2);
+            const bool active = (i < NSUB) && (!(last && R == 3) || ((gammaL ^ i) < 3));
+            if (active) sts_f64(haddr[blk][i], h[blk] + v2);
         }
         __syncwarp();
     }
 }
 
+// the sections of one event's histogram update, each under its own token
+template <typename T, int DIM, int SEC, int NSEC, bool MBAR>
+__device__ __forceinline__ void rot_hist_sections(const uint32_t (&haddr)[(DIM + 3) / 4][4], int gammaL, double v2, bool ring,
+                                                  bool wait, uint32_t my_tok, uint32_t next_tok, uint32_t tok_stride,
+                                                  uint32_t parity, bool lane0
+                                                  ) {
+    if constexpr (SEC < NSEC) {
+        constexpr int NBLK = (DIM + 3) / 4;
+        if (wait) {
+            if (MBAR) token_wait(my_tok + SEC * tok_stride, parity);
+            else token_wait_named((int)my_tok);
+        }
+        rot_hist_update<T, DIM, rot_section_begin(NBLK, NSEC, SEC), rot_section_begin(NBLK, NSEC, SEC + 1)>(haddr, gammaL, v2);
+        if (MBAR) {
+            if (ring && lane0) token_pass(next_tok + SEC * tok_stride);     // after the __syncwarp() of the last round
+        } else if (ring) {
+            token_pass_named((int)next_tok);
+        }
+        rot_hist_sections<T, DIM, SEC + 1, NSEC, MBAR>(haddr, gammaL, v2, ring, wait, my_tok, next_tok, tok_stride, parity, lane0
+                                                 );
+    }
+}
+
 template <int FID, typename T, int DIM>
-__global__ void __launch_bounds__(rot_max_threads(FID), 1)
+__global__ void __launch_bounds__(rot_max_threads(FID, DIM), 1)
 k_iterate_rot(const __grid_constant__ RotArgs a) {
     using E = RotEntry<T>;
     using T2 = typename E::type;
@@ -443,8 +509,11 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     unsigned char* table = smem_rot;                           // rows x 128 B
     unsigned char* hist = smem_rot + (size_t)rows * 128;       // NG x rows x 256 B
     dd* red = reinterpret_cast<dd*>(hist + (size_t)NG * rows * 256);
-    double* obs_sh = reinterpret_cast<double*>(red + 2 * (kRotMaxThreads / 32));   // kRotMaxObsBins doubles
+    double* obs_sh = reinterpret_cast<double*>(red + 2 * kRotScratchWarps);        // kRotMaxObsBins doubles
     (void)obs_sh;
+    constexpr int NSEC = rot_sections(FID, DIM);
+    constexpr bool MBAR = rot_mbar_tokens(FID, DIM);
+    const uint32_t tok_base = (uint32_t)__cvta_generic_to_shared(obs_sh + kRotMaxObsBins);   // [NSEC][warps] mbarriers
 
     // Programmatic dependent launch between the chunk launches of one accumulate call: the next chunk's CTAs may start
     // (prologue, event loop) on SMs this grid has already left; they wait for this grid to complete before they touch
@@ -476,6 +545,10 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     }
     for (int idx = threadIdx.x; idx < NG * rows * 32; idx += blockDim.x) reinterpret_cast<double*>(hist)[idx] = 0.0;
     if (FID == VEGAS_F_USER && threadIdx.x < kRotMaxObsBins) obs_sh[threadIdx.x] = 0.0;
+    if (MBAR && S > 1 && threadIdx.x < NSEC * (blockDim.x >> 5)) {
+        token_init(tok_base + 8u * threadIdx.x);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
     __syncthreads();
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -500,55 +573,63 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     const T fin0 = (T)a.fin0;
     RotCtx<FID, T, NBLK> ctx;
     ctx.init(a, DIM, L.gamma4, L.gammaL);
-    const int my_token = 1 + warp, next_token = 1 + grp * S + ((pos + 1 == S) ? 0 : pos + 1);
+    const uint32_t tok_stride = 8u * (blockDim.x >> 5);
+    const int next_warp = grp * S + ((pos + 1 == S) ? 0 : pos + 1);
+    const uint32_t my_tok = MBAR ? tok_base + 8u * warp : 1u + (uint32_t)warp;              // mbarrier address / barrier id
+    const uint32_t next_tok = MBAR ? tok_base + 8u * next_warp : 1u + (uint32_t)next_warp;
+    const bool ring = S > 1, lane0 = lane == 0;
 
-    // per-thread sums: a few hundred to a few ten thousand terms per launch, plain fp64; everything above
-    // the thread (warp, CTA, launches, CTAs) is added in double-double
-    double s1 = 0.0, s2 = 0.0;
-    // every warp runs the same number of loop iterations (the ring hands the token on once per iteration);
-    // events past the end of the range contribute v = 0
+    // per-thread sums: plain fp64 inside a chunk (a few hundred terms), folded into double-double at the end of every
+    // chunk; everything above the thread (warp, CTA, launches, CTAs) is added in double-double too
+    dd a1{0.0, 0.0}, a2{0.0, 0.0};
+    // every warp runs the same number of loop iterations (the ring hands the tokens on once per iteration);
+    // events past the end of a chunk contribute v = 0
     // The host never lets a launch cross a multiple of 2^32 in the global event index nor exceed 2^32 - 2^20
     // events (vegas_accumulate), so the high counter word of C2 is uniform, the low one is first_lo + q without a
-    // carry, and q fits 32 bits even in the padded last pass.
+    // carry, and q fits 32 bits even in the padded last pass of the last chunk.
     const uint32_t nthr = gridDim.x * blockDim.x;
     const uint32_t count = (uint32_t)a.count;
-    const uint32_t n_iter = (uint32_t)((a.count + nthr - 1) / nthr);
+    const uint32_t chunk = (a.chunk == 0 || a.chunk > a.count) ? count : (uint32_t)a.chunk;
     const uint32_t e_hi = (uint32_t)(a.first_event >> 32), first_lo = (uint32_t)a.first_event;
-    uint32_t q = blockIdx.x * blockDim.x + threadIdx.x;
-    // (A software-pipelined variant -- histogram update of iteration it-1 after the per-event work of iteration
-    // it -- removed the barrier stalls but cost 30 register moves per iteration and measured 2 % slower.)
-    for (uint32_t it = 0; it < n_iter; ++it, q += nthr) {
-        uint32_t taddr[NBLK][4];
-        double obs_val = 0.0;
-        const double v = rot_event<FID, T, DIM>(a, L, ctx, first_lo + q, e_hi, q < count, fin0, taddr, obs_val);
-        const double v2 = v * v;
+    const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
+    uint32_t tick = (pos == 0) ? 1u : 0u;      // parity of the token waits: pos 0 skips the wait of its first iteration
+    bool first = (pos == 0);
+    for (uint32_t c0 = 0, c_end = 0; c0 < count; c0 = c_end) {
+        c_end = (count - c0 < chunk) ? count : c0 + chunk;                     // this chunk: events [c0, c_end) of the launch
+        const uint32_t n_iter = (c_end - c0 + nthr - 1) / nthr;
+        double s1 = 0.0, s2 = 0.0;
+        uint32_t q = c0 + tid;
+        for (uint32_t it = 0; it < n_iter; ++it, q += nthr, ++tick) {
+            uint32_t haddr[NBLK][4];
+            double obs_val = 0.0;
+            const bool live = q < c_end;
+            const double v = rot_event<FID, T, DIM>(a, L, ctx, first_lo + q, e_hi, live, fin0, haddr, obs_val);
+            const double v2 = v * v;
 #ifdef VEGAS_USER_INTEGRAND
-        if constexpr (FID == VEGAS_F_USER) {
-            // observable histogram: one shared-memory add of v per event; v = 0 for padded events
-            if (IntegrandU<FID, T, 1>::kObservable && a.n_obs > 0) {
-                const double t = (obs_val - a.obs_lo) * a.obs_inv_width;
-                if (t >= 0.0 && t < (double)a.n_obs && q < count) atomicAdd(obs_sh + (int)t, v);
+            if constexpr (FID == VEGAS_F_USER) {
+                // observable histogram: one shared-memory add of v per event; v = 0 for padded events
+                if (IntegrandU<FID, T, 1>::kObservable && a.n_obs > 0) {
+                    const double t = (obs_val - a.obs_lo) * a.obs_inv_width;
+                    if (t >= 0.0 && t < (double)a.n_obs && live) atomicAdd(obs_sh + (int)t, v);
+                }
             }
-        }
 #endif
-        s1 += v;
-        s2 += v2;
-        if (S > 1 && (pos != 0 || it != 0)) token_wait(my_token);
-        rot_hist_update<T, DIM>(L, taddr, v2);
-        if (S > 1) token_pass(next_token);
+            s1 += v;
+            s2 += v2;
+            rot_hist_sections<T, DIM, 0, NSEC, MBAR>(haddr, L.gammaL, v2, ring, ring && !first, my_tok, next_tok, tok_stride,
+                                               tick & 1u, lane0
+                                               );
+            first = false;
+        }
+        a1 = dd_add(a1, dd{s1, 0.0});
+        a2 = dd_add(a2, dd{s2, 0.0});
     }
-    if (S > 1 && pos == 0 && n_iter > 0) token_wait(my_token);   // absorbs the ring's last hand-off
+    if (!MBAR && ring && pos == 0 && !first) token_wait_named((int)my_tok);   // absorbs the ring's last hand-off
     if (!kEarlyTrigger) asm volatile("griddepcontrol.launch_dependents;");
 
-    // ---- S5: warp shuffle -> CTA -> this CTA's partial (accumulated over the launches of an iteration)
-    // (the 32 per-thread sums of a warp are added by a plain fp64 shuffle tree, like the per-thread sums
-    // themselves; warps, launches and CTAs -- where thousands of terms meet -- are added in double-double)
-#pragma unroll
-    for (int m = 16; m > 0; m >>= 1) {
-        s1 += __shfl_xor_sync(0xffffffffu, s1, m);
-        s2 += __shfl_xor_sync(0xffffffffu, s2, m);
-    }
-    dd t1{s1, 0.0}, t2{s2, 0.0};
+    // ---- S5: warp shuffle -> CTA -> this CTA's partial (accumulated over the launches of an iteration), all in
+    // double-double
+    dd t1 = dd_warp_sum(a1), t2 = dd_warp_sum(a2);
     const int nwarps = (blockDim.x + 31) >> 5;
     if (lane == 0) { red[2 * warp] = t1; red[2 * warp + 1] = t2; }
     double* part = a.partials + (size_t)blockIdx.x * (4 + DIM * nb);
@@ -628,8 +709,8 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
 #ifndef __CUDACC_RTC__
 inline size_t rot_shared_bytes(int dim, int n_bins, int n_groups) {
     const size_t rows = (size_t)((dim + 3) / 4) * n_bins;
-    return rows * (128 + 256 * (size_t)n_groups) + 2 * sizeof(dd) * (kRotMaxThreads / 32) +
-           sizeof(double) * kRotMaxObsBins;
+    return rows * (128 + 256 * (size_t)n_groups) + 2 * sizeof(dd) * kRotScratchWarps +
+           sizeof(double) * kRotMaxObsBins + 8 * (size_t)kRotMaxSections * kRotScratchWarps;
 }
 
 // one translation unit per (FID, T) instantiates DIM = 1..32 (vegas_rot_inst.cu)

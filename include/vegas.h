@@ -78,11 +78,12 @@ extern "C" {
 
 /* precision of the per-event arithmetic (reading C11): 64 = everything fp64; 32 = grid table, r, x,
  * J, f and v in fp32, v widened to fp64 before S1 += v, S2 += v^2, H += v^2.  Words, bins, the master
- * grid, the sums, the histogram and the refinement are identical / fp64 in both.  An integrand whose values leave
- * the fp32 range (e.g. the un-normalised product peak beyond ~16 dimensions, f up to prod c_j^2) makes the sums
- * non-finite in fp32: the iteration reports VEGAS_ENUMERIC, nothing is clamped.  Values of f below the fp32 normal range
- * (1.2e-38; e.g. exp(-E) with E > 87 everywhere, a narrow Gaussian sampled on an un-adapted grid in many dimensions)
- * lose digits and then vanish: use VEGAS_FP64 until the grid has adapted. */
+ * grid, the sums, the histogram and the refinement are identical / fp64 in both.  What must fit the fp32 range is
+ * v = f J / C with a per-integrand constant C applied after the widening (GAUSS: ln N is folded into the exponent, so
+ * f = N exp(-E) is formed in one piece; product peak: the product is formed in four partial quotients, prod c_j is C);
+ * intermediate factors do not have to.  Where v itself exceeds 3.4e38 the sums become non-finite and the iteration
+ * reports VEGAS_ENUMERIC, nothing is clamped; where it falls below 1.2e-38 it loses digits and then vanishes (the
+ * estimate stays finite and is biased low: an un-adapted narrow Gaussian in many dimensions): use VEGAS_FP64 there. */
 #define VEGAS_FP64 64
 #define VEGAS_FP32 32
 

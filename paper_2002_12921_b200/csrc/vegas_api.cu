@@ -186,17 +186,26 @@ bool use_rot_path(const vegas_grid* g, int fid, int precision) {
 
 // shift_j, scale_j, post_scale, fin0 of the affine pre-composition (see vegas_iterate_rot.cuh)
 void rot_constants(const vegas_grid* g, int fid, int precision, double* shift, double* scale, double* post_scale,
-                   double* fin0, double* jac_init, double* fpar) {
+                   double* fin0, double* fin1, double* jac_init, double* fpar) {
     const int dim = g->dim;
     const double nb = (double)g->n_bins;
     *post_scale = 1.0;
     *fin0 = 0.0;
+    *fin1 = 0.0;
     for (int j = 0; j < VEGAS_MAX_DIM; ++j) { shift[j] = 0.0; scale[j] = nb; }
     if (fid == VEGAS_F_GAUSS) {
         const double a = g->user[fid][0];
         for (int j = 0; j < dim; ++j) shift[j] = 0.5;
         *fin0 = 1.0 / ((nb * a) * (nb * a));
         *post_scale = g->derived[fid][0];                       // (a sqrt(pi))^-d; prod B_j is the Jacobian
+        if (precision == VEGAS_FP32) {
+            // fp32 (C11): ln N goes into the exponent (IntegrandU<GAUSS>::finish); what its rounding to fp32 leaves
+            // of N, a factor 1 +- 2e-6, stays here and is applied after the widening
+            const double ln_n = -(double)dim * std::log(a * std::sqrt(3.14159265358979323846));
+            const float ln_n32 = (float)ln_n;
+            *fin1 = (double)ln_n32;
+            *post_scale = std::exp(ln_n - (double)ln_n32);
+        }
     } else if (fid == VEGAS_F_GENZ_PRODUCT_PEAK) {
         double ps = 1.0;
         for (int j = 0; j < dim; ++j) {
@@ -206,6 +215,14 @@ void rot_constants(const vegas_grid* g, int fid, int precision, double* shift, d
             ps *= c * nb;                                        // f J = prod(c_j nb) prod B_j / prod(1+u_j^2)
         }
         *post_scale = ps;
+        if (precision == VEGAS_FP32) {
+            // fp32 (C11): n_bins^d is shared out over the four chains (IntegrandU<GENZ>::value), prod c_j stays here
+            const float q32 = (float)std::pow(nb, 0.25 * dim);
+            double pc = 1.0;
+            for (int j = 0; j < dim; ++j) pc *= g->user[fid][j];
+            *fin1 = (double)q32;
+            *post_scale = pc * std::exp((double)dim * std::log(nb) - 4.0 * std::log((double)q32));
+        }
     } else if (fid == VEGAS_F_USER) {
         double ps = 1.0;                                         // u_j = x_j; J = prod nb Delta_j = nb^d prod B_j 2^32
         for (int j = 0; j < dim; ++j) { scale[j] = 1.0; ps *= nb; }
@@ -540,7 +557,7 @@ int vegas_accumulate(vegas_grid* g, uint64_t first_event, uint64_t count, uint64
         ra.n_bins = g->n_bins;
         ra.n_groups = rs.n_groups;
         ra.ring = rs.ring;
-        rot_constants(g, fid, precision, ra.shift, ra.scale, &ra.post_scale, &ra.fin0, &ra.jac_init, ra.fpar);
+        rot_constants(g, fid, precision, ra.shift, ra.scale, &ra.post_scale, &ra.fin0, &ra.fin1, &ra.jac_init, ra.fpar);
         if (fid == VEGAS_F_USER && g->n_obs > 0) {
             ra.obs = g->d_obs;
             ra.n_obs = g->n_obs;
@@ -560,6 +577,10 @@ int vegas_accumulate(vegas_grid* g, uint64_t first_event, uint64_t count, uint64
         a.log_ct = ilog2(s.ct);
         a.log_ch = ilog2(s.ch);
         a.jac_scale = jac_scale_for(g, precision);
+        if (fid != VEGAS_F_BW_POLY) {
+            double fpar_unused[vegas::kRotParams];
+            rot_constants(g, fid, precision, a.shift, a.scale, &a.post_scale, &a.fin0, &a.fin1, &a.jac_init, fpar_unused);
+        }
     }
     // The fast path runs the chunk loop inside the kernel (one launch per accumulate call: the grid finishes a chunk
     // before it starts the next); the generic kernel is launched once per chunk.
@@ -768,8 +789,9 @@ int vegas_debug_sample(vegas_grid* g, uint64_t first_event, uint32_t count, uint
     a.bins = (int32_t*)base;                   base += align_up(per_dim * 4);
     a.x = (double*)base;                       base += align_up(per_dim * 8);
     a.fJ = (double*)base;
-    const bool rot = use_rot_path(g, fid, precision);
-    if (rot) rot_constants(g, fid, precision, a.shift, a.scale, &a.post_scale, &a.fin0, &a.jac_init, a.fpar);
+    // both K1 kernels form u_j, f and v through the affine map for every integrand but BW_POLY beyond the fast path
+    const bool rot = fid != VEGAS_F_BW_POLY || use_rot_path(g, fid, precision);
+    if (rot) rot_constants(g, fid, precision, a.shift, a.scale, &a.post_scale, &a.fin0, &a.fin1, &a.jac_init, a.fpar);
     CUDA_TRY(g, vegas::launch_debug(fid, precision, rot, a, g->derived[fid], st));
     g->launches++;
     if (words) CUDA_TRY(g, cudaMemcpyAsync(words, a.words, per_dim * 4, cudaMemcpyDeviceToHost, st));

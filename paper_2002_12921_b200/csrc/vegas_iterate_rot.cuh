@@ -52,7 +52,10 @@ template <int FID, typename T, int NBLK> struct RotCtx {
 // 15-warp CTA is tight and the extra accumulators cost more than the shorter chains give (cfg3: 3.85e10 events/s
 // with 1 chain and Horner exp, 3.76e10 with 2 chains, 3.68e10 with 4 chains and Estrin; cfg4: 4.93e10 -> 5.24e10
 // and cfg2: 8.03e10 -> 8.10e10 with 4)
-__host__ __device__ constexpr int rot_chains(int dim) { return dim > 12 ? 1 : 4; }
+// (fp32 product peak: always 4, so that no partial product of (1 + u^2) leaves the fp32 range, see its value())
+__host__ __device__ constexpr int rot_chains(int dim, int fid = -1, bool fp32 = false) {
+    return (fp32 && fid == VEGAS_F_GENZ_PRODUCT_PEAK) ? 4 : (dim > 12 ? 1 : 4);
+}
 template <int NCH, typename T> __device__ __forceinline__ T chain_sum(const T (&s)[NCH]) {
     if (NCH == 4) return (s[0] + s[NCH > 1 ? 1 : 0]) + (s[NCH > 2 ? 2 : 0] + s[NCH > 3 ? 3 : 0]);
     if (NCH == 2) return s[0] + s[NCH > 1 ? 1 : 0];
@@ -68,7 +71,8 @@ template <int FID, typename T, int NCH> struct IntegrandU;
 template <typename T, int NCH> struct IntegrandU<VEGAS_F_CONST, T, NCH> {
     template <class C> __device__ __forceinline__ void begin(const C&) {}
     template <class C> __device__ __forceinline__ void dim(T, int, int, const C&) {}
-    __device__ __forceinline__ T finish(T) const { return (T)1; }
+    __device__ __forceinline__ T finish(T, T) const { return (T)1; }
+    __device__ __forceinline__ T value(const T (&jac)[NCH], T, T) const { return chain_prod<NCH, T>(jac); }
 };
 // Every integrand keeps NCH partial accumulators, picked by the sub-step i (NCH independent chains instead of one
 // chain of d links: a dependent DFMA issues every ~14 clk on sm_100, r01_s7_ubench_pipes.md), combined in finish().
@@ -81,9 +85,14 @@ template <typename T, int NCH> struct IntegrandU<VEGAS_F_GAUSS, T, NCH> {   // P
     template <class C> __device__ __forceinline__ void dim(T u, int, int i, const C&) {
         s[i & (NCH - 1)] = t_fma(u, u, s[i & (NCH - 1)]);
     }
-    __device__ __forceinline__ T finish(T fin0) const {        // fin0 = 1/(n_bins a)^2
+    // fin0 = 1/(n_bins a)^2.  fp32: fin1 = ln N (the rest of N, a factor 1 +- 2e-6, sits in post_scale), so that
+    // f = N exp(-E) leaves the fp32 range where N exp(-E) does, not already where exp(-E) does (34 decades earlier
+    // for cfg3's N = 1.07e15).
+    __device__ __forceinline__ T finish(T fin0, T fin1) const {
+        if (sizeof(T) == 4) return ExpFast<T, (NCH > 1)>::f(t_fma(-chain_sum<NCH, T>(s), fin0, fin1));
         return ExpFast<T, (NCH > 1)>::f(-chain_sum<NCH, T>(s) * fin0);
     }
+    __device__ __forceinline__ T value(const T (&jac)[NCH], T fin0, T fin1) const { return finish(fin0, fin1) * chain_prod<NCH, T>(jac); }
 };
 template <typename T, int NCH> struct IntegrandU<VEGAS_F_GENZ_PRODUCT_PEAK, T, NCH> {   // PAPER.md:74 Eq.(3); u = c_j (x - w_j)
     T prod[NCH];
@@ -94,7 +103,19 @@ template <typename T, int NCH> struct IntegrandU<VEGAS_F_GENZ_PRODUCT_PEAK, T, N
     template <class C> __device__ __forceinline__ void dim(T u, int, int i, const C&) {
         prod[i & (NCH - 1)] *= t_fma(u, u, (T)1);
     }
-    __device__ __forceinline__ T finish(T) const { return (T)1 / chain_prod<NCH, T>(prod); }
+    __device__ __forceinline__ T finish(T, T) const { return (T)1 / chain_prod<NCH, T>(prod); }
+    // fp32 (C11): f J = prod_j c_j n_bins Delta_j c_j / (1 + u_j^2) is O(I), but prod (1 + u^2) and prod Delta alone
+    // leave the fp32 range in many dimensions.  Each of the 4 chains (<= 8 dimensions) is divided on its own and takes
+    // a quarter of n_bins^d: fin1 = n_bins^(d/4) (what rounding leaves of n_bins^d / fin1^4 sits in post_scale).
+    __device__ __forceinline__ T value(const T (&jac)[NCH], T fin0, T fin1) const {
+        if (sizeof(T) == 4 && NCH == 4) {
+            T r[NCH];
+#pragma unroll
+            for (int c = 0; c < NCH; ++c) r[c] = (jac[c] * fin1) / prod[c];
+            return chain_prod<NCH, T>(r);
+        }
+        return finish(fin0, fin1) * chain_prod<NCH, T>(jac);
+    }
 };
 // BW_POLY (BASELINE.json:configs[4], readings R11, R12): u_0 = (s(x_0) - M^2)/(M Gamma), u_j = x_j for j >= 1;
 // f = [1/(1 + u_0^2)] * [sum_j a_j0 + sum_j u_j (a_j1 + u_j (a_j2 + u_j (a_j3 + u_j a_j4)))].
@@ -117,7 +138,8 @@ template <typename T, int NCH> struct IntegrandU<VEGAS_F_BW_POLY, T, NCH> {
         if (blk == 0 && c.is0[i]) u0 = u;
     }
     // reciprocal first: it depends on u_0 alone, so it runs beside the polynomial chains; one multiply follows them
-    __device__ __forceinline__ T finish(T) const { return chain_sum<NCH, T>(poly) * ((T)1 / t_fma(u0, u0, (T)1)); }
+    __device__ __forceinline__ T finish(T, T) const { return chain_sum<NCH, T>(poly) * ((T)1 / t_fma(u0, u0, (T)1)); }
+    __device__ __forceinline__ T value(const T (&jac)[NCH], T fin0, T fin1) const { return finish(fin0, fin1) * chain_prod<NCH, T>(jac); }
 };
 
 // ---- table entry and u from the low product word ---------------------------------------------------
@@ -209,7 +231,7 @@ struct RotArgs {
     int n_groups, ring;             // histogram copies in the CTA; warps per copy (blockDim = 32 n_groups ring)
     double post_scale;              // v = f_u * jac * post_scale
     double jac_init;                // start value of the running Jacobian product (a power of two, see RotEntry)
-    double fin0;                    // integrand finish constant
+    double fin0, fin1;              // integrand finish constants (IntegrandU::finish / value)
     double shift[VEGAS_MAX_DIM], scale[VEGAS_MAX_DIM];
     int pdl;                        // host side: launch with programmatic stream serialisation (the previous launch in
                                     // the stream is a chunk of the same accumulate call); the kernel does not read it
@@ -269,7 +291,8 @@ template <typename T, int NCH> struct IntegrandU<VEGAS_F_USER, T, NCH> {
     template <class C> __device__ __forceinline__ void dim(T u, int blk, int i, const C& c) {
         f.dim(4 * blk + ((blk == c.nblk - 1 ? c.gammaL : c.gamma4) ^ i), (double)u, p);
     }
-    __device__ __forceinline__ T finish(T) { return (T)f.finish(p); }
+    __device__ __forceinline__ T finish(T, T) { return (T)f.finish(p); }
+    __device__ __forceinline__ T value(const T (&jac)[NCH], T fin0, T fin1) { return finish(fin0, fin1) * chain_prod<NCH, T>(jac); }
 };
 #endif
 
@@ -367,12 +390,12 @@ __device__ __forceinline__ void philox4x32_10_args(uint32_t c0, uint32_t c1, uin
 template <int FID, typename T, int DIM>
 __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, DIM>& L,
                                             const RotCtx<FID, T, (DIM + 3) / 4>& ctx, uint32_t e_lo, uint32_t e_hi,
-                                            bool live, T fin0, uint32_t (&haddr)[(DIM + 3) / 4][4], double& obs_val) {
+                                            bool live, T fin0, T fin1, uint32_t (&haddr)[(DIM + 3) / 4][4], double& obs_val) {
     using E = RotEntry<T>;
     using T2 = typename E::type;
     constexpr int NBLK = RotLane<T, DIM>::NBLK, R = RotLane<T, DIM>::R, GL = RotLane<T, DIM>::GL;
     const int nb = a.n_bins;
-    constexpr int NCH = rot_chains(DIM);
+    constexpr int NCH = rot_chains(DIM, FID, sizeof(T) == 4);
     IntegrandU<FID, T, NCH> f;
     f.begin(ctx);
     T jac[NCH];                                          // partial Jacobian products (see IntegrandU)
@@ -433,13 +456,14 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
     const T jall = chain_prod<NCH, T>(jac);
     if (sizeof(T) == 8) {
         const double wgt = live ? (double)jall * a.post_scale : 0.0;
-        const double fv = (double)f.finish(fin0);
+        const double fv = (double)f.finish(fin0, fin1);
 #ifdef VEGAS_USER_INTEGRAND
         if constexpr (FID == VEGAS_F_USER) obs_val = f.observable();     // after finish(): the user's state is complete
 #endif
         return fv * wgt;
     }
-    return (double)(f.finish(fin0) * jall) * (live ? a.post_scale : 0.0);      // C11: v formed in fp32, then widened
+    (void)jall;
+    return (double)f.value(jac, fin0, fin1) * (live ? a.post_scale : 0.0);     // C11: v formed in fp32, then widened
 }
 
 // S6 for one event and one section (blocks B0..B1-1), by the warp that holds the section's token: H[j][b_j] += v2 with
@@ -570,7 +594,7 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     }
     L.gamma4 = rot_gamma<4>(lane);
     L.gammaL = rot_gamma<GL>(lane);
-    const T fin0 = (T)a.fin0;
+    const T fin0 = (T)a.fin0, fin1 = (T)a.fin1;
     RotCtx<FID, T, NBLK> ctx;
     ctx.init(a, DIM, L.gamma4, L.gammaL);
     const uint32_t tok_stride = 8u * (blockDim.x >> 5);
@@ -603,7 +627,7 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
             uint32_t haddr[NBLK][4];
             double obs_val = 0.0;
             const bool live = q < c_end;
-            const double v = rot_event<FID, T, DIM>(a, L, ctx, first_lo + q, e_hi, live, fin0, haddr, obs_val);
+            const double v = rot_event<FID, T, DIM>(a, L, ctx, first_lo + q, e_hi, live, fin0, fin1, haddr, obs_val);
             const double v2 = v * v;
 #ifdef VEGAS_USER_INTEGRAND
             if constexpr (FID == VEGAS_F_USER) {

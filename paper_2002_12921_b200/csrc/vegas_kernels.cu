@@ -76,10 +76,15 @@ template <> struct MapConst<float> {
 // NBLK = ceil(dim/4) Philox blocks per event, compile time so that the packed bin indices
 // (one byte per dimension) live in registers.
 // ---------------------------------------------------------------------------------------------
+// CONST, GAUSS and the product peak go through the affine variable u_j = scale_j (x_j - shift_j) exactly as on the
+// fast path (table entry (A, B) with u = A + B w, IntegrandU, value()); BW_POLY (dim > 8 only gets here) keeps the
+// plain map x_j = X_b + Delta r and its parameters in the constant bank.
 template <int FID, typename T, int NBLK>
 __global__ void __launch_bounds__(kIterMaxThreads, kIterMinBlocks)
-k_iterate(const IterArgs a, const __grid_constant__ FParams<T> fp) {
+k_iterate(const __grid_constant__ IterArgs a, const __grid_constant__ FParams<T> fp) {
     using T2 = typename Vec2<T>::type;
+    constexpr bool AFF = (FID != VEGAS_F_BW_POLY);
+    constexpr int NCH = rot_chains(VEGAS_MAX_DIM, FID, sizeof(T) == 4);        // 1, or 4 for the fp32 product peak
     extern __shared__ __align__(16) unsigned char smem[];
     const int dim = a.dim, nb = a.n_bins, nent = dim * nb;
     const int ct = 1 << a.log_ct, ch = 1 << a.log_ch;
@@ -91,7 +96,7 @@ k_iterate(const IterArgs a, const __grid_constant__ FParams<T> fp) {
     for (int i = threadIdx.x; i < nent; i += blockDim.x) {
         const int j = i / nb, b = i - j * nb;
         const double* X = a.edges + (size_t)j * (nb + 1);
-        const T2 ent = make_entry<T>(X[b], X[b + 1], nb);
+        const T2 ent = AFF ? RotEntry<T>::make(X[b], X[b + 1], a.shift[j], a.scale[j]) : make_entry<T>(X[b], X[b + 1], nb);
         for (int c = 0; c < ct; ++c) table[i * ct + c] = ent;
     }
     for (int i = threadIdx.x; i < nent * ch; i += blockDim.x) hist[i] = 0.0;
@@ -113,7 +118,12 @@ k_iterate(const IterArgs a, const __grid_constant__ FParams<T> fp) {
         const uint32_t e_lo = (uint32_t)e, e_hi = (uint32_t)(e >> 32);
         Integrand<FID, T> f;
         f.begin();
-        T jac = (T)1;
+        IntegrandU<AFF ? FID : VEGAS_F_CONST, T, NCH> fu;
+        const RotCtx<AFF ? FID : VEGAS_F_CONST, T, 1> ctx{};
+        fu.begin(ctx);
+        T jac[NCH];
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) jac[c] = (c || !AFF) ? (T)1 : (T)a.jac_init;
         uint32_t packed[NBLK];
 #pragma unroll
         for (int blk = 0; blk < NBLK; ++blk) {
@@ -127,15 +137,18 @@ k_iterate(const IterArgs a, const __grid_constant__ FParams<T> fp) {
                     uint32_t b, lo;
                     split_word(w[i], (uint32_t)nb, b, lo);
                     const T2 ent = *reinterpret_cast<const T2*>(tlane + ((uint32_t)(j * nb) + b) * tstride);
-                    const T x = mapc.x(ent, lo);
-                    jac *= ent.y;
-                    f.dim(j, x, fp);
+                    jac[i & (NCH - 1)] *= ent.y;
+                    if (AFF) fu.dim(RotEntry<T>::u(ent, lo), 0, i, ctx);
+                    else f.dim(j, mapc.x(ent, lo), fp);
                     pk |= b << (8 * i);
                 }
             }
             packed[blk] = pk;
         }
-        const double v = (double)(f.finish(fp) * jac) * jac_scale;
+        double v;
+        if (!AFF) v = (double)(f.finish(fp) * jac[0]) * jac_scale;
+        else if (sizeof(T) == 8) v = (double)fu.finish((T)a.fin0, (T)a.fin1) * ((double)chain_prod<NCH, T>(jac) * a.post_scale);
+        else v = (double)fu.value(jac, (T)a.fin0, (T)a.fin1) * a.post_scale;          // C11: v formed in fp32, then widened
         const double v2 = v * v;
         kahan_add(s1, c1, v);
         kahan_add(s2, c2, v2);
@@ -393,9 +406,11 @@ __global__ void k_debug_rot(const __grid_constant__ DebugArgs a) {
     const PhiloxKey ks = philox_key_schedule(a.key0, a.key1);
     RotCtx<FID, T, kRotBwMaxDim / 4> ctx;      // lane 0's view: gamma = 0, dimension j at (j >> 2, j & 3)
     ctx.init(a, dim, 0, 0);
-    IntegrandU<FID, T, 1> f;
+    constexpr int NCH = rot_chains(VEGAS_MAX_DIM, FID, sizeof(T) == 4);     // 1, or 4 for the fp32 product peak
+    IntegrandU<FID, T, NCH> f;
     f.begin(ctx);
-    T jac = (T)a.jac_init;
+    T jac[NCH];
+    for (int c = 0; c < NCH; ++c) jac[c] = c ? (T)1 : (T)a.jac_init;
     uint32_t w[4] = {0, 0, 0, 0};
     for (int j = 0; j < dim; ++j) {
         if ((j & 3) == 0) philox4x32_10((uint32_t)(j >> 2), a.iteration, (uint32_t)e, (uint32_t)(e >> 32), ks, w);
@@ -404,7 +419,7 @@ __global__ void k_debug_rot(const __grid_constant__ DebugArgs a) {
         split_word(word, (uint32_t)nb, b, lo);
         const double* X = a.edges + (size_t)j * (nb + 1);
         const typename E::type ent = E::make(X[b], X[b + 1], a.shift[j], a.scale[j]);
-        jac *= ent.y;
+        jac[j & (NCH - 1)] *= ent.y;
         f.dim(E::u(ent, lo), FID == VEGAS_F_BW_POLY ? (j >> 2) : 0, j & 3, ctx);
         a.words[(size_t)q * dim + j] = word;
         a.bins[(size_t)q * dim + j] = (int32_t)b;
@@ -413,7 +428,7 @@ __global__ void k_debug_rot(const __grid_constant__ DebugArgs a) {
                                                                     offset_f32_scaled(lo, 5.9604644775390625e-08f, 2.98023223876953125e-08f),
                                                                     (float)X[b]);
     }
-    a.fJ[q] = (double)(f.finish((T)a.fin0) * jac) * a.post_scale;
+    a.fJ[q] = (double)f.value(jac, (T)a.fin0, (T)a.fin1) * a.post_scale;
 }
 
 // =============================================================================================

@@ -27,7 +27,11 @@ struct IterArgs {
     uint32_t iteration;
     int dim, n_bins;
     int log_ct, log_ch;             // log2 of the table / histogram copy counts
-    double jac_scale;               // fp64: n_bins^dim (the table holds Delta); fp32: 1
+    double jac_scale;               // BW_POLY: fp64: n_bins^dim (the table holds Delta); fp32: 1
+    // CONST, GAUSS, GENZ: the affine map and constants of the fast path (vegas_iterate_rot.cuh: RotEntry, IntegrandU),
+    // so that both kernels form u_j, f and v by the same arithmetic (C11: same fp32 accuracy and range)
+    double post_scale, fin0, fin1, jac_init;
+    double shift[VEGAS_MAX_DIM], scale[VEGAS_MAX_DIM];
 };
 
 struct DebugArgs {
@@ -42,7 +46,7 @@ struct DebugArgs {
     double* x;
     double* fJ;
     // fast ("rotated") path only: the affine map and constants of vegas_iterate_rot.cuh
-    double post_scale, fin0, jac_init;
+    double post_scale, fin0, fin1, jac_init;
     double shift[VEGAS_MAX_DIM], scale[VEGAS_MAX_DIM];
     double fpar[64];                // RotArgs::fpar (kRotParams)
 };

@@ -41,9 +41,9 @@ def _assert_hist(h_gpu, h_ref, precision):
         np.testing.assert_allclose(h_gpu, h_ref, rtol=RTOL64, atol=0)
         assert np.all(h_gpu[h_ref == 0] == 0)
     else:
-        # H accumulates v^2: a relative error eps on the fp32 v is 2 eps on its square (reading R20)
+        # reading F3 / P3: |dH| <= 1e-5 max_b H[j][.] per dimension
         scale = h_ref.max(axis=1, keepdims=True)
-        assert np.all(np.abs(h_gpu - h_ref) <= 2 * RTOL32 * scale)
+        assert np.all(np.abs(h_gpu - h_ref) <= RTOL32 * scale), float(np.max(np.abs(h_gpu - h_ref) / scale))
 
 
 # parity-sized versions of the five configs: several CTAs x several grid-stride passes and a ragged tail
@@ -377,9 +377,9 @@ def test_edge_shapes(B):
             for precision in (64, 32):
                 I, s, H, st = g.iterate(n, 9, 4, fid, precision)
                 oI, oS, oH = O.iterate(edges, n, 9, 4, fid, p)
-                tol = RTOL64 if precision == 64 else 2 * RTOL32
+                tol = RTOL64 if precision == 64 else RTOL32
                 assert st == 0 and I == pytest.approx(oI, rel=tol)
-                assert s == pytest.approx(oS, rel=tol if precision == 64 else 1e-4, abs=1e-300)
+                assert s == pytest.approx(oS, rel=tol, abs=1e-300)
                 _assert_hist(H, oH, precision) if precision == 64 else None
         g.close()
 
@@ -477,6 +477,41 @@ def test_non_default_stream_and_counters(B):
     g.close()
 
 
+def test_fp32_outside_its_range(B):
+    """include/vegas.h (precision, reading C11): v beyond 3.4e38 in fp32 -> non-finite sums -> VEGAS_ENUMERIC while fp64
+    is fine; v below the fp32 range -> a finite estimate, biased low, status 0.  And the range that matters is that of v,
+    not of exp(-E) alone: cfg3's own shape on a grid that is adapted to something else keeps fp32 parity."""
+    # overflow: a narrow Gaussian in 16 dimensions (N = 1.1e44) on a grid that samples its peak
+    dim, nb, a = 16, 50, 1e-3
+    row = np.concatenate([[0.0], np.linspace(0.5 - 3 * a, 0.5 + 3 * a, nb - 1), [1.0]])
+    edges = np.tile(row, (dim, 1))
+    g = B.VegasGrid(dim, nb)
+    g.set_params(B.VEGAS_F_GAUSS, [a])
+    g.set_edges(edges)
+    I64, s64, _, st64 = g.iterate(200_000, 5, 0, B.VEGAS_F_GAUSS, 64)
+    I32, s32, _, st32 = g.iterate(200_000, 5, 0, B.VEGAS_F_GAUSS, 32)
+    assert st64 == 0 and np.isfinite(I64) and I64 > 0
+    assert st32 == B.VEGAS_ENUMERIC and not np.isfinite(I32)
+    g.close()
+    # underflow: cfg3's Gaussian on the uniform grid (f spans > 100 decades, most of it below 1e-38)
+    w = W.config(3)
+    g = _grid(B, w)
+    I64, s64, _, st64 = g.iterate(400_000, 3, 0, w.integrand_id, 64)
+    I32, s32, H32, st32 = g.iterate(400_000, 3, 0, w.integrand_id, 32)
+    assert st64 == 0 and st32 == 0 and np.isfinite(I32) and np.isfinite(s32) and np.all(np.isfinite(H32))
+    assert 0.0 <= I32 <= I64 * (1 + 1e-5)
+    # cfg3's shape on a grid adapted to a wider peak (workloads.adapted_edges): ln N folded into the exponent keeps f
+    # in range, fp32 agrees with the oracle to 1e-5
+    edges = W.adapted_edges(w.dim, w.n_bins, seed=11)
+    g.set_edges(edges)
+    n = 300_007
+    I32, s32, H32, st32 = g.iterate(n, 3, 1, w.integrand_id, 32)
+    oI, oS, oH = O.iterate(edges, n, 3, 1, w.integrand_id, w.params, threads=THREADS)
+    assert st32 == 0 and I32 == pytest.approx(oI, rel=RTOL32) and s32 == pytest.approx(oS, rel=RTOL32)
+    _assert_hist(H32, oH, 32)
+    g.close()
+
+
 # ------------------------------------------------------------------ full BASELINE sizes, bench launch shape
 @pytest.mark.parametrize("cfg,precision", [(2, 64), (3, 64), (3, 32), (4, 64), (5, 64)])
 def test_full_size_iteration_in_bench_configuration(B, chains, cfg, precision):
@@ -559,7 +594,7 @@ def test_genz_product_peak_at_the_papers_16_dimensions(B):
             g.set_edges(ch["edges_trace"][k])
             I, s, H, st = g.iterate(n, seed, k, B.VEGAS_F_GENZ_PRODUCT_PEAK, prec)
             assert st == 0 and I == pytest.approx(ch["per_iter"][k, 0], rel=tol)
-            assert s == pytest.approx(ch["per_iter"][k, 1], rel=tol if prec == 64 else 1e-4)
+            assert s == pytest.approx(ch["per_iter"][k, 1], rel=tol)
             _assert_hist(H, ch["hist_trace"][k], prec)
     g.set_edges(O.uniform_edges(dim, nb))
     r = g.integrate(8, 4_000_000, seed, 1.5, B.VEGAS_F_GENZ_PRODUCT_PEAK, 64, n_skip=3)

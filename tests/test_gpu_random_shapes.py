@@ -41,11 +41,6 @@ def _case(rng):
     else:
         p = W.bw_poly_params(dim, int(rng.integers(1, 1000)))
     precision = int(rng.choice([64, 64, 32]))
-    if fid == 2 and dim > 12:
-        precision = 64        # Eq.(3) with N = 1 peaks at prod c_j^2 ~ 1e2d: beyond the fp32 range (-> VEGAS_ENUMERIC, by design)
-    if fid == 1 and dim > 12 and p[0] < 0.25:
-        precision = 64        # a narrow Gaussian on an un-adapted grid in many dimensions: every sampled f = exp(-E) has
-                              # E > 87, i.e. lies in fp32's denormal range (C11's fp32 f loses digits there, by design)
     return dict(fid=fid, dim=dim, nb=nb, params=p, precision=precision,
                 n=int(rng.integers(20_000, 120_000)), seed=int(rng.integers(1, 2**40)),
                 iteration=int(rng.integers(0, 2**31)), first=int(rng.choice([0, 0, 12345, (1 << 32) - 30_000, 7 << 33])),
@@ -87,10 +82,11 @@ def test_random_shape_iteration_and_refinement(B, case_id):
         assert s == pytest.approx(oS, rel=1e-10, abs=1e-300), info
         np.testing.assert_allclose(H, Ho, rtol=1e-10, atol=0, err_msg=info)
     else:
-        # fp32 per-event arithmetic against the fp64 oracle: 1e-5 on I (north_star); sigma and H carry v^2
+        # fp32 per-event arithmetic against the fp64 oracle: 1e-5 on I, sigma and H (north_star; H in the
+        # per-dimension max-norm, reading F3)
         assert st == 0 and I == pytest.approx(oI, rel=1e-5), info
-        assert s == pytest.approx(oS, rel=1e-4, abs=1e-300), info
-        assert np.all(np.abs(H - Ho) <= 2e-5 * Ho.max(axis=1, keepdims=True)), info
+        assert s == pytest.approx(oS, rel=1e-5, abs=1e-300), info
+        assert np.all(np.abs(H - Ho) <= 1e-5 * Ho.max(axis=1, keepdims=True)), (info, float(np.max(np.abs(H - Ho) / Ho.max(axis=1, keepdims=True))))
     # refinement of the oracle's histogram on the GPU vs the oracle's own (skip all-zero rows: ENUMERIC on both sides)
     want, ost = O.refine(edges, Ho, 1.5)
     rc = g.refine(1.5, hist=Ho)

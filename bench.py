@@ -300,9 +300,8 @@ def main():
 
     # ---- e2e: the same step through the C ABI with HOST buffers (edges in, I/sigma/hist/edges out)
     edges_host = g.get_edges()
-    barrier()
-    t0 = time.perf_counter()
-    for i in range(args.steps):
+
+    def e2e_step(k, edges_host):
         g.set_edges(edges_host)
         if world > 1:
             I, s, H, st = D.iterate_sharded(g, n_step, w.seed, k, fid, args.precision, w.chunk_events,
@@ -310,7 +309,14 @@ def main():
         else:
             I, s, H, st = g.iterate(n_step, w.seed, k, fid, args.precision, w.chunk_events, want_hist=True)
         g.refine(w.alpha, hist=H)
-        edges_host = g.get_edges()
+        return g.get_edges()
+
+    edges_host = e2e_step(k, edges_host)       # untimed: the stand-alone refinement kernel is loaded on its first launch
+    k += 1
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        edges_host = e2e_step(k, edges_host)
         k += 1
     barrier()
     e2e_s = time.perf_counter() - t0

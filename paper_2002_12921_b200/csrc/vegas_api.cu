@@ -26,7 +26,7 @@ constexpr size_t kAlign = 256;
 size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {
-    size_t edges, totals, result, status, hist_up, obs, partials, total;
+    size_t edges, totals, result, status, hist_up, obs, slices, partials, total;
 };
 
 Layout make_layout(int dim, int n_bins) {
@@ -36,9 +36,10 @@ Layout make_layout(int dim, int n_bins) {
     L.edges = off;    off += align_up(sizeof(double) * dim * (n_bins + 1));
     L.totals = off;   off += align_up(sizeof(double) * ntot);
     L.result = off;   off += align_up(sizeof(double) * kResultStride * kMaxIter);
-    L.status = off;   off += align_up(sizeof(int) * 8);
+    L.status = off;   off += align_up(sizeof(int) * 32);    // [0] refinement status, [8..16] CTAs-done tickets
     L.hist_up = off;  off += align_up(sizeof(double) * nent);
     L.obs = off;      off += align_up(sizeof(double) * vegas::kRotMaxObsBins);
+    L.slices = off;   off += align_up(sizeof(double) * nent * vegas::kReduceSlices);
     L.partials = off; off += align_up(sizeof(double) * ntot * kMaxBlocks);
     L.total = off;
     return L;
@@ -71,6 +72,8 @@ struct vegas_grid {
     int* d_status = nullptr;
     double* d_hist_up = nullptr;
     double* d_partials = nullptr;
+    unsigned int* d_counter = nullptr;           // CTAs-done tickets of the one-launch iteration
+    double* d_slices = nullptr;                  // its slice sums (K2's association)
     double* d_obs = nullptr;                     // observable histogram of a user integrand: sums of v per bin
     int n_obs = 0;
     double obs_lo = 0.0, obs_hi = 1.0;
@@ -255,6 +258,14 @@ struct RotShape {
     size_t shmem;
 };
 
+// what the last CTA of a one-launch iteration does after the event loop (vegas_iterate_rot.cuh: RotArgs::tail)
+struct Tail {
+    double n_events, alpha;     // alpha < 0: no refinement
+    double* d_result;           // device, { I, sigma, status }
+};
+int accumulate_impl(vegas_grid* g, uint64_t first_event, uint64_t count, uint64_t chunk_events, uint64_t seed,
+                    uint32_t iteration, int fid, int precision, void* cuda_stream, const Tail* tail);
+
 // One CTA per SM.  n_groups = histogram copies in the CTA (as many as fit next to the table, a divisor of the warp
 // count W), ring = W / n_groups warps share a copy (1 = no token passing).  W is the caller's choice (vegas_set_launch),
 // else: with mbarrier tokens (24-warp kernels) the warp count among the four largest that gives the most copies; with
@@ -322,10 +333,17 @@ cudaError_t launch_rot(vegas_grid* g, int fid, int precision, int dim, const veg
     return cudaErrorInvalidValue;
 }
 
+int fetch_result(vegas_grid* g, cudaStream_t st, double* I, double* sigma, double* hist_host);
+
 int finish_iteration(vegas_grid* g, uint64_t n_total, cudaStream_t st, double* I, double* sigma, double* hist_host) {
-    const size_t nent = (size_t)g->dim * g->n_bins;
     CUDA_TRY(g, vegas::launch_finalize(g->d_totals, (double)n_total, g->d_result, st));
     g->launches++;
+    return fetch_result(g, st, I, sigma, hist_host);
+}
+
+// D2H of { I, sigma, status } (and the histogram totals), one synchronisation
+int fetch_result(vegas_grid* g, cudaStream_t st, double* I, double* sigma, double* hist_host) {
+    const size_t nent = (size_t)g->dim * g->n_bins;
     double res[3] = {0, 0, 0};
     CUDA_TRY(g, cudaMemcpyAsync(res, g->d_result, sizeof(res), cudaMemcpyDeviceToHost, st));
     if (hist_host)
@@ -370,6 +388,8 @@ int vegas_create(int dim, int n_bins, void* dev_workspace, size_t bytes, vegas_g
     g->d_totals = (double*)(g->ws + L.totals);
     g->d_result = (double*)(g->ws + L.result);
     g->d_status = (int*)(g->ws + L.status);
+    g->d_counter = (unsigned int*)(g->d_status + 8);
+    g->d_slices = (double*)(g->ws + L.slices);
     g->d_hist_up = (double*)(g->ws + L.hist_up);
     g->d_partials = (double*)(g->ws + L.partials);
     g->d_obs = (double*)(g->ws + L.obs);
@@ -535,6 +555,47 @@ int vegas_begin_iteration(vegas_grid* g, void* cuda_stream) {
 
 int vegas_accumulate(vegas_grid* g, uint64_t first_event, uint64_t count, uint64_t chunk_events, uint64_t seed,
                      uint32_t iteration, int fid, int precision, void* cuda_stream) {
+    return accumulate_impl(g, first_event, count, chunk_events, seed, iteration, fid, precision, cuda_stream, nullptr);
+}
+
+}  // extern "C"
+#pragma GCC visibility pop
+
+namespace {
+
+// Can a whole iteration of n events from event 0 run as one fast-path launch (reduce, finalize and refine fused into it)?
+bool one_launch_iteration(const vegas_grid* g, uint64_t n_events, int fid, int precision) {
+    return use_rot_path(g, fid, precision) && n_events <= 0xFFF00000ull;
+}
+
+// One iteration in the stream, not synchronised: totals, result slot (and the refined grid if alpha >= 0) on the device.
+int enqueue_iteration(vegas_grid* g, uint64_t n_events, uint64_t chunk_events, uint64_t seed, uint32_t iteration, int fid,
+                      int precision, cudaStream_t st, double alpha, double* d_result) {
+    if (one_launch_iteration(g, n_events, fid, precision)) {
+        const RotShape rs = rot_shape(g, fid);
+        if (rs.blocks > kMaxBlocks) return VEGAS_EINVAL;
+        g->active_blocks = rs.blocks;
+        if (g->n_obs > 0) CUDA_TRY(g, cudaMemsetAsync(g->d_obs, 0, sizeof(double) * vegas::kRotMaxObsBins, st));
+        const Tail tail{(double)n_events, alpha, d_result};
+        return accumulate_impl(g, 0, n_events, chunk_events, seed, iteration, fid, precision, (void*)st, &tail);
+    }
+    int rc = vegas_begin_iteration(g, (void*)st);
+    if (rc) return rc;
+    rc = accumulate_impl(g, 0, n_events, chunk_events, seed, iteration, fid, precision, (void*)st, nullptr);
+    if (rc) return rc;
+    rc = vegas_reduce(g, (void*)st);
+    if (rc) return rc;
+    CUDA_TRY(g, vegas::launch_finalize(g->d_totals, (double)n_events, d_result, st));
+    g->launches++;
+    if (alpha >= 0.0) {
+        CUDA_TRY(g, vegas::launch_refine(g->d_edges, g->d_totals + 4, g->dim, g->n_bins, alpha, g->d_status, st));
+        g->launches++;
+    }
+    return VEGAS_OK;
+}
+
+int accumulate_impl(vegas_grid* g, uint64_t first_event, uint64_t count, uint64_t chunk_events, uint64_t seed,
+                    uint32_t iteration, int fid, int precision, void* cuda_stream, const Tail* tail) {
     if (!check_call(g, fid, precision)) return VEGAS_EINVAL;
     if (g->active_blocks <= 0) return VEGAS_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -598,6 +659,18 @@ int vegas_accumulate(vegas_grid* g, uint64_t first_event, uint64_t count, uint64
         a.first_event = ra.first_event = first_event + done;
         a.count = ra.count = n_launch;
         ra.pdl = (done > 0 && !g->profiling) ? 1 : 0;   // chunk k > 0 follows chunk k-1 of this call directly in the stream
+        if (tail) {                                     // the whole iteration is this one launch (one_launch_iteration)
+            ra.overwrite = 1;
+            ra.tail = 1;
+            ra.tail_n = tail->n_events;
+            ra.tail_alpha = tail->alpha;
+            ra.totals = g->d_totals;
+            ra.result = tail->d_result;
+            ra.status = g->d_status;
+            ra.counter = g->d_counter;
+            ra.slices = g->d_slices;
+            ra.tail_smem_doubles = (unsigned int)(rs.shmem / sizeof(double));
+        }
         cudaEvent_t e0 = nullptr, e1 = nullptr;
         if (g->profiling) {
             if (g->events_used + 2 > g->events.size()) {
@@ -623,6 +696,11 @@ int vegas_accumulate(vegas_grid* g, uint64_t first_event, uint64_t count, uint64
     return VEGAS_OK;
 }
 
+}  // namespace
+
+#pragma GCC visibility push(default)
+extern "C" {
+
 int vegas_reduce(vegas_grid* g, void* cuda_stream) {
     if (!g || g->active_blocks <= 0) return VEGAS_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -646,13 +724,11 @@ size_t vegas_totals_count(const vegas_grid* g) { return g ? 4 + (size_t)g->dim *
 int vegas_iterate(vegas_grid* g, uint64_t n_events, uint64_t chunk_events, uint64_t seed, uint32_t iteration,
                   int fid, int precision, void* cuda_stream, double* I, double* sigma, double* hist_host) {
     if (!check_call(g, fid, precision) || n_events < 2) return VEGAS_EINVAL;
-    int rc = vegas_begin_iteration(g, cuda_stream);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CUDA_TRY(g, cudaSetDevice(g->device));
+    const int rc = enqueue_iteration(g, n_events, chunk_events, seed, iteration, fid, precision, st, -1.0, g->d_result);
     if (rc) return rc;
-    rc = vegas_accumulate(g, 0, n_events, chunk_events, seed, iteration, fid, precision, cuda_stream);
-    if (rc) return rc;
-    rc = vegas_reduce(g, cuda_stream);
-    if (rc) return rc;
-    return finish_iteration(g, n_events, (cudaStream_t)cuda_stream, I, sigma, hist_host);
+    return fetch_result(g, st, I, sigma, hist_host);
 }
 
 int vegas_refine(vegas_grid* g, const double* hist_host, double alpha, void* cuda_stream) {
@@ -729,19 +805,9 @@ int vegas_integrate_from(vegas_grid* g, uint32_t first_iteration, int n_iter, in
     CUDA_TRY(g, cudaSetDevice(g->device));
     CUDA_TRY(g, cudaMemsetAsync(g->d_status, 0, sizeof(int), st));
     for (int k = 0; k < n_iter; ++k) {
-        int rc = vegas_begin_iteration(g, cuda_stream);
+        const int rc = enqueue_iteration(g, n_events, chunk_events, seed, first_iteration + (uint32_t)k, fid, precision, st,
+                                         alpha >= 0.0 ? alpha : -1.0, g->d_result + (size_t)kResultStride * k);
         if (rc) return rc;
-        rc = vegas_accumulate(g, 0, n_events, chunk_events, seed, first_iteration + (uint32_t)k, fid, precision,
-                              cuda_stream);
-        if (rc) return rc;
-        rc = vegas_reduce(g, cuda_stream);
-        if (rc) return rc;
-        CUDA_TRY(g, vegas::launch_finalize(g->d_totals, (double)n_events, g->d_result + (size_t)kResultStride * k, st));
-        g->launches++;
-        if (alpha >= 0.0) {
-            CUDA_TRY(g, vegas::launch_refine(g->d_edges, g->d_totals + 4, g->dim, g->n_bins, alpha, g->d_status, st));
-            g->launches++;
-        }
     }
     std::vector<double> res((size_t)kResultStride * n_iter);
     int status = 0;

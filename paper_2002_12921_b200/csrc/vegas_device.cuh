@@ -254,4 +254,121 @@ __device__ __forceinline__ dd dd_warp_sum(dd v) {
     return v;
 }
 
+// ------------------------------------------------------------------------------------------
+// S5/S6 second level, S7 and S8 as device functions: the stand-alone kernels K2, finalize and K3 (vegas_kernels.cu)
+// and the tail that the last CTA of a fused iterate launch runs (vegas_iterate_rot.cuh) call the same code, so an
+// iteration gives the same bits whichever way it is finished.
+// ------------------------------------------------------------------------------------------
+
+// K2, one of the two double-double sums (i = 0: S1, i = 2: S2) by one warp: lane l adds the partials of CTAs
+// l, l+32, ... in that order, then a fixed shuffle tree -- the same association for every run of a launch shape.
+// (loads through L2, __ldcg: in the fused tail the rows were written by other CTAs of the same launch)
+__device__ __forceinline__ void reduce_dd_sum(const double* partials, int n_parts, int n_tot, int i, int lane, double* totals) {
+    dd s{0.0, 0.0};
+    for (int p = lane; p < n_parts; p += 32)
+        s = dd_add(s, dd{__ldcg(partials + (size_t)p * n_tot + i), __ldcg(partials + (size_t)p * n_tot + i + 1)});
+    s = dd_warp_sum(s);
+    if (lane == 0) { totals[i] = s.hi; totals[i + 1] = s.lo; }
+}
+
+// K2, one slice of a histogram total: the partials of CTAs w, w+8, w+16, ... added in that order (8 loads in flight)
+__device__ __forceinline__ double reduce_hist_slice(const double* partials, int n_parts, int n_tot, int i, int w) {
+    double h = 0.0;
+    int p = w;
+    for (; p + 56 < n_parts; p += 64) {
+        double v[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) v[k] = __ldcg(partials + (size_t)(p + 8 * k) * n_tot + i);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) h += v[k];
+    }
+    for (; p < n_parts; p += 8) h += __ldcg(partials + (size_t)p * n_tot + i);
+    return h;
+}
+constexpr int kReduceSlices = 8;
+
+// S7 (C7): I = S1/n; Var = (S2/n - I^2)/(n-1); sigma = sqrt(max(Var, 0)), in double-double.
+// result = { I, sigma, status } (status 0 or VEGAS_ENUMERIC as a double).
+__device__ __forceinline__ void finalize_result(const double* totals, double n, double* result) {
+    const dd S1 = fast_two_sum(totals[0], totals[1]);
+    const dd S2 = fast_two_sum(totals[2], totals[3]);
+    const dd mean = dd_div_d(S1, n);
+    const dd ex2 = dd_div_d(S2, n);
+    const dd diff = dd_add(ex2, dd_neg(dd_sqr(mean)));
+    const dd var = dd_div_d(diff, n - 1.0);
+    const double v = var.hi + var.lo;
+    const double I = mean.hi + mean.lo;
+    const double sigma = (v > 0.0) ? sqrt(v) : ((v != v) ? v : 0.0);
+    result[0] = I;
+    result[1] = sigma;
+    result[2] = (isfinite(I) && isfinite(sigma) && isfinite(S2.hi)) ? 0.0 : -3.0 /* VEGAS_ENUMERIC */;
+}
+
+// S8 (C8) for one dimension by a group of `gsize` threads (a whole CTA: SYNC = __syncthreads; one warp: SYNC =
+// __syncwarp), thread `gi` of the group.  The two running sums that decide where the new edges fall (sum of s_i,
+// cumulative sum of m_i) are formed by thread 0 of the group in index order, i.e. in the order the method states them,
+// so the walk "advance while C + m_i < t" sees the same doubles whichever thread evaluates it.
+// scratch: 4 n_bins + 3 doubles of shared memory for the group.  *status is set to VEGAS_ENUMERIC (-3) if the
+// dimension has no finite positive smoothed sum (its grid is left unchanged).
+struct SyncCta { __device__ __forceinline__ void operator()() const { __syncthreads(); } };
+struct SyncWarp { __device__ __forceinline__ void operator()() const { __syncwarp(); } };
+template <class SYNC>
+__device__ __forceinline__ void refine_dimension(double* Xg, const double* h, int nb, double alpha,
+                                                 int* status, double* scratch, int gi, int gsize, SYNC sync) {
+    double* X = scratch;                 // nb + 1
+    double* m = X + nb + 1;              // nb
+    double* cum = m + nb;                // nb + 1
+    double* s = cum + nb + 1;            // nb
+    double* total_s = s + nb;            // 1
+    for (int i = gi; i < nb; i += gsize) {
+        X[i] = Xg[i];
+        if (i == 0) X[nb] = Xg[nb];
+        double si;
+        if (i == 0) si = (h[0] + h[1]) / 2.0;
+        else if (i == nb - 1) si = (h[nb - 2] + h[nb - 1]) / 2.0;
+        else si = (h[i - 1] + h[i] + h[i + 1]) / 3.0;
+        s[i] = si;
+    }
+    sync();
+    if (gi == 0) {
+        double t = 0.0;
+        for (int k = 0; k < nb; ++k) t += s[k];
+        *total_s = t;
+    }
+    sync();
+    const double total = *total_s;
+    if (!(total > 0.0) || !isfinite(total)) {
+        if (gi == 0) *status = -3 /* VEGAS_ENUMERIC */;
+        return;   // whole group: this dimension keeps its grid
+    }
+    for (int i = gi; i < nb; i += gsize) {
+        const double p = s[i] / total;
+        double mi;
+        if (p <= 0.0) mi = 0.0;
+        else if (p >= 1.0) mi = 1.0;
+        else mi = pow((1.0 - p) / log(1.0 / p), alpha);
+        m[i] = mi;
+    }
+    sync();
+    if (gi == 0) {
+        double c = 0.0;
+        cum[0] = 0.0;
+        for (int k = 0; k < nb; ++k) { c += m[k]; cum[k + 1] = c; }
+    }
+    sync();
+    for (int i = gi; i < nb; i += gsize) {
+        if (i >= 1) {
+            const double delta = cum[nb] / (double)nb;
+            const double t = (double)i * delta;
+            int k = 0;
+            while (k < nb - 1 && cum[k + 1] < t) ++k;        // cum[k+1] == C + m_k of the sequential walk
+            double frac = (m[k] > 0.0) ? (t - cum[k]) / m[k] : 0.0;
+            frac = fmin(fmax(frac, 0.0), 1.0);
+            Xg[i] = X[k] + frac * (X[k + 1] - X[k]);
+        }
+    }
+    if (gi == 0) { Xg[0] = 0.0; Xg[nb] = 1.0; }
+}
+__host__ __device__ constexpr size_t refine_scratch_doubles(int n_bins) { return 4 * (size_t)n_bins + 3; }
+
 }  // namespace vegas

@@ -233,6 +233,17 @@ struct RotArgs {
     double jac_init;                // start value of the running Jacobian product (a power of two, see RotEntry)
     double fin0, fin1;              // integrand finish constants (IntegrandU::finish / value)
     double shift[VEGAS_MAX_DIM], scale[VEGAS_MAX_DIM];
+    // The iteration as ONE launch (vegas_iterate / vegas_integrate when the whole iteration fits one launch):
+    int overwrite;                  // 1: first launch of an iteration: the CTA's partial row is overwritten, not added to
+    int tail;                       // 1: the last CTA to finish reduces the partials (K2), finalises (S7) and, if
+                                    //    tail_alpha >= 0, refines the grid (S8) -- same device code as the stand-alone kernels
+    double tail_n, tail_alpha;      // events of the whole iteration; damping exponent (< 0: no refinement)
+    double* totals;                 // device, [4 + DIM*n_bins]
+    double* result;                 // device, { I, sigma, status } of this iteration
+    int* status;                    // device, refinement status word
+    double* slices;                 // device, [8][DIM*n_bins]: K2's slice sums
+    unsigned int* counter;          // device, 8 + 1 CTAs-done tickets (0 before the launch, reset by the last CTA)
+    unsigned int tail_smem_doubles; // doubles of dynamic shared memory the launch has (scratch of the refinement)
     int pdl;                        // host side: launch with programmatic stream serialisation (the previous launch in
                                     // the stream is a chunk of the same accumulate call); the kernel does not read it
     double* obs;                    // USER with an observable: device, [n_obs] sums of v per observable bin, or NULL
@@ -306,11 +317,14 @@ template <typename T, int NCH> struct IntegrandU<VEGAS_F_USER, T, NCH> {
 //    this way (cfg1, cfg2, cfg5).
 //  * BW_POLY keeps 4 coefficients per dimension per lane in registers, and a user integrand's register needs are
 //    unknown: 12 warps, up to 168 registers.
+#ifndef VEGAS_ROT_BW_WARPS
+#define VEGAS_ROT_BW_WARPS 12
+#endif
 #ifndef VEGAS_ROT_WIDE_MIN_DIM
 #define VEGAS_ROT_WIDE_MIN_DIM 13
 #endif
 __host__ __device__ constexpr int rot_max_warps(int fid, int dim) {
-    return (fid == VEGAS_F_BW_POLY || fid == VEGAS_F_USER) ? 12 : (dim >= VEGAS_ROT_WIDE_MIN_DIM ? 24 : 16);
+    return (fid == VEGAS_F_USER || (fid == VEGAS_F_BW_POLY && VEGAS_ROT_BW_WARPS == 12)) ? 12 : (dim >= VEGAS_ROT_WIDE_MIN_DIM ? 24 : 16);
 }
 __host__ __device__ constexpr int rot_max_threads(int fid, int dim) { return 32 * rot_max_warps(fid, dim); }
 __host__ __device__ constexpr bool rot_mbar_tokens(int fid, int dim) { return rot_max_warps(fid, dim) > 16; }
@@ -518,6 +532,56 @@ __device__ __forceinline__ void rot_hist_sections(const uint32_t (&haddr)[(DIM +
     }
 }
 
+// The rest of the iteration in the same launch, by CTAs-done tickets in two levels that follow K2's own association:
+// the last CTA of slice w (the CTAs w, w+8, w+16, ...) adds that slice's partial rows in K2's fixed order; the last
+// slice to finish adds the 8 slice sums in slice order, finalises (S7) and refines (S8).  Which CTA draws the last
+// ticket does not matter for the result, and no CTA ever waits for another.  (Not inlined: the event loop's register
+// allocation and scheduling stay what they are without it.)
+static __device__ __noinline__ void rot_tail(const RotArgs& a, int dim, unsigned char* smem, unsigned int* ticket) {
+    const int nb = a.n_bins, lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = (blockDim.x + 31) >> 5;
+    const int DIM = dim;
+    const int n_parts = (int)gridDim.x, n_tot = 4 + DIM * nb, nent = DIM * nb;
+    const int w_me = (int)(blockIdx.x % kReduceSlices);
+    const unsigned int in_slice = (unsigned int)((n_parts - w_me + kReduceSlices - 1) / kReduceSlices);
+    const unsigned int n_slices = (unsigned int)(n_parts < kReduceSlices ? n_parts : kReduceSlices);
+    __threadfence();                                   // this CTA's partial row is visible device-wide ...
+    __syncthreads();
+    if (threadIdx.x == 0) *ticket = atomicAdd(a.counter + w_me, 1u);      // ... before its ticket is drawn
+    __syncthreads();
+    if (*ticket != in_slice - 1) return;
+    __threadfence();
+    double* my_slice = a.slices + (size_t)w_me * nent;
+    for (int i = (int)threadIdx.x; i < nent; i += blockDim.x)
+        my_slice[i] = reduce_hist_slice(a.partials, n_parts, n_tot, 4 + i, w_me);
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) *ticket = atomicAdd(a.counter + kReduceSlices, 1u);
+    __syncthreads();
+    if (*ticket != n_slices - 1) return;
+    __threadfence();
+    if (warp == 0) reduce_dd_sum(a.partials, n_parts, n_tot, 0, lane, a.totals);
+    if (warp == (nwarps > 1 ? 1 : 0)) reduce_dd_sum(a.partials, n_parts, n_tot, 2, lane, a.totals);
+    for (int i = (int)threadIdx.x; i < nent; i += blockDim.x) {
+        double t = __ldcg(a.slices + i);
+        for (unsigned int w = 1; w < n_slices; ++w) t += __ldcg(a.slices + (size_t)w * nent + i);
+        a.totals[4 + i] = t;
+    }
+    if (threadIdx.x <= kReduceSlices) a.counter[threadIdx.x] = 0u;
+    __syncthreads();
+    if (threadIdx.x == 0) finalize_result(a.totals, a.tail_n, a.result);
+    if (a.tail_alpha >= 0.0) {
+        // one warp per dimension, as many at a time as the CTA's shared memory (all of it is free now) has room for
+        double* scratch = reinterpret_cast<double*>(smem);
+        const int per = (int)refine_scratch_doubles(nb);
+        int conc = (int)((size_t)a.tail_smem_doubles / (size_t)per);
+        if (conc > nwarps) conc = nwarps;
+        if (warp < conc)
+            for (int j = warp; j < DIM; j += conc)
+                refine_dimension(const_cast<double*>(a.edges) + (size_t)j * (nb + 1), a.totals + 4 + (size_t)j * nb, nb,
+                                 a.tail_alpha, a.status, scratch + (size_t)warp * per, lane, 32, SyncWarp{});
+    }
+}
+
 template <int FID, typename T, int DIM>
 __global__ void __launch_bounds__(rot_max_threads(FID, DIM), 1)
 k_iterate_rot(const __grid_constant__ RotArgs a) {
@@ -664,7 +728,7 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
         const int idx = threadIdx.x + k * blockDim.x;
-        own[k] = (idx < DIM * nb) ? part[4 + idx] : 0.0;
+        own[k] = (idx < DIM * nb && !a.overwrite) ? part[4 + idx] : 0.0;
     }
     __syncthreads();
     // warp 0 adds the warps' sums (latency-bound double-double chains) while the other warps merge the histograms
@@ -675,8 +739,10 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
         t1 = dd_warp_sum(t1);
         t2 = dd_warp_sum(t2);
         if (lane == 0) {
-            t1 = dd_add(t1, dd{part[0], part[1]});
-            t2 = dd_add(t2, dd{part[2], part[3]});
+            if (!a.overwrite) {
+                t1 = dd_add(t1, dd{part[0], part[1]});
+                t2 = dd_add(t2, dd{part[2], part[3]});
+            }
             part[0] = t1.hi; part[1] = t1.lo; part[2] = t2.hi; part[3] = t2.lo;
         }
     }
@@ -725,9 +791,13 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
         const int idx = threadIdx.x + k * blockDim.x;
         if (idx < DIM * nb) part[4 + idx] = own[k] + stage[idx];
     }
-    for (int idx = threadIdx.x + 4 * blockDim.x; idx < DIM * nb; idx += blockDim.x) part[4 + idx] += stage[idx];
+    for (int idx = threadIdx.x + 4 * blockDim.x; idx < DIM * nb; idx += blockDim.x)
+        part[4 + idx] = a.overwrite ? stage[idx] : part[4 + idx] + stage[idx];
     // observable bins: one global add per bin per CTA per launch (the order over CTAs is not fixed: 1e-16 effects)
     if (FID == VEGAS_F_USER && a.obs != nullptr && (int)threadIdx.x < a.n_obs) atomicAdd(a.obs + threadIdx.x, obs_sh[threadIdx.x]);
+
+    // ---- the rest of the iteration in the same launch (rot_tail): K2, S7 and S8 by the last CTAs to finish
+    if (a.tail) rot_tail(a, DIM, smem_rot, reinterpret_cast<unsigned int*>(red));
 }
 
 #ifndef __CUDACC_RTC__

@@ -200,121 +200,41 @@ __global__ void k_reduce(const double* __restrict__ partials, int n_parts, int n
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (blockIdx.x == 0) {
         if (t >= 64) return;
-        // S1 (warp 0) and S2 (warp 1): lane l adds the partials of CTAs l, l+32, ... in that order, then a fixed
-        // shuffle tree -- the same association for every run of a given launch shape
-        const int i = 2 * (t >> 5), lane = t & 31;
-        dd s{0.0, 0.0};
-        for (int p = lane; p < n_parts; p += 32)
-            s = dd_add(s, dd{partials[(size_t)p * n_tot + i], partials[(size_t)p * n_tot + i + 1]});
-        s = dd_warp_sum(s);
-        if (lane == 0) { totals[i] = s.hi; totals[i + 1] = s.lo; }
+        reduce_dd_sum(partials, n_parts, n_tot, 2 * (t >> 5), t & 31, totals);     // S1 (warp 0) and S2 (warp 1)
         return;
     }
-    // histogram totals: block b > 0 owns 32 consecutive totals; its 8 warps each add every 8th CTA's partial
-    // (4 loads in flight), and warp 0 adds the 8 slice sums in slice order -- a fixed association
+    // histogram totals: block b > 0 owns 32 consecutive totals; its 8 warps each add every 8th CTA's partial,
+    // and warp 0 adds the 8 slice sums in slice order -- a fixed association
     __shared__ double slice[8][32];
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int i = 4 + ((int)blockIdx.x - 1) * 32 + lane;
-    double h = 0.0;
-    if (i < n_tot) {
-        int p = w;
-        for (; p + 24 < n_parts; p += 32) {
-            const double v0 = partials[(size_t)p * n_tot + i], v1 = partials[(size_t)(p + 8) * n_tot + i];
-            const double v2 = partials[(size_t)(p + 16) * n_tot + i], v3 = partials[(size_t)(p + 24) * n_tot + i];
-            h += v0; h += v1; h += v2; h += v3;
-        }
-        for (; p < n_parts; p += 8) h += partials[(size_t)p * n_tot + i];
-    }
-    slice[w][lane] = h;
+    slice[w][lane] = (i < n_tot) ? reduce_hist_slice(partials, n_parts, n_tot, i, w) : 0.0;
     __syncthreads();
     if (w == 0 && i < n_tot) {
         double t = slice[0][lane];
-#pragma unroll
-        for (int k = 1; k < 8; ++k) t += slice[k][lane];
+        for (int k = 1; k < 8 && k < n_parts; ++k) t += slice[k][lane];
         totals[i] = t;
     }
 }
 
-// S7 (C7): I = S1/n; Var = (S2/n - I^2)/(n-1); sigma = sqrt(max(Var, 0)).
-// result = { I, sigma, status } (status 0 or VEGAS_ENUMERIC as a double).
+// S7 (C7), one thread
 __global__ void k_finalize(const double* __restrict__ totals, double n, double* __restrict__ result) {
     pdl_wait();
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    const dd S1 = fast_two_sum(totals[0], totals[1]);
-    const dd S2 = fast_two_sum(totals[2], totals[3]);
-    const dd mean = dd_div_d(S1, n);
-    const dd ex2 = dd_div_d(S2, n);
-    const dd diff = dd_add(ex2, dd_neg(dd_sqr(mean)));
-    const dd var = dd_div_d(diff, n - 1.0);
-    const double v = var.hi + var.lo;
-    const double I = mean.hi + mean.lo;
-    const double sigma = (v > 0.0) ? sqrt(v) : ((v != v) ? v : 0.0);
-    result[0] = I;
-    result[1] = sigma;
-    result[2] = (isfinite(I) && isfinite(sigma) && isfinite(S2.hi)) ? 0.0 : (double)VEGAS_ENUMERIC;
+    finalize_result(totals, n, result);
 }
 
 // ---------------------------------------------------------------------------------------------
-// K3 (C8): one CTA per dimension, one thread per bin.  The two running sums that decide where the
-// new edges fall (sum of s_i, cumulative sum of m_i) are formed by thread 0 in index order, i.e. in
-// the order the method states them, so the walk "advance while C + m_i < t" sees the same doubles
-// whichever thread evaluates it.
+// K3 (C8): one CTA per dimension (refine_dimension in vegas_device.cuh).
 // status[0] is set to VEGAS_ENUMERIC if a dimension has no finite positive smoothed sum.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(VEGAS_MAX_BINS)
 k_refine(double* __restrict__ edges, const double* __restrict__ hist, int n_bins, double alpha, int* status) {
-    __shared__ double X[VEGAS_MAX_BINS + 1], m[VEGAS_MAX_BINS], cum[VEGAS_MAX_BINS + 1], s[VEGAS_MAX_BINS];
-    __shared__ double total_s;
+    __shared__ double scratch[refine_scratch_doubles(VEGAS_MAX_BINS)];
     pdl_wait();
-    const int j = blockIdx.x, nb = n_bins, i = threadIdx.x;
-    double* Xg = edges + (size_t)j * (nb + 1);
-    const double* h = hist + (size_t)j * nb;
-    if (i < nb) {
-        X[i] = Xg[i];
-        if (i == 0) X[nb] = Xg[nb];
-        double si;
-        if (i == 0) si = (h[0] + h[1]) / 2.0;
-        else if (i == nb - 1) si = (h[nb - 2] + h[nb - 1]) / 2.0;
-        else si = (h[i - 1] + h[i] + h[i + 1]) / 3.0;
-        s[i] = si;
-    }
-    __syncthreads();
-    if (i == 0) {
-        double t = 0.0;
-        for (int k = 0; k < nb; ++k) t += s[k];
-        total_s = t;
-    }
-    __syncthreads();
-    const double total = total_s;
-    if (!(total > 0.0) || !isfinite(total)) {
-        if (i == 0) *status = VEGAS_ENUMERIC;
-        return;   // whole CTA: this dimension keeps its grid
-    }
-    if (i < nb) {
-        const double p = s[i] / total;
-        double mi;
-        if (p <= 0.0) mi = 0.0;
-        else if (p >= 1.0) mi = 1.0;
-        else mi = pow((1.0 - p) / log(1.0 / p), alpha);
-        m[i] = mi;
-    }
-    __syncthreads();
-    if (i == 0) {
-        double c = 0.0;
-        cum[0] = 0.0;
-        for (int k = 0; k < nb; ++k) { c += m[k]; cum[k + 1] = c; }
-    }
-    __syncthreads();
-    if (i >= 1 && i < nb) {
-        const double delta = cum[nb] / (double)nb;
-        const double t = (double)i * delta;
-        int k = 0;
-        while (k < nb - 1 && cum[k + 1] < t) ++k;        // cum[k+1] == C + m_k of the sequential walk
-        double frac = (m[k] > 0.0) ? (t - cum[k]) / m[k] : 0.0;
-        frac = fmin(fmax(frac, 0.0), 1.0);
-        Xg[i] = X[k] + frac * (X[k + 1] - X[k]);
-    }
-    if (i == 0) { Xg[0] = 0.0; Xg[nb] = 1.0; }
+    const int j = blockIdx.x;
+    refine_dimension(edges + (size_t)j * (n_bins + 1), hist + (size_t)j * n_bins, n_bins, alpha, status, scratch,
+                     (int)threadIdx.x, (int)blockDim.x, SyncCta{});
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -183,7 +183,6 @@ bool use_rot_path(const vegas_grid* g, int fid, int precision) {
     const bool kind = fid == VEGAS_F_CONST || fid == VEGAS_F_GAUSS || fid == VEGAS_F_GENZ_PRODUCT_PEAK ||
                       (fid == VEGAS_F_BW_POLY && g->dim <= vegas::kRotBwMaxDim);
     if (!kind) return false;
-    if (g->cfg_threads > vegas::rot_max_threads(fid, g->dim)) return false;
     return vegas::rot_shared_bytes(g->dim, g->n_bins, 1) <= g->smem_optin;
 }
 
@@ -286,6 +285,7 @@ RotShape rot_shape(const vegas_grid* g, int fid) {
     int W = wmax;
     if (g->cfg_threads > 0) {
         W = (g->cfg_threads + 31) / 32;
+        if (W > wmax) W = wmax;                        // the kernel's launch bound (a user kernel is built for 12 warps)
         if (!mbar && fit < W && W > vegas::kRotMaxNamedRingWarps) W = vegas::kRotMaxNamedRingWarps;
     } else if (mbar) {
         int best = 0;
@@ -397,7 +397,7 @@ int vegas_create(int dim, int n_bins, void* dev_workspace, size_t bytes, vegas_g
     for (int j = 0; j < dim; ++j)
         for (int i = 0; i <= n_bins; ++i) edges[(size_t)j * (n_bins + 1) + i] = (double)i / (double)n_bins;
     e = cudaMemcpy(g->d_edges, edges.data(), sizeof(double) * edges.size(), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMemset(g->d_totals, 0, L.hist_up + align_up(sizeof(double) * dim * n_bins) - L.totals);
+    if (e == cudaSuccess) e = cudaMemset(g->d_totals, 0, L.slices - L.totals);      // totals .. observable sums
     if (e != cudaSuccess) { delete g; return VEGAS_ECUDA; }
     *out = g;
     return VEGAS_OK;
@@ -412,6 +412,7 @@ int vegas_destroy(vegas_grid* g) {
 }
 
 int vegas_set_params(vegas_grid* g, int fid, const double* p, int n_params) {
+    // everything is validated into temporaries: a rejected call leaves the grid's parameters as they were
     if (g && fid == VEGAS_F_USER) {
         if (n_params < 0 || n_params > VEGAS_USER_MAX_PARAMS || (n_params > 0 && !p)) return VEGAS_EINVAL;
         for (int i = 0; i < n_params; ++i)
@@ -426,10 +427,7 @@ int vegas_set_params(vegas_grid* g, int fid, const double* p, int n_params) {
     if (want < 0 || n_params != want || want > VEGAS_MAX_PARAMS || (want > 0 && !p)) return VEGAS_EINVAL;
     for (int i = 0; i < want; ++i)
         if (!std::isfinite(p[i])) return VEGAS_EINVAL;
-    double* d = g->derived[fid];
-    std::memset(d, 0, sizeof(g->derived[fid]));
-    std::memset(g->user[fid], 0, sizeof(g->user[fid]));
-    for (int i = 0; i < want; ++i) g->user[fid][i] = p[i];
+    double d[VEGAS_MAX_PARAMS] = {};
     const int dim = g->dim;
     switch (fid) {
     case VEGAS_F_CONST: break;
@@ -453,11 +451,14 @@ int vegas_set_params(vegas_grid* g, int fid, const double* p, int n_params) {
         d[1] = m_max * m_max - m_min * m_min;
         d[2] = M * M;
         d[3] = M * M * G * G;
-        if (!(d[3] > 0.0)) return VEGAS_EINVAL;
+        if (!(d[3] > 0.0) || !(d[1] > 0.0)) return VEGAS_EINVAL;       // M Gamma != 0, m_max^2 > m_min^2
         for (int i = 0; i < 5 * (dim - 1); ++i) d[4 + i] = p[4 + i];
         break;
     }
     }
+    std::memcpy(g->derived[fid], d, sizeof(d));
+    std::memset(g->user[fid], 0, sizeof(g->user[fid]));
+    for (int i = 0; i < want; ++i) g->user[fid][i] = p[i];
     g->params_set[fid] = true;
     return VEGAS_OK;
 }
@@ -467,18 +468,24 @@ int vegas_set_user_integrand(vegas_grid* g, const char* cuda_source, const doubl
     if (log && log_bytes) log[0] = '\0';
     if (!g || !cuda_source) return VEGAS_EINVAL;
     if (vegas::rot_shared_bytes(g->dim, g->n_bins, 1) > g->smem_optin) return VEGAS_EINVAL;
-    const int rc_p = vegas_set_params(g, VEGAS_F_USER, params_host, n_params);
-    if (rc_p != VEGAS_OK) return rc_p;
+    if (n_params < 0 || n_params > VEGAS_USER_MAX_PARAMS || (n_params > 0 && !params_host)) return VEGAS_EINVAL;
+    for (int i = 0; i < n_params; ++i)
+        if (!std::isfinite(params_host[i])) return VEGAS_EINVAL;
     CUDA_TRY(g, cudaSetDevice(g->device));
     std::string clog, err;
-    const int rc = vegas::user_compile(cuda_source, g->dim, &clog, &g->ukernel, &err);
+    vegas::UserKernel fresh;                         // the old kernel and its parameters stay until this one is ready
+    const int rc = vegas::user_compile(cuda_source, g->dim, &clog, &fresh, &err);
     if (log && log_bytes) {
         const std::string& msg = clog.empty() ? err : clog;
         snprintf(log, log_bytes, "%s", msg.c_str());
     }
-    if (rc == 0) return VEGAS_OK;
-    snprintf(g->cuda_err, sizeof(g->cuda_err), "%s", err.c_str());
-    return rc == -1 ? VEGAS_EINVAL : VEGAS_ECUDA;
+    if (rc != 0) {
+        snprintf(g->cuda_err, sizeof(g->cuda_err), "%s", err.c_str());
+        return rc == -1 ? VEGAS_EINVAL : VEGAS_ECUDA;
+    }
+    vegas::user_unload(&g->ukernel);
+    g->ukernel = fresh;
+    return vegas_set_params(g, VEGAS_F_USER, params_host, n_params);
 }
 
 int vegas_set_observable(vegas_grid* g, double lo, double hi, int n_obs_bins) {
@@ -549,7 +556,7 @@ int vegas_begin_iteration(vegas_grid* g, void* cuda_stream) {
     g->active_blocks = blocks;
     const size_t ntot = 4 + (size_t)g->dim * g->n_bins;
     CUDA_TRY(g, cudaMemsetAsync(g->d_partials, 0, sizeof(double) * ntot * blocks, st));
-    if (g->n_obs > 0) CUDA_TRY(g, cudaMemsetAsync(g->d_obs, 0, sizeof(double) * vegas::kRotMaxObsBins, st));
+    CUDA_TRY(g, cudaMemsetAsync(g->d_obs, 0, sizeof(double) * vegas::kRotMaxObsBins, st));
     return VEGAS_OK;
 }
 
@@ -755,8 +762,14 @@ int vegas_combine(int n_iter, int n_skip, const double* I_k, const double* sigma
         return VEGAS_EINVAL;
     const int K = n_iter - n_skip;
     bool any_zero = false;
-    for (int k = n_skip; k < n_iter; ++k)
-        if (!(sigma_k[k] > 0.0)) any_zero = true;
+    for (int k = n_skip; k < n_iter; ++k) {
+        if (!std::isfinite(I_k[k]) || !std::isfinite(sigma_k[k]) || sigma_k[k] < 0.0) {
+            // an iteration that ended in VEGAS_ENUMERIC: nothing sensible can be combined
+            *I = *sigma = *chi2_dof = std::nan("");
+            return VEGAS_ENUMERIC;
+        }
+        if (sigma_k[k] == 0.0) any_zero = true;
+    }
     if (any_zero) {
         double acc = 0.0;
         for (int k = n_skip; k < n_iter; ++k) acc += I_k[k];

@@ -49,6 +49,13 @@ def test_host_only_entry_points(B):
     assert I == pytest.approx(1.2) and s == pytest.approx(1e-200 / np.sqrt(1.25))
     with pytest.raises(B.VegasError):
         B.vegas_combine([1.0], [1.0], n_skip=1)
+    # an iteration that ended in VEGAS_ENUMERIC (non-finite I or sigma) is not averaged away: ENUMERIC, NaN outputs
+    I, s, c = C.c_double(7.0), C.c_double(7.0), C.c_double(7.0)
+    for Ik, sk in (([1.0, 2.0], [0.1, float("nan")]), ([1.0, float("inf")], [0.1, 0.1]), ([1.0, 2.0], [0.1, -1.0])):
+        Ik, sk = np.array(Ik), np.array(sk)
+        f64p = C.POINTER(C.c_double)
+        rc = B.lib.vegas_combine(2, 0, Ik.ctypes.data_as(f64p), sk.ctypes.data_as(f64p), C.byref(I), C.byref(s), C.byref(c))
+        assert rc == B.VEGAS_ENUMERIC and np.isnan(I.value) and np.isnan(s.value) and np.isnan(c.value)
 
 
 def test_null_arguments_are_rejected(B):

@@ -460,6 +460,28 @@ def test_errors(B):
     g.close()
 
 
+def test_rejected_parameters_leave_the_grid_as_it_was(B):
+    w = _small(5)
+    g = _grid(B, w)
+    I0, s0, _, _ = g.iterate(50_000, 5, 0, w.integrand_id, 64)
+    bad = np.array(w.params, dtype=float)
+    for idx, val in ((0, 0.0), (3, bad[2]), (3, bad[2] - 1.0), (5, float("nan"))):   # M = 0; m_max = m_min; m_max < m_min; NaN
+        p = bad.copy(); p[idx] = val
+        with pytest.raises(B.VegasError) as e:
+            g.set_params(w.integrand_id, p)
+        assert e.value.code == B.VEGAS_EINVAL
+        I1, s1, _, st = g.iterate(50_000, 5, 0, w.integrand_id, 64)
+        assert st == 0 and I1 == I0 and s1 == s0
+    g.close()
+    g = B.VegasGrid(4, 50)
+    g.set_params(B.VEGAS_F_GAUSS, [0.1])
+    I0, s0, _, _ = g.iterate(50_000, 1, 0, B.VEGAS_F_GAUSS, 64)
+    with pytest.raises(B.VegasError):
+        g.set_params(B.VEGAS_F_GAUSS, [-1.0])
+    assert g.iterate(50_000, 1, 0, B.VEGAS_F_GAUSS, 64)[:2] == (I0, s0)
+    g.close()
+
+
 def test_non_default_stream_and_counters(B):
     import torch
     w = _small(1)

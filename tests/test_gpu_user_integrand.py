@@ -111,6 +111,17 @@ def test_user_integrand_parameters_and_errors(B):
     oI2, oS2, oH2 = O.iterate(edges, 100_003, 5, 0, O.GENZ_DISCONTINUOUS, p2)
     assert I2 == pytest.approx(oI2, rel=RTOL64) and s2 == pytest.approx(oS2, rel=RTOL64)
     _hist_ok(H2, oH2)
+    # a source that does not compile leaves the installed kernel AND its parameters as they were
+    with pytest.raises(B.VegasError):
+        g.set_user_integrand(U.BROKEN, W.genz_discontinuous_params(6, 9))
+    I2b, s2b, _, _ = g.iterate(100_003, 5, 0, B.VEGAS_F_USER, 64)
+    assert I2b == I2 and s2b == s2
+    # a launch shape wider than the user kernel is built for (12 warps) is clamped, not launched out of bounds
+    g.set_launch(0, 512, 0, 0)
+    assert g.get_launch(B.VEGAS_F_USER, 64)["threads"] <= 384
+    I2c, s2c, _, _ = g.iterate(100_003, 5, 0, B.VEGAS_F_USER, 64)
+    assert I2c == pytest.approx(oI2, rel=RTOL64) and s2c == pytest.approx(oS2, rel=RTOL64)
+    g.set_launch(0, 0, 0, 0)
     # replacing the integrand replaces the kernel
     g.set_user_integrand(U.GENZ_PRODUCT_PEAK, W.genz_params(6, 8))
     I3, _, _, _ = g.iterate(100_003, 5, 0, B.VEGAS_F_USER, 64)
@@ -182,6 +193,14 @@ def test_user_integrand_shape_limits_and_no_parameters(B):
     assert I == pytest.approx(Iu, rel=1e-12) and s == pytest.approx(su, rel=1e-11)
     np.testing.assert_allclose(H, Hu, rtol=1e-11)
     g.close(); g2.close(); g3.close()
+
+
+def test_observable_buffer_is_zero_before_any_iteration(B):
+    g = B.VegasGrid(3, 20)
+    g.set_user_integrand(U.GENZ_PRODUCT_PEAK_WITH_OBSERVABLE, W.genz_params(3, 8))
+    g.set_observable(0.0, 1.0, 16)
+    assert np.all(g.get_observable_hist() == 0.0)
+    g.close()
 
 
 def test_observable_histogram_during_integration(B):

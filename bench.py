@@ -40,18 +40,33 @@ def n_issue(w, precision):
 
 
 def n_wide(w):
-    """32x32->64 multiplies per event: 20 per Philox block plus the split of every dimension.  The step-0
-    microbenchmark (profiles/r01_s7_ubench_pipes.md) measured 3.4 dispatch slots for IMAD.WIDE.U32, not 1:
-    the refined issue roofline charges the extra 2.4 slots ("refine them only via the
-    step-0 microbenchmarks")."""
+    """32x32->64 multiplies per event in the SURVEY count: 20 per Philox block plus the split of every dimension."""
     return 20 * ((w.dim + 3) // 4) + w.dim
 
 
-WIDE_EXTRA_SLOTS = 2.4
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE K1 launch, from the `ncu --set full` captures summarised in
-# profiles/r01_s15_head.md and r01_s14_final.md (bench.py never runs under a profiler): (workload, precision) -> bytes per launch
-NCU_TRAFFIC_BYTES = {("cfg3_gauss_d20", 64): 1.24e6, ("cfg3_gauss_d20", 32): 1.24e6, ("cfg4_genz_pp_d12", 64): 1.48e6,
-                     ("cfg5_bw_poly_d6", 64): 0.41e6}
+# Refined machine model from the round-2 microbenchmarks (profiles/r02_ubench_pipes.md; SURVEY.md 8(d): "refine them
+# only via the step-0 microbenchmarks"): IMAD.WIDE.U32 runs at 32 lanes/clk/SM (4 clk per warp instruction on the one
+# fma-heavy pipe of a scheduler), IMAD at 64, LOP3/IADD3/SEL at 64 (ALU pipe), one instruction issued per clock.
+# The refined bound per event is the largest of: issue slots (N_issue), fma-heavy clocks (4 N_wide + 2 N_imad) and
+# ALU clocks (2 N_alu), with N_imad = d (table address) and N_alu = 20 ceil(d/4) (XORs) + 2 ceil(d/4) + 3 d + 3.
+def refined_slots(w, precision):
+    d, nblk = w.dim, (w.dim + 3) // 4
+    fma_heavy = 4 * n_wide(w) + 2 * d
+    alu = 2 * (20 * nblk + 2 * nblk + 3 * d + 3)
+    return max(n_issue(w, precision), fma_heavy, alu), {"issue": n_issue(w, precision), "fma_heavy_clk": fma_heavy, "alu_clk": alu}
+
+
+def ncu_traffic(workload, precision):
+    """DRAM bytes per K1 launch from the committed `ncu --set full` summary (profiles/r02_traffic.json), with its source."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r02_traffic.json")) as fh:
+            t = json.load(fh)
+        e = t["entries"].get("%s/%d" % (workload, precision))
+        if e:
+            return e["dram_bytes_per_launch"], {"source": t["source"], "commit": t["commit"], "events_per_launch": e["events_per_launch"]}
+    except Exception:
+        pass
+    return None, None
 
 
 def n_fp(w, precision):
@@ -69,48 +84,60 @@ def measured_peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
-    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
-         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-         "clocks_event_reasons.sw_power_cap")
+    """SM clock, power and throttle reasons polled through NVML every 2 ms in a thread (nvidia-smi's 100 ms loop
+    cannot witness a 2.5 ms step); windows are cut out of the one sample stream by perf_counter time stamps."""
+    PERIOD_S = 0.002
 
     def __init__(self, gpu_index):
-        self.gpu, self.rows, self.proc = gpu_index, [], None
+        self.gpu, self.rows, self.stop_flag, self.thread, self.smax = gpu_index, [], False, None, None
 
     def start(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
-                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            threading.Thread(target=self._read, daemon=True).start()
+            import pynvml as N
+            N.nvmlInit()
+            idx = self.gpu
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            if vis:
+                try:
+                    idx = int(vis.split(",")[self.gpu])
+                except Exception:
+                    idx = self.gpu
+            h = N.nvmlDeviceGetHandleByIndex(idx)
+            self.smax = float(N.nvmlDeviceGetMaxClockInfo(h, N.NVML_CLOCK_SM))
+            reasons = {"hw_slowdown": N.nvmlClocksEventReasonHwSlowdown, "hw_thermal_slowdown": N.nvmlClocksEventReasonHwThermalSlowdown,
+                       "sw_thermal_slowdown": N.nvmlClocksEventReasonSwThermalSlowdown, "sw_power_cap": N.nvmlClocksEventReasonSwPowerCap}
+            get_reasons = getattr(N, "nvmlDeviceGetCurrentClocksEventReasons", None) or N.nvmlDeviceGetCurrentClocksThrottleReasons
+
+            def loop():
+                while not self.stop_flag:
+                    try:
+                        clk = float(N.nvmlDeviceGetClockInfo(h, N.NVML_CLOCK_SM))
+                        pw = N.nvmlDeviceGetPowerUsage(h) / 1000.0
+                        mask = int(get_reasons(h))
+                        self.rows.append((time.perf_counter(), clk, pw, [k for k, b in reasons.items() if mask & b]))
+                    except Exception:
+                        pass
+                    time.sleep(self.PERIOD_S)
+
+            self.thread = threading.Thread(target=loop, daemon=True)
+            self.thread.start()
         except Exception:
-            self.proc = None
+            self.thread = None
 
-    def _read(self):
-        for line in self.proc.stdout:
-            self.rows.append((time.perf_counter(), [t.strip() for t in line.split(",")]))
+    def window(self, t_begin, t_end, label):
+        rows = [r for r in self.rows if t_begin <= r[0] <= t_end]
+        sm = [r[1] for r in rows]
+        smax = self.smax or (max(sm) if sm else None)
+        busy = [c for c in sm if smax and c > 0.5 * smax] or sm
+        reasons = sorted({k for r in rows for k in r[3]})
+        return {"sm_mhz": statistics.median(busy) if busy else None, "sm_max_mhz": smax, "reasons": reasons,
+                "power_w_max": max((r[2] for r in rows), default=None), "samples": len(sm),
+                "sampler": "NVML every %g ms" % (1e3 * self.PERIOD_S), "window": label}
 
-    def stop(self, t_begin=None, t_end=None):
-        """Summary of the samples taken between t_begin and t_end (perf_counter; None = all)."""
-        if self.proc:
-            self.proc.terminate()
-            try:
-                self.proc.wait(timeout=2)
-            except Exception:
-                self.proc.kill()
-        sm, smax, reasons, power = [], 0.0, set(), 0.0
-        rows = [r for t, r in self.rows if (t_begin is None or t >= t_begin) and (t_end is None or t <= t_end)]
-        for r in rows:
-            try:
-                sm.append(float(r[1])); smax = max(smax, float(r[2])); power = max(power, float(r[3]))
-            except Exception:
-                continue
-            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
-                if val.lower().startswith("active"):
-                    reasons.add(name)
-        busy = [c for c in sm if c > 0.5 * smax] or sm
-        return {"sm_mhz": statistics.median(busy) if busy else None, "sm_max_mhz": smax or None,
-                "reasons": sorted(reasons), "power_w_max": power or None, "samples": len(sm)}
+    def stop(self):
+        self.stop_flag = True
+        if self.thread:
+            self.thread.join(timeout=1)
 
 
 def cpu_baseline(w, edges, target_cpu_seconds=16.0):
@@ -177,6 +204,7 @@ def main():
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32])
     ap.add_argument("--n-events", type=int, default=0, help="override events per step per GPU")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the `workloads` array (cfg3 fp32, cfg5, cfg4 at 1e8)")
     ap.add_argument("--alpha", type=float, default=None,
                     help="override the damping exponent (0 = plain MC: the grid stays uniform; SURVEY.md 8(d) asks for "
                          "one timing on the uniform grid)")
@@ -227,154 +255,183 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    g = B.VegasGrid(w.dim, w.n_bins)
-    g.set_params(w.integrand_id, w.params)
-    if args.launch:
-        g.set_launch(*[int(v) for v in args.launch.split(",")])
-    fid = w.integrand_id
-    if args.user_integrand:
-        from paper_2002_12921_b200 import user_integrands as U
-        src = {W.GAUSS: U.GAUSS, W.GENZ_PRODUCT_PEAK: U.GENZ_PRODUCT_PEAK}[w.integrand_id]
-        g.set_user_integrand(src, w.params)
-        fid = B.VEGAS_F_USER
-    shape = g.get_launch(fid, args.precision)
-    n_step = w.n_events * world                                   # weak scaling: n_events per GPU per step
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
-
-    def step(k):
-        if world == 1:
-            # one iteration + refinement enqueued back to back, one synchronisation (vegas_integrate_from, n_iter = 1)
-            r = g.integrate(1, n_step, w.seed, w.alpha, fid, args.precision, chunk_events=w.chunk_events,
-                            first_iteration=k)
-            return r["I"], r["sigma"]
-        I, s, _, st = D.iterate_sharded(g, n_step, w.seed, k, fid, args.precision, w.chunk_events,
-                                        rank, world, want_hist=False)
-        g.refine(w.alpha)
-        return I, s
-
-    sampler = ClockSampler(local_rank)      # started early: nvidia-smi needs ~0.3 s before its first row
+    sampler = ClockSampler(local_rank)
     sampler.start()
-    k = 0
-    for _ in range(args.warmup):
-        step(k)
-        k += 1
-    # ---- timed region: K steps, device events per step (L2 flushed between steps, outside the brackets)
-    g.reset_counters()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    results = []
-    barrier()
-    t_begin = time.perf_counter()
-    t_wall = time.perf_counter()
-    for i in range(args.steps):
-        flush.zero_()
-        ev[i][0].record()
-        results.append(step(k))
-        ev[i][1].record()
-        k += 1
-    barrier()
-    t_wall = time.perf_counter() - t_wall
-    ms = sum(a.elapsed_time(b) for a, b in ev)
-    launches = g.launch_count()
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = n_step * args.steps / (ms * 1e-3)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+    peaks = measured_peaks()
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
 
-    # ---- the dominant kernel alone: the same steps again with the library's per-launch CUDA events switched on
-    # (event pairs on the caller's stream around every K1 launch; kept out of the region `value` is taken from)
-    k1_steps = min(args.steps, 50)
-    g.set_profiling(True)
-    g.reset_counters()
-    evk = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(k1_steps)]
-    for i in range(k1_steps):
-        flush.zero_()
-        evk[i][0].record()
-        step(k)
-        evk[i][1].record()
-        k += 1
-    barrier()
-    k1_ms, k1_launches = g.kernel_time_ms()
-    k1_region_ms = sum(a.elapsed_time(b) for a, b in evk)
-    g.set_profiling(False)
+    def measure(w, precision, steps, warmup, label, with_cpu_baseline=False):
+        """Warm-up (the chain's first iterations adapt the grid), `steps` device-timed steps, the same steps with the
+        library's per-launch events (K1 alone), and the same steps end to end through the C ABI with host buffers."""
+        g = B.VegasGrid(w.dim, w.n_bins)
+        g.set_params(w.integrand_id, w.params)
+        if args.launch:
+            g.set_launch(*[int(v) for v in args.launch.split(",")])
+        fid = w.integrand_id
+        if args.user_integrand:
+            from paper_2002_12921_b200 import user_integrands as U
+            src = {W.GAUSS: U.GAUSS, W.GENZ_PRODUCT_PEAK: U.GENZ_PRODUCT_PEAK}[w.integrand_id]
+            g.set_user_integrand(src, w.params)
+            fid = B.VEGAS_F_USER
+        shape = g.get_launch(fid, precision)
+        n_step = w.n_events * world                                   # weak scaling: n_events per GPU per step
 
-    # ---- e2e: the same step through the C ABI with HOST buffers (edges in, I/sigma/hist/edges out)
-    edges_host = g.get_edges()
+        def step(k):
+            if world == 1:
+                # one iteration + refinement, ONE launch (vegas_integrate_from, n_iter = 1), one synchronisation
+                r = g.integrate(1, n_step, w.seed, w.alpha, fid, precision, chunk_events=w.chunk_events, first_iteration=k)
+                return r["I"], r["sigma"]
+            I, s, _, st = D.iterate_sharded(g, n_step, w.seed, k, fid, precision, w.chunk_events, rank, world, want_hist=False)
+            g.refine(w.alpha)
+            return I, s
 
-    def e2e_step(k, edges_host):
-        g.set_edges(edges_host)
+        k = 0
+        for _ in range(warmup):
+            step(k)
+            k += 1
+        # ---- timed region: `steps` steps, device events per step (L2 flushed between steps, outside the brackets)
+        g.reset_counters()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        results = []
+        barrier()
+        t_begin = time.perf_counter()
+        for i in range(steps):
+            flush.zero_()
+            ev[i][0].record()
+            results.append(step(k))
+            ev[i][1].record()
+            k += 1
+        barrier()
+        t_wall = time.perf_counter() - t_begin
+        ms = sum(a.elapsed_time(b) for a, b in ev)
+        launches = g.launch_count()
         if world > 1:
-            I, s, H, st = D.iterate_sharded(g, n_step, w.seed, k, fid, args.precision, w.chunk_events,
-                                            rank, world, want_hist=True)
-        else:
-            I, s, H, st = g.iterate(n_step, w.seed, k, fid, args.precision, w.chunk_events, want_hist=True)
-        g.refine(w.alpha, hist=H)
-        return g.get_edges()
+            t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        value = n_step * steps / (ms * 1e-3)
 
-    edges_host = e2e_step(k, edges_host)       # untimed: the stand-alone refinement kernel is loaded on its first launch
-    k += 1
-    barrier()
-    t0 = time.perf_counter()
-    for i in range(args.steps):
-        edges_host = e2e_step(k, edges_host)
+        # ---- the dominant kernel alone: the same steps again with the library's per-launch CUDA events switched on
+        # (event pairs on the caller's stream around every K1 launch; kept out of the region `value` is taken from)
+        k1_steps = min(steps, 50)
+        g.set_profiling(True)
+        g.reset_counters()
+        evk = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(k1_steps)]
+        for i in range(k1_steps):
+            flush.zero_()
+            evk[i][0].record()
+            step(k)
+            evk[i][1].record()
+            k += 1
+        barrier()
+        k1_ms, k1_launches = g.kernel_time_ms()
+        k1_region_ms = sum(a.elapsed_time(b) for a, b in evk)
+        g.set_profiling(False)
+
+        # ---- e2e: the same step through the C ABI with HOST buffers (edges in, I/sigma/hist/edges out)
+        edges_host = g.get_edges()
+
+        def e2e_step(k, edges_host):
+            g.set_edges(edges_host)
+            if world > 1:
+                I, s, H, st = D.iterate_sharded(g, n_step, w.seed, k, fid, precision, w.chunk_events, rank, world, want_hist=True)
+            else:
+                I, s, H, st = g.iterate(n_step, w.seed, k, fid, precision, w.chunk_events, want_hist=True)
+            g.refine(w.alpha, hist=H)
+            return g.get_edges()
+
+        edges_host = e2e_step(k, edges_host)       # untimed: the stand-alone refinement kernel is loaded on its first launch
         k += 1
-    barrier()
-    e2e_s = time.perf_counter() - t0
-    # clocks: samples taken during the two timed regions (device-timed steps, then the e2e steps: same kernels)
-    clocks = sampler.stop(t_begin, time.perf_counter())
-    clocks["window"] = "timed steps + e2e steps"
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    nent = w.dim * w.n_bins
-    h2d = 8 * w.dim * (w.n_bins + 1) + 8 * nent + 8 * B.VEGAS_MAX_PARAMS   # edges + hist for refine + by-value params
-    d2h = 24 + 8 * nent + 8 * w.dim * (w.n_bins + 1) + 4
+        barrier()
+        t0 = time.perf_counter()
+        for i in range(steps):
+            edges_host = e2e_step(k, edges_host)
+            k += 1
+        barrier()
+        t_end = time.perf_counter()
+        e2e_s = t_end - t0
+        clocks = sampler.window(t_begin, t_end, "%s: timed steps + K1 steps + e2e steps" % label)
+        if world > 1:
+            t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e_s = float(t.item())
+        nent = w.dim * w.n_bins
+        h2d = 8 * w.dim * (w.n_bins + 1) + 8 * nent + 8 * B.VEGAS_MAX_PARAMS   # edges + hist for refine + by-value params
+        d2h = 24 + 8 * nent + 8 * w.dim * (w.n_bins + 1) + 4
+        out = None
+        if rank == 0:
+            clk = float(clocks["sm_mhz"] or sm_max)
+            ni, nf = n_issue(w, precision), n_fp(w, precision)
+            k1_s = (k1_ms * 1e-3) / max(1, k1_launches)
+            events_per_launch = w.n_events * k1_steps / max(1, k1_launches)   # the fast path runs the chunk loop in the kernel
+            k1_rate = events_per_launch / k1_s                         # events/s of the fused kernel alone
+            peak_instr = SM_COUNT * ISSUE_LANES * sm_max * 1e6         # thread-instructions/s at max clock
+            rs, rs_parts = refined_slots(w, precision)
+            traffic, traffic_src = ncu_traffic(w.name, precision)
+            roofline = {"bound": "alu", "kernel": ("k_iterate_rot<%s>" % shape["path"]) if shape["path"] == "rotated" else "k_iterate",
+                        "achieved": k1_rate * ni / 1e12, "peak": peak_instr / 1e12, "unit": "Tinstr/s",
+                        "frac": k1_rate * ni / peak_instr,
+                        "frac_at_measured_clock": k1_rate * ni / (SM_COUNT * ISSUE_LANES * clk * 1e6),
+                        "peak_source": "148 SMs x 128 issue lanes x sm_max_mhz of MEASURED_PEAKS.json (%s); one instruction per "
+                                       "scheduler per clock confirmed by profiles/r02_ubench_pipes.md" % ("measured" if peaks else "fallback 1965 MHz"),
+                        "instr_per_event": ni, "fp_instr_per_event": nf,
+                        "refined": {"slots_per_event": rs, "parts": rs_parts, "frac": k1_rate * rs / peak_instr,
+                                    "why": "IMAD.WIDE.U32 occupies the scheduler's one fma-heavy pipe for 4 clk, LOP3/IADD3/SEL the ALU "
+                                           "pipe for 2 (profiles/r02_ubench_pipes.md): the bound is the busiest of issue, fma-heavy, ALU"},
+                        "fp_pipe_frac": k1_rate * nf / (SM_COUNT * (FP64_LANES if precision == 64 else ISSUE_LANES) * sm_max * 1e6),
+                        "kernel_events_per_s": k1_rate, "kernel_ms_per_launch": k1_s * 1e3, "kernel_launches": int(k1_launches),
+                        "kernel_includes": "the whole iteration: event loop + reduce + finalize + refine run in the one launch",
+                        "kernel_share_of_step": k1_ms / k1_region_ms if world == 1 else None,
+                        "traffic": traffic, "traffic_source": traffic_src,
+                        "traffic_note": "algorithmic global bytes per launch = grid read + partial row write per CTA = %d" % (
+                            shape["blocks"] * 8 * (w.dim * (w.n_bins + 1) + (4 + w.dim * w.n_bins)))}
+            out = {"workload": w.name, "dtype": "f64" if precision == 64 else "f32", "value": value, "ms_per_step": ms / steps,
+                   "steps": steps, "warmup": warmup,
+                   "config": {"workload": w.name, "dim": w.dim, "n_bins": w.n_bins,
+                              "integrand": W.INTEGRAND_NAMES[w.integrand_id] + (" (user source, NVRTC)" if args.user_integrand else ""),
+                              "n_events_per_gpu_per_step": w.n_events, "chunk_events": w.chunk_events, "alpha": w.alpha,
+                              "seed": w.seed, "launch": shape,
+                              "l2": "256 MiB memset between timed steps, outside the event brackets (the path reads ~10 KB of global memory per launch)",
+                              "grid": ("uniform (alpha = 0)" if w.alpha == 0 else "adapted by the %d warm-up iterations" % warmup)},
+                   "clocks": clocks, "wall_s_timed_region": t_wall,
+                   "e2e": {"value": n_step * steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+                   "gpu_launches": int(launches), "roofline": roofline,
+                   "last_iteration": {"I": results[-1][0], "sigma": results[-1][1], "closed_form": w.closed_form}}
+            if with_cpu_baseline:
+                out["cpu_baseline"] = cpu_baseline(w, edges_host)
+        g.close()
+        return out
 
+    head = measure(w, args.precision, args.steps, args.warmup, "headline", with_cpu_baseline=(world == 1 and not args.no_cpu_baseline))
+    # the other workloads SURVEY.md 8(d) gates (>= 1e8 events per iteration): a few steps each, own clock window
+    extra = []
+    if world == 1 and not args.no_extra and args.workload == "cfg3" and args.precision == 64 and not args.n_events:
+        for cfg, prec, n_ev in ((3, 32, 0), (5, 64, 0), (4, 64, 100_000_000)):
+            we = W.config(cfg)
+            if n_ev:
+                we = we.scaled(n_ev)
+            r = measure(we, prec, max(3, min(args.steps, 10)), max(args.warmup, 4), "%s/%d" % (we.name, prec))
+            if r:
+                extra.append({"workload": r["workload"], "dtype": r["dtype"], "n_events": we.n_events, "chunk_events": we.chunk_events,
+                              "value": r["value"], "e2e": r["e2e"]["value"], "ms_per_step": r["ms_per_step"], "steps": r["steps"],
+                              "kernel_ms_per_launch": r["roofline"]["kernel_ms_per_launch"],
+                              "kernel_events_per_s": r["roofline"]["kernel_events_per_s"],
+                              "roofline_frac": r["roofline"]["frac"], "refined_frac": r["roofline"]["refined"]["frac"],
+                              "instr_per_event": r["roofline"]["instr_per_event"], "launch": r["config"]["launch"],
+                              "clocks": r["clocks"], "last_iteration": r["last_iteration"]})
+    sampler.stop()
     if rank == 0:
-        peaks = measured_peaks()
-        sm_max = float(peaks.get("sm_max_mhz", 1965.0))
-        clk = float(clocks["sm_mhz"] or sm_max)
-        ni, nf = n_issue(w, args.precision), n_fp(w, args.precision)
-        k1_s = (k1_ms * 1e-3) / max(1, k1_launches)
-        events_per_launch = w.n_events * k1_steps / max(1, k1_launches)   # the fast path runs the chunk loop in the kernel
-        k1_rate = events_per_launch / k1_s                         # events/s of the fused kernel alone
-        peak_instr = SM_COUNT * ISSUE_LANES * sm_max * 1e6         # thread-instructions/s at max clock
-        roofline = {"bound": "alu", "kernel": "k_iterate",
-                    "achieved": k1_rate * ni / 1e12, "peak": peak_instr / 1e12, "unit": "Tinstr/s",
-                    "frac": k1_rate * ni / peak_instr,
-                    "frac_at_measured_clock": k1_rate * ni / (SM_COUNT * ISSUE_LANES * clk * 1e6),
-                    "peak_source": "148 SMs x 128 issue lanes x sm_max_mhz of MEASURED_PEAKS.json (%s); issue rate "
-                                   "confirmed by profiles/r01_s7_ubench_pipes.md" % ("measured" if peaks else "fallback 1965 MHz"),
-                    "instr_per_event": ni, "fp_instr_per_event": nf,
-                    "refined": {"slots_per_event": ni + WIDE_EXTRA_SLOTS * n_wide(w),
-                                "frac": k1_rate * (ni + WIDE_EXTRA_SLOTS * n_wide(w)) / peak_instr,
-                                "frac_at_measured_clock": k1_rate * (ni + WIDE_EXTRA_SLOTS * n_wide(w)) / (SM_COUNT * ISSUE_LANES * clk * 1e6),
-                                "why": "IMAD.WIDE.U32 holds the dispatch port 3.4 clk (profiles/r01_s7_ubench_pipes.md)"},
-                    "fp_pipe_frac": k1_rate * nf / (SM_COUNT * (FP64_LANES if args.precision == 64 else ISSUE_LANES) * sm_max * 1e6),
-                    "kernel_events_per_s": k1_rate, "kernel_ms_per_launch": k1_s * 1e3, "kernel_launches": int(k1_launches),
-                    "kernel_share_of_step": k1_ms / k1_region_ms if world == 1 else None,
-                    "traffic": NCU_TRAFFIC_BYTES.get((w.name, args.precision)),
-                    "traffic_note": "DRAM bytes per K1 launch (ncu, profiles/r01_s14_final.md); algorithmic global bytes "
-                                    "per launch = grid read + partial row read/write per CTA = %d" % (
-                                        shape["blocks"] * 8 * (w.dim * (w.n_bins + 1) + 2 * (4 + w.dim * w.n_bins)))}
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
-                "vs_baseline": None, "dtype": "f64" if args.precision == 64 else "f32", "data": "synthetic",
-                "config": {"workload": w.name, "dim": w.dim, "n_bins": w.n_bins, "integrand": W.INTEGRAND_NAMES[w.integrand_id] + (" (user source, NVRTC)" if args.user_integrand else ""),
-                           "n_events_per_gpu_per_step": w.n_events, "chunk_events": w.chunk_events, "alpha": w.alpha,
-                           "seed": w.seed, "launch": shape, "l2": "256 MiB memset between timed steps, outside the event brackets "
-                           "(the path reads ~10 KB of global memory per launch)",
-                           "grid": ("uniform (alpha = 0)" if w.alpha == 0 else "adapted by the %d warm-up iterations" % args.warmup)},
-                "clocks": clocks, "wall_s_timed_region": t_wall,
-                "e2e": {"value": n_step * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
-                "gpu_launches": int(launches),
-                "roofline": roofline,
-                "last_iteration": {"I": results[-1][0], "sigma": results[-1][1], "closed_form": w.closed_form}}
-        if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(w, edges_host)
+        line = {"metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": head["dtype"], "data": "synthetic", "config": head["config"],
+                "clocks": head["clocks"], "wall_s_timed_region": head["wall_s_timed_region"], "e2e": head["e2e"],
+                "gpu_launches": head["gpu_launches"], "roofline": head["roofline"], "last_iteration": head["last_iteration"]}
+        if "cpu_baseline" in head:
+            line["cpu_baseline"] = head["cpu_baseline"]
+        if extra:
+            line["workloads"] = extra
         print(json.dumps(line))
-    g.close()
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()

@@ -10,6 +10,7 @@
 #include <stdint.h>
 #include <stdio.h>
 #include <stdlib.h>
+#include <string.h>
 
 #define CHECK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { \
     fprintf(stderr, "%s: %s\n", #x, cudaGetErrorString(e_)); exit(1); } } while (0)
@@ -230,6 +231,7 @@ __global__ void k_ring(Stamp* out, int work, double a) {
 
 static Stamp* d_out;
 static int n_sm;
+static void philox_section();
 
 static void report_alu(const char* name, int ops_per_chain_step, int threads = THREADS) {
     Stamp h[1024];
@@ -253,12 +255,107 @@ static void report_smem(const char* name, double warp_accesses_per_thread, int t
            cyc / (warp_accesses_per_thread * (threads / 32)), 1e3 * cyc / ns);
 }
 
-int main() {
+
+// ---- round 2: Philox-shaped instruction mixes (profiles/r02_ubench_pipes.md) ---------------------------------------
+// NB independent Philox4x32 round chains per thread (one round = 2 IMAD.WIDE.U32 + 2 three-input LOP3, as in K1's
+// event loop), plus, per round, XD independent DFMA, XL independent LOP3 and XI independent IMAD (32-bit low) on
+// chains of their own: what does a round cost per warp on one scheduler, and which extras hide under the multiplies?
+template <int NB, int XD, int XL, int XI>
+__global__ void __launch_bounds__(THREADS) k_philox_mix(Stamp* out, uint32_t k0, uint32_t k1, double da, uint32_t la, int rounds) {
+    uint32_t pc0[NB], pc1[NB], pc2[NB], pc3[NB];
+    double z[XD > 0 ? XD : 1];
+    uint32_t y[XL > 0 ? XL : 1], q[XI > 0 ? XI : 1];
+#pragma unroll
+    for (int b = 0; b < NB; ++b) { pc0[b] = b; pc1[b] = threadIdx.x; pc2[b] = blockIdx.x * 977u + b; pc3[b] = 7u * b; }
+#pragma unroll
+    for (int k = 0; k < (XD > 0 ? XD : 1); ++k) z[k] = k + 0.5;
+#pragma unroll
+    for (int k = 0; k < (XL > 0 ? XL : 1); ++k) y[k] = threadIdx.x + k;
+#pragma unroll
+    for (int k = 0; k < (XI > 0 ? XI : 1); ++k) q[k] = threadIdx.x * 3u + k;
+    BENCH_PROLOG
+#pragma unroll 2
+    for (int r = 0; r < rounds; ++r) {
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            const uint64_t p0 = (uint64_t)0xD2511F53u * pc0[b], p1 = (uint64_t)0xCD9E8D57u * pc2[b];
+            const uint32_t n0 = (uint32_t)(p1 >> 32) ^ pc1[b] ^ k0, n2 = (uint32_t)(p0 >> 32) ^ pc3[b] ^ k1;
+            pc1[b] = (uint32_t)p1; pc3[b] = (uint32_t)p0; pc0[b] = n0; pc2[b] = n2;
+        }
+#pragma unroll
+        for (int k = 0; k < XD; ++k) z[k] = fma(z[k], da, 1.0);
+#pragma unroll
+        for (int k = 0; k < XL; ++k) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(y[k]) : "r"(la), "r"(k0));
+#pragma unroll
+        for (int k = 0; k < XI; ++k) asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(q[k]) : "r"(la), "r"(k1));
+    }
+    uint32_t s = 0;
+#pragma unroll
+    for (int b = 0; b < NB; ++b) s ^= pc0[b] ^ pc1[b] ^ pc2[b] ^ pc3[b];
+    for (int k = 0; k < (XD > 0 ? XD : 1); ++k) s ^= (uint32_t)__double2loint(z[k]);
+    for (int k = 0; k < (XL > 0 ? XL : 1); ++k) s ^= y[k];
+    for (int k = 0; k < (XI > 0 ? XI : 1); ++k) s ^= q[k];
+    BENCH_EPILOG(s)
+}
+
+// pure IMAD.WIDE.U32 with a 64-bit accumulate (no other instruction in the chain step)
+__global__ void __launch_bounds__(THREADS) k_wide_acc(Stamp* out, uint32_t m) {
+    uint64_t x[UNR];
+    for (int u = 0; u < UNR; ++u) x[u] = threadIdx.x * 2654435761u + u;
+    BENCH_PROLOG
+    for (int i = 0; i < ITER; ++i)
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) x[u] = (uint64_t)(uint32_t)x[u] * m + x[u];
+    uint32_t s = 0; for (int u = 0; u < UNR; ++u) s ^= (uint32_t)x[u] ^ (uint32_t)(x[u] >> 32);
+    BENCH_EPILOG(s)
+}
+
+static void report_round(const char* name, int threads, int rounds, int nb) {
+    Stamp h[1024];
+    CHECK(cudaDeviceSynchronize());
+    CHECK(cudaMemcpy(h, d_out, sizeof(Stamp) * n_sm, cudaMemcpyDeviceToHost));
+    double cyc = 0; for (int i = 0; i < n_sm; ++i) cyc += (double)h[i].cycles; cyc /= n_sm;
+    // a scheduler serves threads/128 warps; each runs rounds * nb Philox rounds
+    printf("%-66s %6.2f clk per Philox round per warp per scheduler\n", name, cyc / ((double)rounds * nb * (threads / 128)));
+}
+template <int NB, int XD, int XL, int XI>
+static void run_mix(int threads, const char* what) {
+    const int rounds = 8192;
+    char nm[160];
+    k_philox_mix<NB, XD, XL, XI><<<n_sm, threads>>>(d_out, 0x9E3779B9u, 0xBB67AE85u, 1.0000001, 0x5bd1e995u, rounds);
+    snprintf(nm, sizeof nm, "%d warps/scheduler, %d blocks: round%s", threads / 128, NB, what);
+    report_round(nm, threads, rounds, NB);
+}
+static void philox_section() {
+    printf("# Philox-shaped mixes: one round = 2 IMAD.WIDE.U32 + 2 LOP3 per block; extras are per ROUND OF ALL BLOCKS / NB, i.e. per block-round\n");
+    for (int threads : {256, 512, 768, 1024}) {
+        run_mix<5, 0, 0, 0>(threads, "");
+        run_mix<5, 5, 0, 0>(threads, " + 1 DFMA");
+        run_mix<5, 10, 0, 0>(threads, " + 2 DFMA");
+        run_mix<5, 20, 0, 0>(threads, " + 4 DFMA");
+        run_mix<5, 0, 5, 0>(threads, " + 1 LOP3");
+        run_mix<5, 0, 10, 0>(threads, " + 2 LOP3");
+        run_mix<5, 0, 20, 0>(threads, " + 4 LOP3");
+        run_mix<5, 0, 0, 5>(threads, " + 1 IMAD");
+        run_mix<5, 0, 0, 10>(threads, " + 2 IMAD");
+        run_mix<5, 10, 10, 0>(threads, " + 2 DFMA + 2 LOP3");
+        run_mix<5, 10, 20, 5>(threads, " + 2 DFMA + 4 LOP3 + 1 IMAD");
+    }
+    k_wide_acc<<<n_sm, THREADS>>>(d_out, 0xD2511F53u);
+    report_alu("IMAD.WIDE.U32 with 64-bit accumulate, alone", 1);
+}
+
+int main(int argc, char** argv) {
     cudaDeviceProp prop;
     CHECK(cudaGetDeviceProperties(&prop, 0));
     n_sm = prop.multiProcessorCount;
     printf("# %s, %d SMs, %zu KB shared/SM opt-in\n", prop.name, n_sm, prop.sharedMemPerBlockOptin >> 10);
     CHECK(cudaMalloc(&d_out, sizeof(Stamp) * 1024));
+    if (argc > 1 && !strcmp(argv[1], "philox")) {       // the round-2 section alone (what the ncu capture runs)
+        philox_section();
+        CHECK(cudaFree(d_out));
+        return 0;
+    }
     for (int rep = 0; rep < 2; ++rep) {          // first pass warms clocks up
         if (rep) printf("# ALU pipes: one 1024-thread CTA per SM, %d independent chains per thread\n", UNR);
         k_ffma<<<n_sm, THREADS>>>(d_out, 1.0001f, 0.5f);              if (rep) report_alu("FFMA", 1);
@@ -276,6 +373,7 @@ int main() {
         k_i2f64<<<n_sm, THREADS>>>(d_out, 0x55555555u);               if (rep) report_alu("I2F.F64.U32 (+1 LOP3 each)", 1);
         k_mant64<<<n_sm, THREADS>>>(d_out, 0x55555555u);              if (rep) report_alu("mantissa build (SHF+LOP/IMAD+LOP3)", 1);
     }
+    philox_section();
     printf("# shared memory, random rows\n");
     for (int rows : {50, 250}) {
         char nm[128];

@@ -188,7 +188,7 @@ bool use_rot_path(const vegas_grid* g, int fid, int precision) {
 
 // shift_j, scale_j, post_scale, fin0 of the affine pre-composition (see vegas_iterate_rot.cuh)
 void rot_constants(const vegas_grid* g, int fid, int precision, double* shift, double* scale, double* post_scale,
-                   double* fin0, double* fin1, double* jac_init, double* fpar) {
+                   double* fin0, double* fin1, double* jac_init, double* fpar, bool word_map) {
     const int dim = g->dim;
     const double nb = (double)g->n_bins;
     *post_scale = 1.0;
@@ -249,6 +249,10 @@ void rot_constants(const vegas_grid* g, int fid, int precision, double* shift, d
         const int h = dim / 2;
         *jac_init = std::ldexp(1.0, 32 * h);
         *post_scale *= std::ldexp(1.0, 32 * (dim - h));
+        // the fast path's fp64 table entries are affine in the whole Philox word (RotEntry<double>::make_w): their
+        // slope, the Jacobian factor, carries one more n_bins per dimension
+        if (word_map)
+            for (int j = 0; j < dim; ++j) *post_scale /= nb;
     }
 }
 
@@ -625,7 +629,8 @@ int accumulate_impl(vegas_grid* g, uint64_t first_event, uint64_t count, uint64_
         ra.n_bins = g->n_bins;
         ra.n_groups = rs.n_groups;
         ra.ring = rs.ring;
-        rot_constants(g, fid, precision, ra.shift, ra.scale, &ra.post_scale, &ra.fin0, &ra.fin1, &ra.jac_init, ra.fpar);
+        rot_constants(g, fid, precision, ra.shift, ra.scale, &ra.post_scale, &ra.fin0, &ra.fin1, &ra.jac_init, ra.fpar,
+                      vegas::rot_word_map(precision == VEGAS_FP64 ? 64 : 32, g->dim));
         if (fid == VEGAS_F_USER && g->n_obs > 0) {
             ra.obs = g->d_obs;
             ra.n_obs = g->n_obs;
@@ -647,7 +652,7 @@ int accumulate_impl(vegas_grid* g, uint64_t first_event, uint64_t count, uint64_
         a.jac_scale = jac_scale_for(g, precision);
         if (fid != VEGAS_F_BW_POLY) {
             double fpar_unused[vegas::kRotParams];
-            rot_constants(g, fid, precision, a.shift, a.scale, &a.post_scale, &a.fin0, &a.fin1, &a.jac_init, fpar_unused);
+            rot_constants(g, fid, precision, a.shift, a.scale, &a.post_scale, &a.fin0, &a.fin1, &a.jac_init, fpar_unused, false);
         }
     }
     // The fast path runs the chunk loop inside the kernel (one launch per accumulate call: the grid finishes a chunk
@@ -870,7 +875,8 @@ int vegas_debug_sample(vegas_grid* g, uint64_t first_event, uint32_t count, uint
     a.fJ = (double*)base;
     // both K1 kernels form u_j, f and v through the affine map for every integrand but BW_POLY beyond the fast path
     const bool rot = fid != VEGAS_F_BW_POLY || use_rot_path(g, fid, precision);
-    if (rot) rot_constants(g, fid, precision, a.shift, a.scale, &a.post_scale, &a.fin0, &a.fin1, &a.jac_init, a.fpar);
+    a.word_map = rot && vegas::rot_word_map(precision == VEGAS_FP64 ? 64 : 32, g->dim);
+    if (rot) rot_constants(g, fid, precision, a.shift, a.scale, &a.post_scale, &a.fin0, &a.fin1, &a.jac_init, a.fpar, a.word_map != 0);
     CUDA_TRY(g, vegas::launch_debug(fid, precision, rot, a, g->derived[fid], st));
     g->launches++;
     if (words) CUDA_TRY(g, cudaMemcpyAsync(words, a.words, per_dim * 4, cudaMemcpyDeviceToHost, st));

@@ -149,6 +149,7 @@ template <> struct RotEntry<double> {
     // u = scale (X_b + Delta r - shift), r = (w + 1/2) 2^-32  ==>  u = A + B' w with
     // B' = scale Delta 2^-32 (exact scaling) and A = scale (X_b - shift) + B'/2.  The Jacobian factor is
     // B' 2^32 / scale; the 2^32 per dimension goes into post_scale (vegas_api.cu: rot_constants).
+    // (the generic kernel's form: w is the low word of the split product)
     static __device__ __forceinline__ double2 make(double x0, double x1, double shift, double scale) {
         const double B = (x1 - x0) * scale, A = (x0 - shift) * scale;
         return make_double2(fma(B, 1.1641532182693481e-10, A), B * 2.3283064365386963e-10);   // 2^-33, 2^-32
@@ -157,6 +158,18 @@ template <> struct RotEntry<double> {
         return fma(e.y, (double)lo, e.x);              // I2F.F64.U32 (its own pipe) + DFMA
     }
     static constexpr double kJacUnit = 4294967296.0;   // table B = kJacUnit^-1 * scale * Delta
+    // The fast path's form: u as an affine function of the WHOLE Philox word W of the dimension, per bin b.
+    // With P = W n_bins, b = P >> 32 and lo = P - b 2^32 (C3), r = (lo + 1/2) 2^-32 = W n_bins 2^-32 - b + 2^-33, so
+    //   u = A_b + B_b W,   B_b = scale Delta n_bins 2^-32,   A_b = scale (X_b - shift) + scale Delta (2^-33 - b).
+    // The split needs no integer multiply then (IMAD.WIDE.U32 costs 3.4..4.4 issue clocks on sm_100a, a DFMA 1.3..2:
+    // profiles/r02_ubench_pipes.md): with Wd = (double)W, t = RZ(Wd n_bins 2^-32 + 2^52) has b = floor(P 2^-32) in its
+    // low word -- exactly, the sum is formed exactly before the one rounding towards zero -- and u = fma(B_b, Wd, A_b).
+    // A_b + B_b W cancels Delta b, so u carries an absolute error of ~1.5e-16 scale (x_j within ~3e-16 absolute of
+    // the plain map instead of 1 ulp; reading R21); the Jacobian factor B_b is a product of exact values.
+    static __device__ __forceinline__ double2 make_w(double x0, double x1, double shift, double scale, int b, int n_bins) {
+        const double B = (x1 - x0) * scale, A = (x0 - shift) * scale;
+        return make_double2(fma(B, 1.1641532182693481e-10 - (double)b, A), B * ((double)n_bins * 2.3283064365386963e-10));
+    }
 };
 template <> struct RotEntry<float> {
     using type = float2;
@@ -170,6 +183,39 @@ template <> struct RotEntry<float> {
         return fmaf(e.y, m, e.x);
     }
     static constexpr double kJacUnit = 1.0;
+};
+
+// C3 + C4 on the fast path: word -> (bin, operand of the table entry's affine map), and the entry itself.  Bins are
+// bit-exact in both forms.  WORD (fp64 only): the entry is affine in the whole word (RotEntry<double>::make_w).
+// It pays where the kernel is bound by its instruction stream (more than 8 dimensions: cfg3 +1 %, cfg4 +5 %); the
+// small shapes are latency-bound and lose (cfg5 -7 %), they keep the integer split.
+#ifndef VEGAS_ROT_WORD_MIN_DIM
+#define VEGAS_ROT_WORD_MIN_DIM 9
+#endif
+__host__ __device__ constexpr bool rot_word_map(int precision_bits, int dim) {
+    return precision_bits == 64 && dim >= VEGAS_ROT_WORD_MIN_DIM;
+}
+template <typename T, bool WORD> struct RotSplit;
+template <> struct RotSplit<double, true> {
+    using arg = double;                                  // the word itself as a double (I2F.F64.U32, exact)
+    static __device__ __forceinline__ void split(uint32_t w, uint32_t, double nb_2m32, uint32_t& b, double& o) {
+        o = (double)w;
+        b = (uint32_t)__double2loint(__fma_rz(o, nb_2m32, 4503599627370496.0));       // 2^52 + floor(w n_bins 2^-32)
+    }
+    static __device__ __forceinline__ double u(double2 e, double o) { return fma(e.y, o, e.x); }
+    static __device__ __forceinline__ double2 make(double x0, double x1, double shift, double scale, int b, int nb) {
+        return RotEntry<double>::make_w(x0, x1, shift, scale, b, nb);
+    }
+};
+template <typename T> struct RotSplit<T, false> {
+    using arg = uint32_t;                                // the low word of the product (fp32, C11: its top 23 bits are used)
+    static __device__ __forceinline__ void split(uint32_t w, uint32_t nb, double, uint32_t& b, uint32_t& o) {
+        split_word(w, nb, b, o);
+    }
+    static __device__ __forceinline__ T u(typename RotEntry<T>::type e, uint32_t o) { return RotEntry<T>::u(e, o); }
+    static __device__ __forceinline__ typename RotEntry<T>::type make(double x0, double x1, double shift, double scale, int, int) {
+        return RotEntry<T>::make(x0, x1, shift, scale);
+    }
 };
 
 // 32-bit shared-window addressing: one register per address, no generic-to-shared conversion
@@ -367,17 +413,18 @@ __device__ __forceinline__ int rot_gamma(int lane) {
     return (lane & 7) >> (3 - LG);
 }
 
-// per-thread constants of the event loop.  Addresses are 32-bit shared-window addresses.
-//   table entry of (blk, bin, sub-step i):  taddr = tbase + (blk nb + bin) 128 + tx[i]
-//   histogram word of the same:             haddr = hbase + (blk nb + bin) 256 + hx[i] = 2 taddr + hc[i]
-// so the histogram address costs one LEA from the table address kept in a register (no bin packing).
+// per-thread constants of the event loop.  Addresses are 32-bit shared-window addresses; rows are ordered
+// [bin][Philox block], so the block enters every address as a compile-time immediate:
+//   table entry of (blk, bin, sub-step i):  taddr + 128 blk,  taddr = bin (128 NBLK) + tx[i]   (tx includes the base)
+//   histogram word of the same:             haddr + 256 blk,  haddr = 2 taddr + hc[i]
+// one multiply-add and one three-input add per dimension, no per-block base to add.
 template <typename T, int DIM>
 struct RotLane {
     static constexpr int NBLK = (DIM + 3) / 4;
     static constexpr int R = DIM - 4 * (NBLK - 1);               // dimensions in the last block, 1..4
     static constexpr int GL = rot_groups(R);
     uint32_t tbase;
-    uint32_t tx4[4], txL[4];      // full blocks / last block: row offset of sub-step i (lane-dependent)
+    uint32_t tx4[4], txL[4];      // full blocks / last block: table base + row offset of sub-step i (lane-dependent)
     uint32_t hc4[4], hcL[4];      // haddr - 2 taddr
     int gamma4, gammaL;
 };
@@ -406,9 +453,11 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
                                             const RotCtx<FID, T, (DIM + 3) / 4>& ctx, uint32_t e_lo, uint32_t e_hi,
                                             bool live, T fin0, T fin1, uint32_t (&haddr)[(DIM + 3) / 4][4], double& obs_val) {
     using E = RotEntry<T>;
+    using SP = RotSplit<T, rot_word_map(8 * (int)sizeof(T), DIM)>;
     using T2 = typename E::type;
     constexpr int NBLK = RotLane<T, DIM>::NBLK, R = RotLane<T, DIM>::R, GL = RotLane<T, DIM>::GL;
     const int nb = a.n_bins;
+    const double nb_2m32 = (double)nb * 2.3283064365386963e-10;
     constexpr int NCH = rot_chains(DIM, FID, sizeof(T) == 4);
     IntegrandU<FID, T, NCH> f;
     f.begin(ctx);
@@ -434,8 +483,7 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
             w[0] = t0; w[1] = t1;
         }
         // the block's table reads are issued together, then consumed (their latency overlaps)
-        const uint32_t tblk = L.tbase + (uint32_t)(blk * nb) * 128u;
-        uint32_t lo[4];
+        typename SP::arg lo[4];
         T2 ent[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
@@ -446,13 +494,12 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
                 lo[i] = 0;
                 ent[i] = T2{};
                 if (active) {
-                    split_word(w[i], (uint32_t)nb, b, lo[i]);
-                    // one multiply-add (ptxas: LEA/IMAD); written in C the compiler folds the shift into a
-                    // 64-bit funnel shift of the product plus a mask plus an add
+                    SP::split(w[i], (uint32_t)nb, nb_2m32, b, lo[i]);
+                    // one multiply-add (written in C the compiler turns it into shifts and masks of the split product)
                     uint32_t taddr;
-                    asm("mad.lo.u32 %0, %1, 128, %2;" : "=r"(taddr) : "r"(b), "r"(tblk + (last ? L.txL[i] : L.tx4[i])));
-                    ent[i] = lds_entry<T2>(taddr);
-                    haddr[blk][i] = 2u * taddr + (last ? L.hcL[i] : L.hc4[i]);
+                    asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(taddr) : "r"(b), "n"(NBLK * 128), "r"(last ? L.txL[i] : L.tx4[i]));
+                    ent[i] = lds_entry<T2>(taddr + (uint32_t)(blk * 128));        // [R + immediate]
+                    haddr[blk][i] = 2u * taddr + (last ? L.hcL[i] : L.hc4[i]);    // + 256 blk at the point of use
                 }
             }
         }
@@ -461,7 +508,7 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
             const bool active = !(last && R == 3) || ((gamma ^ i) < 3);
             if (active) {
                 jac[i & (NCH - 1)] *= ent[i].y;
-                f.dim(E::u(ent[i], lo[i]), blk, i, ctx);
+                f.dim(SP::u(ent[i], lo[i]), blk, i, ctx);
             }
         }
     }
@@ -496,14 +543,14 @@ __device__ __forceinline__ void rot_hist_update(const uint32_t (&haddr)[(DIM + 3
             const bool last = (blk == NBLK - 1);
             const int NSUB = last ? ((R == 3) ? 4 : R) : 4;
             const bool active = (i < NSUB) && (!(last && R == 3) || ((gammaL ^ i) < 3));
-            if (active) h[blk] = lds_f64(haddr[blk][i]);
+            if (active) h[blk] = lds_f64(haddr[blk][i] + (uint32_t)(blk * 256));
         }
 #pragma unroll
         for (int blk = B0; blk < B1; ++blk) {
             const bool last = (blk == NBLK - 1);
             const int NSUB = last ? ((R == 3) ? 4 : R) : 4;
             const bool active = (i < NSUB) && (!(last && R == 3) || ((gammaL ^ i) < 3));
-            if (active) sts_f64(haddr[blk][i], h[blk] + v2);
+            if (active) sts_f64(haddr[blk][i] + (uint32_t)(blk * 256), h[blk] + v2);
         }
         __syncwarp();
     }
@@ -618,14 +665,14 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
         __syncthreads();
         for (int idx = threadIdx.x; idx < rows * (128 / ENTRY); idx += blockDim.x) {
             const int row = idx / (128 / ENTRY), e = idx - row * (128 / ENTRY);   // entry e of the row
-            const int blk = row / nb, b = row - blk * nb;
+            const int b = row / NBLK, blk = row - b * NBLK;                       // rows are ordered [bin][block]
             const int G = (blk < NBLK - 1) ? 4 : GL;
             const int slot = e / ((128 / ENTRY) / G);
             const int j = 4 * blk + slot;
             T2 ent = T2{};
             if (j < DIM) {
                 const double* X = stage_e + j * (nb + 1);
-                ent = E::make(X[b], X[b + 1], a.shift[j], a.scale[j]);
+                ent = RotSplit<T, rot_word_map(8 * (int)sizeof(T), DIM)>::make(X[b], X[b + 1], a.shift[j], a.scale[j], b, nb);
             }
             reinterpret_cast<T2*>(table)[idx] = ent;
         }
@@ -650,10 +697,10 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
         constexpr int SHL = (GL == 4) ? 5 : (GL == 2) ? 6 : 7;     // slot -> byte offset shift
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-            L.tx4[i] = toff4 ^ (uint32_t)(i << 5);
-            L.txL[i] = toffL ^ (uint32_t)(i << SHL);
-            L.hc4[i] = hbase + (hoff4 ^ (uint32_t)(i << 5)) - 2u * (L.tbase + L.tx4[i]);
-            L.hcL[i] = hbase + (hoffL ^ (uint32_t)(i << SHL)) - 2u * (L.tbase + L.txL[i]);
+            L.tx4[i] = L.tbase + (toff4 ^ (uint32_t)(i << 5));
+            L.txL[i] = L.tbase + (toffL ^ (uint32_t)(i << SHL));
+            L.hc4[i] = hbase + (hoff4 ^ (uint32_t)(i << 5)) - 2u * L.tx4[i];
+            L.hcL[i] = hbase + (hoffL ^ (uint32_t)(i << SHL)) - 2u * L.txL[i];
         }
     }
     L.gamma4 = rot_gamma<4>(lane);
@@ -775,11 +822,11 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
         for (int u = 0; u < 4; ++u) {
             const int row = row0 + u * mwarps;
             if (row >= rows) continue;                                // warp-uniform
-            const bool last = row >= (NBLK - 1) * nb;
+            const int b = row / NBLK, blk = row - b * NBLK;
+            const bool last = blk == NBLK - 1;
             const int lgp = last ? LGPL : 2;
             if (lgp >= 3) h[u] += __shfl_xor_sync(0xffffffffu, h[u], 4);
             if (lgp >= 4) h[u] += __shfl_xor_sync(0xffffffffu, h[u], 8);
-            const int blk = last ? NBLK - 1 : row / nb, b = row - blk * nb;
             const int slot = (lane & 15) >> lgp, c = lane & ((1 << lgp) - 1);
             const int j = 4 * blk + slot;
             if (lane < 16 && c == 0 && j < DIM) stage[j * nb + b] = h[u];

@@ -336,11 +336,25 @@ __global__ void k_debug_rot(const __grid_constant__ DebugArgs a) {
         if ((j & 3) == 0) philox4x32_10((uint32_t)(j >> 2), a.iteration, (uint32_t)e, (uint32_t)(e >> 32), ks, w);
         const uint32_t word = (j & 3) == 0 ? w[0] : (j & 3) == 1 ? w[1] : (j & 3) == 2 ? w[2] : w[3];
         uint32_t b, lo;
-        split_word(word, (uint32_t)nb, b, lo);
+        split_word(word, (uint32_t)nb, b, lo);                 // for the plain map below (x is reported, not used)
         const double* X = a.edges + (size_t)j * (nb + 1);
-        const typename E::type ent = E::make(X[b], X[b + 1], a.shift[j], a.scale[j]);
+        typename E::type ent;
+        T u;
+        if (sizeof(T) == 8 && a.word_map) {                   // the fast path's own split and map for this shape
+            using SW = RotSplit<double, true>;
+            uint32_t bw;
+            double o;
+            SW::split(word, (uint32_t)nb, (double)nb * 2.3283064365386963e-10, bw, o);
+            b = bw;
+            const double2 ew = SW::make(X[b], X[b + 1], a.shift[j], a.scale[j], (int)b, nb);
+            ent.x = (T)ew.x; ent.y = (T)ew.y;
+            u = (T)SW::u(ew, o);
+        } else {
+            ent = E::make(X[b], X[b + 1], a.shift[j], a.scale[j]);
+            u = E::u(ent, lo);
+        }
         jac[j & (NCH - 1)] *= ent.y;
-        f.dim(E::u(ent, lo), FID == VEGAS_F_BW_POLY ? (j >> 2) : 0, j & 3, ctx);
+        f.dim(u, FID == VEGAS_F_BW_POLY ? (j >> 2) : 0, j & 3, ctx);
         a.words[(size_t)q * dim + j] = word;
         a.bins[(size_t)q * dim + j] = (int32_t)b;
         a.x[(size_t)q * dim + j] = (sizeof(T) == 8) ? fma(X[b + 1] - X[b], offset_f64(lo), X[b])

@@ -49,6 +49,7 @@ struct DebugArgs {
     double post_scale, fin0, fin1, jac_init;
     double shift[VEGAS_MAX_DIM], scale[VEGAS_MAX_DIM];
     double fpar[64];                // RotArgs::fpar (kRotParams)
+    int word_map;                   // fp64: this shape's fast-path kernel uses the word-affine table entries (rot_word_map)
 };
 
 size_t iterate_shared_bytes(int dim, int n_bins, int precision, int table_copies, int hist_copies);

@@ -19,6 +19,8 @@ import numpy as np
 from .build import build as _build
 
 CONST, GAUSS, GENZ_PRODUCT_PEAK, BW_POLY, GENZ_DISCONTINUOUS = 0, 1, 2, 3, 4
+# variants of the sampling map (readings C3', C4'); a bit mask
+V_U53, V_Q32 = 1, 2
 OK, EINVAL, ENUMERIC = 0, -1, -3
 
 _lib = None
@@ -39,12 +41,18 @@ def lib():
         L.oracle_n_params.restype = C.c_int
         L.oracle_f.argtypes = [C.c_int, C.c_int, f64p, f64p]
         L.oracle_f.restype = C.c_double
-        L.oracle_sample.argtypes = [C.c_int, C.c_int, f64p, C.c_uint64, C.c_uint32, C.c_uint64,
-                                    C.c_uint64, C.c_int, f64p, u32p, i32p, f64p, f64p]
-        L.oracle_sample.restype = C.c_int
-        L.oracle_accumulate.argtypes = [C.c_int, C.c_int, f64p, C.c_uint64, C.c_uint32,
-                                        C.c_uint64, C.c_uint64, C.c_int, f64p, f64p, f64p, f64p]
-        L.oracle_accumulate.restype = C.c_int
+        L.oracle_word53.argtypes = [C.c_uint64, C.c_uint32, C.c_uint64, C.c_int]
+        L.oracle_word53.restype = C.c_uint64
+        L.oracle_split53.argtypes = [C.c_uint64, C.c_int, i32p, f64p]
+        L.oracle_split53.restype = None
+        L.oracle_q32.argtypes = [C.c_double]
+        L.oracle_q32.restype = C.c_double
+        L.oracle_sample_v.argtypes = [C.c_int, C.c_int, C.c_int, f64p, C.c_uint64, C.c_uint32, C.c_uint64,
+                                      C.c_uint64, C.c_int, f64p, u32p, i32p, f64p, f64p]
+        L.oracle_sample_v.restype = C.c_int
+        L.oracle_accumulate_v.argtypes = [C.c_int, C.c_int, C.c_int, f64p, C.c_uint64, C.c_uint32,
+                                          C.c_uint64, C.c_uint64, C.c_int, f64p, f64p, f64p, f64p]
+        L.oracle_accumulate_v.restype = C.c_int
         L.oracle_estimate.argtypes = [f64p, C.c_uint64, f64p, f64p]
         L.oracle_estimate.restype = C.c_int
         L.oracle_iterate.argtypes = [C.c_int, C.c_int, f64p, C.c_uint64, C.c_uint64, C.c_uint32,
@@ -56,10 +64,10 @@ def lib():
         L.oracle_combine.restype = C.c_int
         L.oracle_uniform_edges.argtypes = [C.c_int, C.c_int, f64p]
         L.oracle_uniform_edges.restype = None
-        L.oracle_integrate.argtypes = [C.c_int, C.c_int, f64p, C.c_int, C.c_int, C.c_uint64,
-                                       C.c_uint64, C.c_double, C.c_int, f64p, f64p, f64p, f64p,
-                                       f64p, f64p, f64p]
-        L.oracle_integrate.restype = C.c_int
+        L.oracle_integrate_v.argtypes = [C.c_int, C.c_int, C.c_int, f64p, C.c_int, C.c_int, C.c_uint64,
+                                         C.c_uint64, C.c_double, C.c_int, f64p, f64p, f64p, f64p,
+                                         f64p, f64p, f64p]
+        L.oracle_integrate_v.restype = C.c_int
         _lib = L
     return _lib
 
@@ -106,6 +114,23 @@ def split(w, n_bins):
     return b.value, r.value
 
 
+def word53(seed, iteration, event, j):
+    """C3': the 53-bit integer U of (seed, iteration, event, dimension j), two Philox words per draw."""
+    return int(lib().oracle_word53(int(seed), int(iteration), int(event), int(j)))
+
+
+def split53(U, n_bins):
+    """C3': U -> (bin, r) with r in [0,1)."""
+    b, r = C.c_int32(), C.c_double()
+    lib().oracle_split53(int(U), int(n_bins), C.byref(b), C.byref(r))
+    return b.value, r.value
+
+
+def q32(v):
+    """C4': a table entry rounded to fp32 and widened back."""
+    return float(lib().oracle_q32(float(v)))
+
+
 def n_params(integrand_id, dim):
     return int(lib().oracle_n_params(integrand_id, dim))
 
@@ -124,8 +149,9 @@ def uniform_edges(dim, n_bins):
     return e
 
 
-def sample(edges, seed, iteration, first_event, count, integrand_id, params=None):
-    """C2..C5 for events [first_event, first_event+count): (words, bins, x, fJ)."""
+def sample(edges, seed, iteration, first_event, count, integrand_id, params=None, variant=0):
+    """C2..C5 for events [first_event, first_event+count): (words, bins, x, fJ).
+    With V_U53 the words column holds the top 32 bits of each 53-bit U."""
     edges = _f64(edges)
     dim, nb = edges.shape[0], edges.shape[1] - 1
     p = _params(params)
@@ -133,15 +159,15 @@ def sample(edges, seed, iteration, first_event, count, integrand_id, params=None
     bins = np.zeros((count, dim), dtype=np.int32)
     x = np.zeros((count, dim))
     fJ = np.zeros(count)
-    rc = lib().oracle_sample(dim, nb, _p(edges), int(seed), int(iteration), int(first_event),
-                             int(count), integrand_id, _p(p), _p(words, C.c_uint32),
-                             _p(bins, C.c_int32), _p(x), _p(fJ))
+    rc = lib().oracle_sample_v(int(variant), dim, nb, _p(edges), int(seed), int(iteration), int(first_event),
+                               int(count), integrand_id, _p(p), _p(words, C.c_uint32),
+                               _p(bins, C.c_int32), _p(x), _p(fJ))
     if rc:
         raise OracleError(rc)
     return words, bins, x, fJ
 
 
-def accumulate(edges, seed, iteration, first_event, count, integrand_id, params=None):
+def accumulate(edges, seed, iteration, first_event, count, integrand_id, params=None, variant=0):
     """C6 on one event range: (S1, S2, H) as np.longdouble scalars / array [dim, n_bins]."""
     edges = _f64(edges)
     dim, nb = edges.shape[0], edges.shape[1] - 1
@@ -149,8 +175,8 @@ def accumulate(edges, seed, iteration, first_event, count, integrand_id, params=
     sums = np.zeros(4)
     hi = np.zeros((dim, nb))
     lo = np.zeros((dim, nb))
-    rc = lib().oracle_accumulate(dim, nb, _p(edges), int(seed), int(iteration), int(first_event),
-                                 int(count), integrand_id, _p(p), _p(sums), _p(hi), _p(lo))
+    rc = lib().oracle_accumulate_v(int(variant), dim, nb, _p(edges), int(seed), int(iteration), int(first_event),
+                                   int(count), integrand_id, _p(p), _p(sums), _p(hi), _p(lo))
     if rc:
         raise OracleError(rc)
     ld = np.longdouble
@@ -171,7 +197,7 @@ def estimate(S1, S2, n_events):
     return I.value, sg.value
 
 
-def iterate(edges, n_events, seed, iteration, integrand_id, params=None, threads=1):
+def iterate(edges, n_events, seed, iteration, integrand_id, params=None, threads=1, variant=0):
     """One Vegas iteration (C2..C7) on the given grid: (I, sigma, H[dim, n_bins] fp64).
 
     threads > 1 runs the single-threaded C routine on disjoint event ranges concurrently
@@ -184,7 +210,7 @@ def iterate(edges, n_events, seed, iteration, integrand_id, params=None, threads
     jobs = [(bounds[t], bounds[t + 1] - bounds[t]) for t in range(threads)]
 
     def run(job):
-        return accumulate(edges, seed, iteration, job[0], job[1], integrand_id, params)
+        return accumulate(edges, seed, iteration, job[0], job[1], integrand_id, params, variant)
 
     if threads == 1:
         parts = [run(jobs[0])]
@@ -227,7 +253,7 @@ def combine(I_k, sigma_k, n_skip=0):
 
 
 def integrate(dim, n_bins, n_iter, n_events, seed, alpha, integrand_id, params=None, n_skip=0,
-              edges=None, threads=1):
+              edges=None, threads=1, variant=0):
     """Whole chain (C2..C9).  Returns a dict with I, sigma, chi2_dof, per_iter [n_iter,2],
     edges_trace [n_iter, dim, n_bins+1] (grid each iteration sampled from), hist_trace
     [n_iter, dim, n_bins], edges (final grid), status.  threads > 1 uses iterate(threads=...)
@@ -240,17 +266,17 @@ def integrate(dim, n_bins, n_iter, n_events, seed, alpha, integrand_id, params=N
     status = OK
     if threads == 1:
         I, s, c = C.c_double(), C.c_double(), C.c_double()
-        status = lib().oracle_integrate(dim, n_bins, _p(edges), n_iter, n_skip, int(n_events),
-                                        int(seed), float(alpha), integrand_id, _p(p),
-                                        C.byref(I), C.byref(s), C.byref(c), _p(per_iter),
-                                        _p(et), _p(ht))
+        status = lib().oracle_integrate_v(int(variant), dim, n_bins, _p(edges), n_iter, n_skip, int(n_events),
+                                          int(seed), float(alpha), integrand_id, _p(p),
+                                          C.byref(I), C.byref(s), C.byref(c), _p(per_iter),
+                                          _p(et), _p(ht))
         if status == EINVAL:
             raise OracleError(status)
         res = (I.value, s.value, c.value)
     else:
         for k in range(n_iter):
             et[k] = edges
-            Ik, sk, H = iterate(edges, n_events, seed, k, integrand_id, params, threads)
+            Ik, sk, H = iterate(edges, n_events, seed, k, integrand_id, params, threads, variant)
             ht[k] = H
             per_iter[k] = (Ik, sk)
             if alpha >= 0:

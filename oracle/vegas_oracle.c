@@ -28,6 +28,14 @@
  * invariant (C6, C7), fixed points / interp-based rebin / worked examples (C8), closed forms
  * (C9), 5-sigma agreement of whole chains with the closed-form integrals.
  *
+ * Variants (readings C3' and C4' of DESIGN.md section 2), selected by the `variant` bit mask of
+ * the *_v functions (0 = the method as above; the functions without _v are variant 0):
+ *   ORACLE_V_U53 (1)  C3': 53-bit uniforms, two Philox words per draw (oracle_word53, oracle_split53);
+ *   ORACLE_V_Q32 (2)  C4': the per-bin pair (X_b, Delta_b) of the sampling map rounded to fp32 (oracle_q32); the
+ *                     master grid and the refinement stay fp64.
+ * Pins: tests/test_oracle_variants.py (exact rationals for the 53-bit split and for the rounded map, an independent
+ * Python-integer Philox for the two-word layout, brute-force re-accumulation, 5-sigma chains).
+ *
  * Build: gcc -O2 -ffp-contract=off -fPIC -shared (see oracle/build.py).
  */
 #include <math.h>
@@ -41,6 +49,9 @@
 #define ORACLE_ENUMERIC (-3)
 
 #define ORACLE_MAX_DIM 64
+
+#define ORACLE_V_U53 1
+#define ORACLE_V_Q32 2
 
 enum { F_CONST = 0, F_GAUSS = 1, F_GENZ_PRODUCT_PEAK = 2, F_BW_POLY = 3, F_GENZ_DISCONTINUOUS = 4 };
 
@@ -90,6 +101,38 @@ void oracle_split(uint32_t word, int n_bins, int32_t *bin, double *r)
     uint32_t lo = (uint32_t)(P & 0xFFFFFFFFu);
     *bin = (int32_t)(P >> 32);
     *r = ((double)lo + 0.5) * (1.0 / 4294967296.0);
+}
+
+/* C3' (variant ORACLE_V_U53)  53-bit uniforms from two words per draw.  One Philox block serves TWO dimensions:
+ * key = (seed lo, seed hi); counter = (j>>1, iteration, e lo, e hi); dimension j takes hi = output[2(j&1)],
+ * lo = output[2(j&1)+1] and U = hi * 2^21 + (lo >> 11), a 53-bit integer (the usual construction of a double in
+ * [0,1) from two 32-bit words). */
+uint64_t oracle_word53(uint64_t seed, uint32_t iteration, uint64_t event, int j)
+{
+    uint32_t ctr[4] = { (uint32_t)(j >> 1), iteration, (uint32_t)(event & 0xFFFFFFFFu),
+                        (uint32_t)(event >> 32) };
+    uint32_t key[2] = { (uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32) };
+    uint32_t out[4];
+    oracle_philox4x32_10(ctr, key, out);
+    uint64_t hi = out[2 * (j & 1)], lo = out[2 * (j & 1) + 1];
+    return (hi << 21) | (lo >> 11);
+}
+
+/* C3' split: P = U*nb exactly (U < 2^53, nb <= 256: P < 2^61); bin b = P >> 53; frac = P mod 2^53;
+ * r = frac * 2^-53, exact in fp64, r in [0,1). */
+void oracle_split53(uint64_t U, int n_bins, int32_t *bin, double *r)
+{
+    uint64_t P = U * (uint64_t)(uint32_t)n_bins;
+    uint64_t frac = P & ((1ull << 53) - 1ull);
+    *bin = (int32_t)(P >> 53);
+    *r = (double)frac * (1.0 / 9007199254740992.0);
+}
+
+/* C4' (variant ORACLE_V_Q32)  a grid-table entry rounded to fp32 (round to nearest even) and widened back. */
+double oracle_q32(double v)
+{
+    volatile float q = (float)v;
+    return (double)q;
 }
 
 /* C5  built-in integrands, fp64 formulas.
@@ -181,22 +224,32 @@ static int check_grid(int dim, int n_bins, const double *edges)
 
 /* C2..C5 for ONE event: words, bins, x (C4: x_j = X[j][b] + (X[j][b+1]-X[j][b]) * r),
  * Jacobian J = prod_j n_bins * Delta_j, and f(x).  edges is [dim][n_bins+1], row-major. */
-int oracle_sample_event(int dim, int n_bins, const double *edges, uint64_t seed,
-                        uint32_t iteration, uint64_t event, int integrand_id,
-                        const double *params, uint32_t *words, int32_t *bins, double *x,
-                        double *jac, double *f)
+int oracle_sample_event_v(int variant, int dim, int n_bins, const double *edges, uint64_t seed,
+                          uint32_t iteration, uint64_t event, int integrand_id,
+                          const double *params, uint32_t *words, int32_t *bins, double *x,
+                          double *jac, double *f)
 {
     double J = 1.0;
     for (int j = 0; j < dim; ++j) {
         const double *X = edges + (size_t)j * (n_bins + 1);
-        uint32_t word = oracle_word(seed, iteration, event, j);
         int32_t b;
         double r;
-        oracle_split(word, n_bins, &b, &r);
-        double delta = X[b + 1] - X[b];
-        x[j] = X[b] + delta * r;
+        if (variant & ORACLE_V_U53) {               /* C3': words[j] reports the top 32 bits of U */
+            uint64_t U = oracle_word53(seed, iteration, event, j);
+            oracle_split53(U, n_bins, &b, &r);
+            if (words) words[j] = (uint32_t)(U >> 21);
+        } else {
+            uint32_t word = oracle_word(seed, iteration, event, j);
+            oracle_split(word, n_bins, &b, &r);
+            if (words) words[j] = word;
+        }
+        double x0 = X[b], delta = X[b + 1] - X[b];
+        if (variant & ORACLE_V_Q32) {               /* C4': the table entry (X_b, Delta_b) in fp32 */
+            x0 = oracle_q32(x0);
+            delta = oracle_q32(delta);
+        }
+        x[j] = x0 + delta * r;
         J *= (double)n_bins * delta;
-        if (words) words[j] = word;
         bins[j] = b;
     }
     *jac = J;
@@ -204,23 +257,40 @@ int oracle_sample_event(int dim, int n_bins, const double *edges, uint64_t seed,
     return ORACLE_OK;
 }
 
+int oracle_sample_event(int dim, int n_bins, const double *edges, uint64_t seed,
+                        uint32_t iteration, uint64_t event, int integrand_id,
+                        const double *params, uint32_t *words, int32_t *bins, double *x,
+                        double *jac, double *f)
+{
+    return oracle_sample_event_v(0, dim, n_bins, edges, seed, iteration, event, integrand_id, params,
+                                 words, bins, x, jac, f);
+}
+
 /* debug view of a range of events (parity hook for the CUDA K4 kernel, P1/P2):
  * words [count][dim], bins [count][dim], x [count][dim], fJ [count]. */
+int oracle_sample_v(int variant, int dim, int n_bins, const double *edges, uint64_t seed, uint32_t iteration,
+                    uint64_t first_event, uint64_t count, int integrand_id, const double *params,
+                    uint32_t *words, int32_t *bins, double *x, double *fJ)
+{
+    int rc = check_grid(dim, n_bins, edges);
+    if (rc) return rc;
+    if (oracle_n_params(integrand_id, dim) < 0 || (variant & ~3)) return ORACLE_EINVAL;
+    for (uint64_t q = 0; q < count; ++q) {
+        double J, f;
+        oracle_sample_event_v(variant, dim, n_bins, edges, seed, iteration, first_event + q, integrand_id,
+                              params, words ? words + q * dim : NULL, bins + q * dim,
+                              x + q * dim, &J, &f);
+        fJ[q] = f * J;
+    }
+    return ORACLE_OK;
+}
+
 int oracle_sample(int dim, int n_bins, const double *edges, uint64_t seed, uint32_t iteration,
                   uint64_t first_event, uint64_t count, int integrand_id, const double *params,
                   uint32_t *words, int32_t *bins, double *x, double *fJ)
 {
-    int rc = check_grid(dim, n_bins, edges);
-    if (rc) return rc;
-    if (oracle_n_params(integrand_id, dim) < 0) return ORACLE_EINVAL;
-    for (uint64_t q = 0; q < count; ++q) {
-        double J, f;
-        oracle_sample_event(dim, n_bins, edges, seed, iteration, first_event + q, integrand_id,
-                            params, words ? words + q * dim : NULL, bins + q * dim,
-                            x + q * dim, &J, &f);
-        fJ[q] = f * J;
-    }
-    return ORACLE_OK;
+    return oracle_sample_v(0, dim, n_bins, edges, seed, iteration, first_event, count, integrand_id, params,
+                           words, bins, x, fJ);
 }
 
 /* C6  accumulate events [first_event, first_event+count): v = f*J; S1 += v; S2 += v*v;
@@ -228,14 +298,14 @@ int oracle_sample(int dim, int n_bins, const double *edges, uint64_t seed, uint3
  * (hi, lo) double pairs (hi = (double)S, lo = (double)(S - hi)) so that disjoint event
  * ranges run by independent callers can be added without losing the extra bits.
  * sums = { S1_hi, S1_lo, S2_hi, S2_lo }; hist_hi / hist_lo are [dim][n_bins]. */
-int oracle_accumulate(int dim, int n_bins, const double *edges, uint64_t seed,
-                      uint32_t iteration, uint64_t first_event, uint64_t count,
-                      int integrand_id, const double *params, double *sums, double *hist_hi,
-                      double *hist_lo)
+int oracle_accumulate_v(int variant, int dim, int n_bins, const double *edges, uint64_t seed,
+                        uint32_t iteration, uint64_t first_event, uint64_t count,
+                        int integrand_id, const double *params, double *sums, double *hist_hi,
+                        double *hist_lo)
 {
     int rc = check_grid(dim, n_bins, edges);
     if (rc) return rc;
-    if (oracle_n_params(integrand_id, dim) < 0) return ORACLE_EINVAL;
+    if (oracle_n_params(integrand_id, dim) < 0 || (variant & ~3)) return ORACLE_EINVAL;
     size_t nh = (size_t)dim * n_bins;
     long double *H = (long double *)calloc(nh, sizeof(long double));
     if (!H) return ORACLE_EINVAL;
@@ -244,8 +314,8 @@ int oracle_accumulate(int dim, int n_bins, const double *edges, uint64_t seed,
     double x[ORACLE_MAX_DIM];
     for (uint64_t q = 0; q < count; ++q) {
         double J, f;
-        oracle_sample_event(dim, n_bins, edges, seed, iteration, first_event + q, integrand_id,
-                            params, NULL, bins, x, &J, &f);
+        oracle_sample_event_v(variant, dim, n_bins, edges, seed, iteration, first_event + q, integrand_id,
+                              params, NULL, bins, x, &J, &f);
         double v = f * J;
         double v2 = v * v;
         S1 += (long double)v;
@@ -260,6 +330,15 @@ int oracle_accumulate(int dim, int n_bins, const double *edges, uint64_t seed,
     }
     free(H);
     return ORACLE_OK;
+}
+
+int oracle_accumulate(int dim, int n_bins, const double *edges, uint64_t seed,
+                      uint32_t iteration, uint64_t first_event, uint64_t count,
+                      int integrand_id, const double *params, double *sums, double *hist_hi,
+                      double *hist_lo)
+{
+    return oracle_accumulate_v(0, dim, n_bins, edges, seed, iteration, first_event, count, integrand_id,
+                               params, sums, hist_hi, hist_lo);
 }
 
 /* C7  estimate from the sums of n events: I = S1/n; Var = (S2/n - I^2)/(n-1);
@@ -280,16 +359,23 @@ int oracle_estimate(const double *sums, uint64_t n_events, double *I, double *si
 }
 
 /* One whole iteration (C2..C7) on a given grid: I, sigma, hist [dim][n_bins] (fp64). */
+int oracle_iterate_v(int variant, int dim, int n_bins, const double *edges, uint64_t n_events, uint64_t seed,
+                     uint32_t iteration, int integrand_id, const double *params, double *I,
+                     double *sigma, double *hist)
+{
+    double sums[4];
+    if (n_events < 2) return ORACLE_EINVAL;
+    int rc = oracle_accumulate_v(variant, dim, n_bins, edges, seed, iteration, 0, n_events, integrand_id,
+                                 params, sums, hist, NULL);
+    if (rc) return rc;
+    return oracle_estimate(sums, n_events, I, sigma);
+}
+
 int oracle_iterate(int dim, int n_bins, const double *edges, uint64_t n_events, uint64_t seed,
                    uint32_t iteration, int integrand_id, const double *params, double *I,
                    double *sigma, double *hist)
 {
-    double sums[4];
-    if (n_events < 2) return ORACLE_EINVAL;
-    int rc = oracle_accumulate(dim, n_bins, edges, seed, iteration, 0, n_events, integrand_id,
-                               params, sums, hist, NULL);
-    if (rc) return rc;
-    return oracle_estimate(sums, n_events, I, sigma);
+    return oracle_iterate_v(0, dim, n_bins, edges, n_events, seed, iteration, integrand_id, params, I, sigma, hist);
 }
 
 /* C8  refine one grid from a histogram (classic 1978 Vegas: smooth, normalise, compress with
@@ -406,10 +492,10 @@ void oracle_uniform_edges(int dim, int n_bins, double *edges)
  * [n_iter][2] = (I_k, sigma_k) or NULL; edges_trace is [n_iter][dim][n_bins+1] (the grid each
  * iteration SAMPLED from) or NULL; hist_trace is [n_iter][dim][n_bins] or NULL.
  * alpha < 0 disables refinement (plain importance sampling on a fixed grid). */
-int oracle_integrate(int dim, int n_bins, double *edges, int n_iter, int n_skip,
-                     uint64_t n_events, uint64_t seed, double alpha, int integrand_id,
-                     const double *params, double *I, double *sigma, double *chi2_dof,
-                     double *per_iter, double *edges_trace, double *hist_trace)
+int oracle_integrate_v(int variant, int dim, int n_bins, double *edges, int n_iter, int n_skip,
+                       uint64_t n_events, uint64_t seed, double alpha, int integrand_id,
+                       const double *params, double *I, double *sigma, double *chi2_dof,
+                       double *per_iter, double *edges_trace, double *hist_trace)
 {
     if (n_iter < 1) return ORACLE_EINVAL;
     size_t ne = (size_t)dim * (n_bins + 1), nh = (size_t)dim * n_bins;
@@ -421,8 +507,8 @@ int oracle_integrate(int dim, int n_bins, double *edges, int n_iter, int n_skip,
     if (!hist || !next || !Ik || !sk) { status = ORACLE_EINVAL; goto done; }
     for (int k = 0; k < n_iter; ++k) {
         if (edges_trace) memcpy(edges_trace + (size_t)k * ne, edges, sizeof(double) * ne);
-        int rc = oracle_iterate(dim, n_bins, edges, n_events, seed, (uint32_t)k, integrand_id,
-                                params, &Ik[k], &sk[k], hist);
+        int rc = oracle_iterate_v(variant, dim, n_bins, edges, n_events, seed, (uint32_t)k, integrand_id,
+                                  params, &Ik[k], &sk[k], hist);
         if (rc) { status = rc; goto done; }
         if (hist_trace) memcpy(hist_trace + (size_t)k * nh, hist, sizeof(double) * nh);
         if (per_iter) { per_iter[2 * k] = Ik[k]; per_iter[2 * k + 1] = sk[k]; }
@@ -440,4 +526,13 @@ int oracle_integrate(int dim, int n_bins, double *edges, int n_iter, int n_skip,
 done:
     free(hist); free(next); free(Ik); free(sk);
     return status;
+}
+
+int oracle_integrate(int dim, int n_bins, double *edges, int n_iter, int n_skip,
+                     uint64_t n_events, uint64_t seed, double alpha, int integrand_id,
+                     const double *params, double *I, double *sigma, double *chi2_dof,
+                     double *per_iter, double *edges_trace, double *hist_trace)
+{
+    return oracle_integrate_v(0, dim, n_bins, edges, n_iter, n_skip, n_events, seed, alpha, integrand_id, params,
+                              I, sigma, chi2_dof, per_iter, edges_trace, hist_trace);
 }

@@ -247,6 +247,27 @@ int vegas_set_launch(vegas_grid* g, int blocks, int threads, int table_copies, i
 int vegas_get_launch(vegas_grid* g, int integrand_id, int precision, int* path, int* blocks, int* threads,
                      int* table_copies, int* hist_copies, size_t* shared_bytes);
 
+/* Variants of the sampling map (readings C3' and C4'; "how to
+ * generate the random numbers" and PAPER.md:88 "number of subdivisions of the grid" are all the paper fixes).  Opt-in, per
+ * grid, for every later iterate / accumulate / integrate / debug_sample call:
+ *   VEGAS_VARIANT_NONE  the method as vegas_iterate describes it (32 random bits per event and dimension, fp64 table).
+ *   VEGAS_VARIANT_U53   C3': 53-bit uniforms from two Philox words per draw.  One Philox block serves two dimensions:
+ *                       counter = (j>>1, iteration, e lo, e hi); U = out[2(j&1)] * 2^21 + (out[2(j&1)+1] >> 11);
+ *                       P = U * n_bins, bin = P >> 53, r = (P mod 2^53) * 2^-53 in [0,1).  A different sample from the
+ *                       same seed; twice the generator work per event.
+ *   VEGAS_VARIANT_Q32   C4': the fused kernel's grid table holds the per-bin pair (X_b, Delta_b = X_{b+1} - X_b) rounded
+ *                       to fp32 (half the table read); x = X~_b + Delta~_b * r and J = prod n_bins * Delta~_b in fp64.
+ *                       The master grid, the histogram and the refinement stay fp64.  The rounded bins do not tile [0,1)
+ *                       exactly: a relative bias of up to dim * 2^-24 on I (measured: DESIGN.md section 11).
+ * Both are fp64 modes of the built-in integrands on the fast path: with a variant set, a call with precision 32, with
+ * VEGAS_F_USER, or for a shape that only the generic kernel serves returns VEGAS_EINVAL.  vegas_debug_sample reports
+ * the top 32 bits of U in `words` under VEGAS_VARIANT_U53. */
+#define VEGAS_VARIANT_NONE 0
+#define VEGAS_VARIANT_U53 1
+#define VEGAS_VARIANT_Q32 2
+int vegas_set_variant(vegas_grid* g, int variant);
+int vegas_get_variant(const vegas_grid* g);
+
 /* Instrumentation for bench.py: with profiling on, every fused-kernel launch is bracketed by CUDA
  * events on its stream; vegas_kernel_time_ms() synchronises those events and returns their summed
  * duration and the number of launches since the last vegas_reset_counters().  vegas_launch_count()

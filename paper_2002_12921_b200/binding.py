@@ -19,6 +19,7 @@ VEGAS_OK, VEGAS_EINVAL, VEGAS_ECUDA, VEGAS_ENUMERIC = 0, -1, -2, -3
 VEGAS_F_CONST, VEGAS_F_GAUSS, VEGAS_F_GENZ_PRODUCT_PEAK, VEGAS_F_BW_POLY, VEGAS_F_USER = 0, 1, 2, 3, 4
 VEGAS_USER_MAX_PARAMS = 64
 VEGAS_FP64, VEGAS_FP32 = 64, 32
+VEGAS_VARIANT_NONE, VEGAS_VARIANT_U53, VEGAS_VARIANT_Q32 = 0, 1, 2
 VEGAS_MAX_DIM, VEGAS_MAX_BINS, VEGAS_MAX_PARAMS = 32, 256, 160
 
 if not os.path.exists(LIB_PATH):
@@ -65,6 +66,8 @@ SIGNATURES = {
     "vegas_set_launch": (C.c_int, [_vp, C.c_int, C.c_int, C.c_int, C.c_int]),
     "vegas_get_launch": (C.c_int, [_vp, C.c_int, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int),
                                    C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_size_t)]),
+    "vegas_set_variant": (C.c_int, [_vp, C.c_int]),
+    "vegas_get_variant": (C.c_int, [_vp]),
     "vegas_set_profiling": (C.c_int, [_vp, C.c_int]),
     "vegas_kernel_time_ms": (C.c_int, [_vp, _f64p, C.POINTER(_u64)]),
     "vegas_launch_count": (_u64, [_vp]),
@@ -314,6 +317,13 @@ class VegasGrid:
                                          C.byref(ct), C.byref(ch), C.byref(sh)))
         return dict(path="rotated" if pa.value else "generic", blocks=b.value, threads=t.value,
                     table_copies=ct.value, hist_copies=ch.value, shared_bytes=sh.value)
+
+    def set_variant(self, variant):
+        """VEGAS_VARIANT_NONE / _U53 (53-bit uniforms) / _Q32 (fp32-rounded table entries); fp64 fast path only."""
+        self._check(lib.vegas_set_variant(self._h, int(variant)))
+
+    def get_variant(self):
+        return int(lib.vegas_get_variant(self._h))
 
     def set_profiling(self, on=True):
         self._check(lib.vegas_set_profiling(self._h, int(bool(on))))

@@ -82,6 +82,7 @@ struct vegas_grid {
     double user[5][VEGAS_MAX_PARAMS] = {};       // the caller's arrays as given to vegas_set_params
     vegas::UserKernel ukernel;                   // VEGAS_F_USER: the run-time compiled fused kernel
     int cfg_blocks = 0, cfg_threads = 0, cfg_ct = 0, cfg_ch = 0;
+    int variant = 0;                // VEGAS_VARIANT_*: the sampling map of the iterate calls (vegas_set_variant)
     int active_blocks = 0;          // CTAs whose partial slots the current iteration uses
     bool profiling = false;
     std::vector<cudaEvent_t> events;   // pairs (start, stop)
@@ -158,11 +159,18 @@ int ilog2(int v) {
     return l;
 }
 
+bool use_rot_path(const vegas_grid* g, int fid, int precision);
+// the variants of the sampling map exist as fp64 fast-path kernels of the built-in integrands
+bool variant_available(const vegas_grid* g, int fid, int precision) {
+    return precision == VEGAS_FP64 && fid != VEGAS_F_USER && use_rot_path(g, fid, precision);
+}
+
 bool check_call(const vegas_grid* g, int fid, int precision) {
     if (!g) return false;
     if (fid < 0 || fid > VEGAS_F_USER || !g->params_set[fid]) return false;
-    if (fid == VEGAS_F_USER) return g->ukernel.kernel != nullptr && precision == VEGAS_FP64;
+    if (fid == VEGAS_F_USER) return g->ukernel.kernel != nullptr && precision == VEGAS_FP64 && g->variant == 0;
     if (expected_n_params(fid, g->dim) < 0) return false;
+    if (g->variant != 0 && !variant_available(g, fid, precision)) return false;
     return precision == VEGAS_FP64 || precision == VEGAS_FP32;
 }
 
@@ -188,7 +196,7 @@ bool use_rot_path(const vegas_grid* g, int fid, int precision) {
 
 // shift_j, scale_j, post_scale, fin0 of the affine pre-composition (see vegas_iterate_rot.cuh)
 void rot_constants(const vegas_grid* g, int fid, int precision, double* shift, double* scale, double* post_scale,
-                   double* fin0, double* fin1, double* jac_init, double* fpar, bool word_map) {
+                   double* fin0, double* fin1, double* jac_init, double* fpar, bool word_map, int variant = 0) {
     const int dim = g->dim;
     const double nb = (double)g->n_bins;
     *post_scale = 1.0;
@@ -245,13 +253,17 @@ void rot_constants(const vegas_grid* g, int fid, int precision, double* shift, d
     // fp64 table entries carry 2^-32 per dimension (RotEntry<double>): start the running Jacobian product at
     // 2^(32 floor(d/2)) and give the rest back in post_scale -- exact powers of two, the product stays in range
     *jac_init = 1.0;
-    if (precision == VEGAS_FP64) {
-        const int h = dim / 2;
-        *jac_init = std::ldexp(1.0, 32 * h);
-        *post_scale *= std::ldexp(1.0, 32 * (dim - h));
+    if (precision == VEGAS_FP64 && variant == VEGAS_VARIANT_Q32) {
+        // C4': the table holds (X~_b, Delta~_b) themselves; the running product is prod Delta~_b and
+        // J = n_bins^d prod Delta~_b, so the scale_j and n_bins that the other tables carry in B come back here
+        for (int j = 0; j < dim; ++j) *post_scale *= scale[j];
+    } else if (precision == VEGAS_FP64) {
+        const int h = dim / 2, bits = vegas::rot_jac_bits(64, variant);      // 2^-32 per dimension, 2^-53 for C3'
+        *jac_init = std::ldexp(1.0, bits * h);
+        *post_scale *= std::ldexp(1.0, bits * (dim - h));
         // the fast path's fp64 table entries are affine in the whole Philox word (RotEntry<double>::make_w): their
         // slope, the Jacobian factor, carries one more n_bins per dimension
-        if (word_map)
+        if (word_map && variant == 0)
             for (int j = 0; j < dim; ++j) *post_scale /= nb;
     }
 }
@@ -315,6 +327,21 @@ RotShape rot_shape(const vegas_grid* g, int fid) {
 cudaError_t launch_rot(vegas_grid* g, int fid, int precision, int dim, const vegas::RotArgs& a, const RotShape& s,
                        cudaStream_t st) {
     if (fid == VEGAS_F_USER) return vegas::user_launch(&g->ukernel, a, s.blocks, s.threads, s.shmem, st);
+    if (precision == VEGAS_FP64 && g->variant != 0) {
+#define VEGAS_VAR_CASE(F)                                                                                              \
+    case F:                                                                                                            \
+        return g->variant == VEGAS_VARIANT_U53                                                                         \
+                   ? vegas::launch_iterate_rot<F, double, vegas::kVarU53>(dim, a, s.blocks, s.threads, s.shmem, st)    \
+                   : vegas::launch_iterate_rot<F, double, vegas::kVarQ32>(dim, a, s.blocks, s.threads, s.shmem, st);
+        switch (fid) {
+            VEGAS_VAR_CASE(VEGAS_F_CONST)
+            VEGAS_VAR_CASE(VEGAS_F_GAUSS)
+            VEGAS_VAR_CASE(VEGAS_F_GENZ_PRODUCT_PEAK)
+            VEGAS_VAR_CASE(VEGAS_F_BW_POLY)
+        }
+#undef VEGAS_VAR_CASE
+        return cudaErrorInvalidValue;
+    }
     if (precision == VEGAS_FP64) {
         switch (fid) {
         case VEGAS_F_CONST: return vegas::launch_iterate_rot<VEGAS_F_CONST, double>(dim, a, s.blocks, s.threads, s.shmem, st);
@@ -630,7 +657,7 @@ int accumulate_impl(vegas_grid* g, uint64_t first_event, uint64_t count, uint64_
         ra.n_groups = rs.n_groups;
         ra.ring = rs.ring;
         rot_constants(g, fid, precision, ra.shift, ra.scale, &ra.post_scale, &ra.fin0, &ra.fin1, &ra.jac_init, ra.fpar,
-                      vegas::rot_word_map(precision == VEGAS_FP64 ? 64 : 32, g->dim));
+                      vegas::rot_word_map(precision == VEGAS_FP64 ? 64 : 32, g->dim), g->variant);
         if (fid == VEGAS_F_USER && g->n_obs > 0) {
             ra.obs = g->d_obs;
             ra.n_obs = g->n_obs;
@@ -876,7 +903,8 @@ int vegas_debug_sample(vegas_grid* g, uint64_t first_event, uint32_t count, uint
     // both K1 kernels form u_j, f and v through the affine map for every integrand but BW_POLY beyond the fast path
     const bool rot = fid != VEGAS_F_BW_POLY || use_rot_path(g, fid, precision);
     a.word_map = rot && vegas::rot_word_map(precision == VEGAS_FP64 ? 64 : 32, g->dim);
-    if (rot) rot_constants(g, fid, precision, a.shift, a.scale, &a.post_scale, &a.fin0, &a.fin1, &a.jac_init, a.fpar, a.word_map != 0);
+    a.variant = g->variant;
+    if (rot) rot_constants(g, fid, precision, a.shift, a.scale, &a.post_scale, &a.fin0, &a.fin1, &a.jac_init, a.fpar, a.word_map != 0, g->variant);
     CUDA_TRY(g, vegas::launch_debug(fid, precision, rot, a, g->derived[fid], st));
     g->launches++;
     if (words) CUDA_TRY(g, cudaMemcpyAsync(words, a.words, per_dim * 4, cudaMemcpyDeviceToHost, st));
@@ -958,6 +986,14 @@ int vegas_set_launch(vegas_grid* g, int blocks, int threads, int table_copies, i
     g->active_blocks = 0;
     return VEGAS_OK;
 }
+
+int vegas_set_variant(vegas_grid* g, int variant) {
+    if (!g || (variant != VEGAS_VARIANT_NONE && variant != VEGAS_VARIANT_U53 && variant != VEGAS_VARIANT_Q32)) return VEGAS_EINVAL;
+    g->variant = variant;
+    return VEGAS_OK;
+}
+
+int vegas_get_variant(const vegas_grid* g) { return g ? g->variant : VEGAS_EINVAL; }
 
 int vegas_get_launch(vegas_grid* g, int integrand_id, int precision, int* path, int* blocks, int* threads,
                      int* table_copies, int* hist_copies, size_t* shared_bytes) {

@@ -218,6 +218,46 @@ template <typename T> struct RotSplit<T, false> {
     }
 };
 
+// ---- variants of the sampling map (readings C3', C4'; fp64, built-in integrands) ------
+// VAR 0: the method (C2, C3, C4).
+// VAR 1 (VEGAS_VARIANT_U53, C3'): 53-bit uniforms, two Philox words per draw: one Philox block serves two dimensions
+//        (counter word 0 = j >> 1), U = hi 2^21 + (lo >> 11), P = U n_bins, b = P >> 53, r = (P mod 2^53) 2^-53.
+//        Table entry (A, B) = (scale (X_b - shift), scale Delta 2^-53), u = A + B (double)(P mod 2^53).
+// VAR 2 (VEGAS_VARIANT_Q32, C4'): the table holds the per-bin pair (X_b, Delta_b) rounded to fp32 (8 bytes per entry,
+//        half the table read of VAR 0); x = X~_b + Delta~_b r in fp64, u = scale (x - shift), J = prod n_bins Delta~_b.
+constexpr int kVarU53 = 1, kVarQ32 = 2;
+__host__ __device__ constexpr int rot_jac_bits(int precision_bits, int var) {     // table B = scale Delta 2^-bits
+    return precision_bits != 64 ? 0 : (var == kVarU53 ? 53 : (var == kVarQ32 ? 0 : 32));
+}
+template <typename T, int VAR> struct RotTableEntry { using type = typename RotEntry<T>::type; };
+template <> struct RotTableEntry<double, kVarQ32> { using type = float2; };
+struct RotVarU53 {
+    static __device__ __forceinline__ double2 make(double x0, double x1, double shift, double scale) {
+        return make_double2((x0 - shift) * scale, ((x1 - x0) * scale) * 1.1102230246251565e-16);      // 2^-53
+    }
+    static __device__ __forceinline__ void split(uint64_t U, uint32_t nb, uint32_t& b, double& o) {
+        const uint64_t P = U * (uint64_t)nb;                      // < 2^61
+        b = (uint32_t)(P >> 53);
+        o = (double)(P & 0x1FFFFFFFFFFFFFull);                    // exact: 53 bits
+    }
+};
+struct RotVarQ32 {
+    static __device__ __forceinline__ float2 make(double x0, double x1) { return make_float2((float)x0, (float)(x1 - x0)); }
+};
+// w'[i] = w[gamma ^ i] for the G lane groups of a block (two conditional swaps, SELs)
+template <int G, typename W>
+__device__ __forceinline__ void rot_permute(W (&w)[4], int gamma) {
+    if (G == 4) {
+        const bool g1 = gamma & 1, g2 = gamma & 2;
+        const W t0 = g1 ? w[1] : w[0], t1 = g1 ? w[0] : w[1], t2 = g1 ? w[3] : w[2], t3 = g1 ? w[2] : w[3];
+        w[0] = g2 ? t2 : t0; w[1] = g2 ? t3 : t1; w[2] = g2 ? t0 : t2; w[3] = g2 ? t1 : t3;
+    } else if (G == 2) {
+        const bool g1 = gamma & 1;
+        const W t0 = g1 ? w[1] : w[0], t1 = g1 ? w[0] : w[1];
+        w[0] = t0; w[1] = t1;
+    }
+}
+
 // 32-bit shared-window addressing: one register per address, no generic-to-shared conversion
 template <typename T2> __device__ __forceinline__ T2 lds_entry(uint32_t addr);
 template <> __device__ __forceinline__ double2 lds_entry<double2>(uint32_t addr) {
@@ -448,13 +488,13 @@ __device__ __forceinline__ void philox4x32_10_args(uint32_t c0, uint32_t c1, uin
 
 // S1..S5 for one event: Philox -> split -> table -> u -> integrand; returns v = f J and leaves the
 // histogram address of every (block, sub-step) in haddr (one LEA from the table address, outside the critical section).
-template <int FID, typename T, int DIM>
+template <int FID, typename T, int DIM, int VAR>
 __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, DIM>& L,
                                             const RotCtx<FID, T, (DIM + 3) / 4>& ctx, uint32_t e_lo, uint32_t e_hi,
                                             bool live, T fin0, T fin1, uint32_t (&haddr)[(DIM + 3) / 4][4], double& obs_val) {
-    using E = RotEntry<T>;
-    using SP = RotSplit<T, rot_word_map(8 * (int)sizeof(T), DIM)>;
-    using T2 = typename E::type;
+    using SP = RotSplit<T, rot_word_map(8 * (int)sizeof(T), DIM) && VAR == 0>;
+    using T2 = typename RotTableEntry<T, VAR>::type;
+    static_assert(VAR == 0 || sizeof(T) == 8, "the variants are fp64 modes");
     constexpr int NBLK = RotLane<T, DIM>::NBLK, R = RotLane<T, DIM>::R, GL = RotLane<T, DIM>::GL;
     const int nb = a.n_bins;
     const double nb_2m32 = (double)nb * 2.3283064365386963e-10;
@@ -471,19 +511,30 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
         const int NSUB = last ? ((R == 3) ? 4 : R) : 4;             // sub-steps of this block
         const int gamma = last ? L.gammaL : L.gamma4;
         uint32_t w[4];
-        philox4x32_10_args((uint32_t)blk, a.iteration, e_lo, e_hi, a, w);
-        // w'[i] = w[gamma ^ i]
-        if (G == 4) {
-            const bool g1 = gamma & 1, g2 = gamma & 2;
-            const uint32_t t0 = g1 ? w[1] : w[0], t1 = g1 ? w[0] : w[1], t2 = g1 ? w[3] : w[2], t3 = g1 ? w[2] : w[3];
-            w[0] = g2 ? t2 : t0; w[1] = g2 ? t3 : t1; w[2] = g2 ? t0 : t2; w[3] = g2 ? t1 : t3;
-        } else if (G == 2) {
-            const bool g1 = gamma & 1;
-            const uint32_t t0 = g1 ? w[1] : w[0], t1 = g1 ? w[0] : w[1];
-            w[0] = t0; w[1] = t1;
+        uint64_t U[4];
+        (void)U;
+        (void)w;
+        if constexpr (VAR == kVarU53) {
+            // C3': Philox block 2 blk serves dimensions 4 blk, 4 blk + 1; block 2 blk + 1 the next two
+            const int dims_here = last ? R : 4;
+            uint32_t wa[4], wb[4] = {0u, 0u, 0u, 0u};
+            philox4x32_10_args((uint32_t)(2 * blk), a.iteration, e_lo, e_hi, a, wa);
+            if (dims_here > 2) philox4x32_10_args((uint32_t)(2 * blk + 1), a.iteration, e_lo, e_hi, a, wb);
+            U[0] = ((uint64_t)wa[0] << 21) | (wa[1] >> 11);
+            U[1] = ((uint64_t)wa[2] << 21) | (wa[3] >> 11);
+            U[2] = ((uint64_t)wb[0] << 21) | (wb[1] >> 11);
+            U[3] = ((uint64_t)wb[2] << 21) | (wb[3] >> 11);
+            if (G == 4) rot_permute<4>(U, gamma);
+            else if (G == 2) rot_permute<2>(U, gamma);
+        } else {
+            philox4x32_10_args((uint32_t)blk, a.iteration, e_lo, e_hi, a, w);
+            if (G == 4) rot_permute<4>(w, gamma);
+            else if (G == 2) rot_permute<2>(w, gamma);
         }
         // the block's table reads are issued together, then consumed (their latency overlaps)
         typename SP::arg lo[4];
+        double lo53[4];
+        (void)lo53;
         T2 ent[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
@@ -492,9 +543,11 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
                 const bool active = !(last && R == 3) || ((gamma ^ i) < 3);
                 uint32_t b = 0;
                 lo[i] = 0;
+                lo53[i] = 0.0;
                 ent[i] = T2{};
                 if (active) {
-                    SP::split(w[i], (uint32_t)nb, nb_2m32, b, lo[i]);
+                    if constexpr (VAR == kVarU53) RotVarU53::split(U[i], (uint32_t)nb, b, lo53[i]);
+                    else SP::split(w[i], (uint32_t)nb, nb_2m32, b, lo[i]);
                     // one multiply-add (written in C the compiler turns it into shifts and masks of the split product)
                     uint32_t taddr;
                     asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(taddr) : "r"(b), "n"(NBLK * 128), "r"(last ? L.txL[i] : L.tx4[i]));
@@ -507,8 +560,23 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
         for (int i = 0; i < NSUB; ++i) {
             const bool active = !(last && R == 3) || ((gamma ^ i) < 3);
             if (active) {
-                jac[i & (NCH - 1)] *= ent[i].y;
-                f.dim(SP::u(ent[i], lo[i]), blk, i, ctx);
+                if constexpr (VAR == kVarQ32) {
+                    // C4': x = X~_b + Delta~_b r from the fp32 pair, then the integrand's affine variable
+                    const double x0 = (double)ent[i].x, dl = (double)ent[i].y;
+                    const double r = fma((double)lo[i], 2.3283064365386963e-10, 1.1641532182693481e-10);
+                    const double x = fma(dl, r, x0);
+                    double sc, sh;
+                    if (FID == VEGAS_F_CONST || FID == VEGAS_F_GAUSS) { sc = a.scale[0]; sh = a.shift[0]; }
+                    else { const int j = 4 * blk + (gamma ^ i); sc = a.scale[j]; sh = a.shift[j]; }
+                    jac[i & (NCH - 1)] *= (T)dl;
+                    f.dim((T)((x - sh) * sc), blk, i, ctx);
+                } else if constexpr (VAR == kVarU53) {
+                    jac[i & (NCH - 1)] *= ent[i].y;
+                    f.dim((T)fma((double)ent[i].y, lo53[i], (double)ent[i].x), blk, i, ctx);
+                } else {
+                    jac[i & (NCH - 1)] *= ent[i].y;
+                    f.dim(SP::u(ent[i], lo[i]), blk, i, ctx);
+                }
             }
         }
     }
@@ -629,11 +697,10 @@ static __device__ __noinline__ void rot_tail(const RotArgs& a, int dim, unsigned
     }
 }
 
-template <int FID, typename T, int DIM>
+template <int FID, typename T, int DIM, int VAR = 0>
 __global__ void __launch_bounds__(rot_max_threads(FID, DIM), 1)
 k_iterate_rot(const __grid_constant__ RotArgs a) {
-    using E = RotEntry<T>;
-    using T2 = typename E::type;
+    using T2 = typename RotTableEntry<T, VAR>::type;
     using Lane = RotLane<T, DIM>;
     constexpr int NBLK = Lane::NBLK, GL = Lane::GL;
     constexpr int ENTRY = (int)sizeof(T2);
@@ -672,7 +739,9 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
             T2 ent = T2{};
             if (j < DIM) {
                 const double* X = stage_e + j * (nb + 1);
-                ent = RotSplit<T, rot_word_map(8 * (int)sizeof(T), DIM)>::make(X[b], X[b + 1], a.shift[j], a.scale[j], b, nb);
+                if constexpr (VAR == kVarU53) ent = RotVarU53::make(X[b], X[b + 1], a.shift[j], a.scale[j]);
+                else if constexpr (VAR == kVarQ32) ent = RotVarQ32::make(X[b], X[b + 1]);
+                else ent = RotSplit<T, rot_word_map(8 * (int)sizeof(T), DIM)>::make(X[b], X[b + 1], a.shift[j], a.scale[j], b, nb);
             }
             reinterpret_cast<T2*>(table)[idx] = ent;
         }
@@ -738,7 +807,7 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
             uint32_t haddr[NBLK][4];
             double obs_val = 0.0;
             const bool live = q < c_end;
-            const double v = rot_event<FID, T, DIM>(a, L, ctx, first_lo + q, e_hi, live, fin0, fin1, haddr, obs_val);
+            const double v = rot_event<FID, T, DIM, VAR>(a, L, ctx, first_lo + q, e_hi, live, fin0, fin1, haddr, obs_val);
             const double v2 = v * v;
 #ifdef VEGAS_USER_INTEGRAND
             if constexpr (FID == VEGAS_F_USER) {
@@ -854,8 +923,8 @@ inline size_t rot_shared_bytes(int dim, int n_bins, int n_groups) {
            sizeof(double) * kRotMaxObsBins + 8 * (size_t)kRotMaxSections * kRotScratchWarps;
 }
 
-// one translation unit per (FID, T) instantiates DIM = 1..32 (vegas_rot_inst.cu)
-template <int FID, typename T>
+// one translation unit per (FID, T, VAR) instantiates DIM = 1..32 (vegas_rot_inst.cu)
+template <int FID, typename T, int VAR = 0>
 cudaError_t launch_iterate_rot(int dim, const RotArgs& a, int blocks, int threads, size_t shmem, cudaStream_t st);
 #endif
 

@@ -340,7 +340,27 @@ __global__ void k_debug_rot(const __grid_constant__ DebugArgs a) {
         const double* X = a.edges + (size_t)j * (nb + 1);
         typename E::type ent;
         T u;
-        if (sizeof(T) == 8 && a.word_map) {                   // the fast path's own split and map for this shape
+        double x_var = 0.0;
+        uint32_t word_var = word;
+        if (sizeof(T) == 8 && a.variant == kVarU53) {          // C3': two words per draw, block j >> 1
+            uint32_t o4[4];
+            philox4x32_10((uint32_t)(j >> 1), a.iteration, (uint32_t)e, (uint32_t)(e >> 32), ks, o4);
+            const uint32_t hi = (j & 1) ? o4[2] : o4[0], lw = (j & 1) ? o4[3] : o4[1];
+            const uint64_t U = ((uint64_t)hi << 21) | (lw >> 11);
+            double o;
+            RotVarU53::split(U, (uint32_t)nb, b, o);
+            const double2 ev = RotVarU53::make(X[b], X[b + 1], a.shift[j], a.scale[j]);
+            ent.x = (T)ev.x; ent.y = (T)ev.y;
+            u = (T)fma(ev.y, o, ev.x);
+            x_var = fma(X[b + 1] - X[b], o * 1.1102230246251565e-16, X[b]);
+            word_var = hi;
+        } else if (sizeof(T) == 8 && a.variant == kVarQ32) {   // C4': the fp32 pair (X~_b, Delta~_b)
+            const float2 q = RotVarQ32::make(X[b], X[b + 1]);
+            const double r = fma((double)lo, 2.3283064365386963e-10, 1.1641532182693481e-10);
+            x_var = fma((double)q.y, r, (double)q.x);
+            ent.x = (T)q.x; ent.y = (T)q.y;
+            u = (T)((x_var - a.shift[j]) * a.scale[j]);
+        } else if (sizeof(T) == 8 && a.word_map) {                   // the fast path's own split and map for this shape
             using SW = RotSplit<double, true>;
             uint32_t bw;
             double o;
@@ -355,9 +375,10 @@ __global__ void k_debug_rot(const __grid_constant__ DebugArgs a) {
         }
         jac[j & (NCH - 1)] *= ent.y;
         f.dim(u, FID == VEGAS_F_BW_POLY ? (j >> 2) : 0, j & 3, ctx);
-        a.words[(size_t)q * dim + j] = word;
+        a.words[(size_t)q * dim + j] = word_var;
         a.bins[(size_t)q * dim + j] = (int32_t)b;
-        a.x[(size_t)q * dim + j] = (sizeof(T) == 8) ? fma(X[b + 1] - X[b], offset_f64(lo), X[b])
+        a.x[(size_t)q * dim + j] = (sizeof(T) == 8 && a.variant != 0) ? x_var
+                                   : (sizeof(T) == 8) ? fma(X[b + 1] - X[b], offset_f64(lo), X[b])
                                                      : (double)fmaf((float)(X[b + 1] - X[b]),
                                                                     offset_f32_scaled(lo, 5.9604644775390625e-08f, 2.98023223876953125e-08f),
                                                                     (float)X[b]);

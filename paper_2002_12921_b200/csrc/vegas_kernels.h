@@ -49,6 +49,7 @@ struct DebugArgs {
     double post_scale, fin0, fin1, jac_init;
     double shift[VEGAS_MAX_DIM], scale[VEGAS_MAX_DIM];
     double fpar[64];                // RotArgs::fpar (kRotParams)
+    int variant;                    // VEGAS_VARIANT_* (fp64 fast path only): the sampling map of this grid
     int word_map;                   // fp64: this shape's fast-path kernel uses the word-affine table entries (rot_word_map)
 };
 

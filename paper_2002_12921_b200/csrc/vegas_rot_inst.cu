@@ -1,9 +1,14 @@
-// vegas_rot_inst.cu -- instantiates k_iterate_rot<ROT_FID, T, DIM> for DIM = 1..32 (BW_POLY: 2..8).
-// Compiled once per (ROT_FID, ROT_FP) pair by build.py so that the pairs build in parallel.
+// vegas_rot_inst.cu -- instantiates k_iterate_rot<ROT_FID, T, DIM, ROT_VAR> for DIM = 1..32 (BW_POLY: 2..8).
+// Compiled once per (ROT_FID, ROT_FP, ROT_VAR) triple by build.py so that they build in parallel
+// (ROT_VAR: 0 = the method, 1 = 53-bit uniforms, 2 = fp32-rounded table; the variants are fp64 only).
 #include "vegas_iterate_rot.cuh"
 
 #ifndef ROT_FID
 #error "compile with -DROT_FID=<integrand id> -DROT_FP=<64|32>"
+#endif
+
+#ifndef ROT_VAR
+#define ROT_VAR 0
 #endif
 
 namespace vegas {
@@ -16,7 +21,7 @@ using RT = float;
 
 template <int DIM>
 static cudaError_t go(const RotArgs& a, int blocks, int threads, size_t shmem, cudaStream_t st) {
-    auto kern = k_iterate_rot<ROT_FID, RT, DIM>;
+    auto kern = k_iterate_rot<ROT_FID, RT, DIM, ROT_VAR>;
     static size_t configured_dev[kMaxDevices] = {};   // per device: the attribute is per context
     int dev_ = 0;
     if (cudaGetDevice(&dev_) != cudaSuccess || dev_ < 0 || dev_ >= kMaxDevices) return cudaErrorInvalidDevice;
@@ -40,7 +45,7 @@ static cudaError_t go(const RotArgs& a, int blocks, int threads, size_t shmem, c
 }
 
 template <>
-cudaError_t launch_iterate_rot<ROT_FID, RT>(int dim, const RotArgs& a, int blocks, int threads, size_t shmem,
+cudaError_t launch_iterate_rot<ROT_FID, RT, ROT_VAR>(int dim, const RotArgs& a, int blocks, int threads, size_t shmem,
                                             cudaStream_t st) {
     switch (dim) {
 #define CASE(D) case D: return go<D>(a, blocks, threads, shmem, st);

@@ -1,0 +1,165 @@
+"""Parity of the two opt-in variants of the sampling map (readings C3', C4') against the
+oracle's own variant modes, element by element, on the same seeded inputs: 53-bit uniforms from two Philox words per
+draw (VEGAS_VARIANT_U53) and grid-table entries rounded to fp32 (VEGAS_VARIANT_Q32).  Same tolerances as the method
+itself: top words and bins bit-exact; I, sigma, H <= 1e-10 relative; refined edges <= 1e-10 absolute."""
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import oracle as O
+from paper_2002_12921_b200 import workloads as W
+
+THREADS = os.cpu_count() or 8
+RTOL64 = 1e-10
+ORACLE_VARIANT = {1: O.V_U53, 2: O.V_Q32}
+
+SMALL = {
+    1: dict(n_events=100_000, n_iter=3),
+    2: dict(n_events=400_003, n_iter=3),
+    3: dict(n_events=300_007, n_iter=3),
+    4: dict(n_events=200_003, n_iter=3),
+    5: dict(n_events=500_009, n_iter=3, chunk_events=125_000),
+}
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
+    from paper_2002_12921_b200 import build
+    build.build()
+    from paper_2002_12921_b200 import binding
+    return binding
+
+
+def _grid(B, w, variant, edges=None):
+    g = B.VegasGrid(w.dim, w.n_bins)
+    g.set_params(w.integrand_id, w.params)
+    g.set_variant(variant)
+    assert g.get_variant() == variant
+    if edges is not None:
+        g.set_edges(edges)
+    return g
+
+
+@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("cfg", [1, 3, 4, 5])
+def test_variant_words_bins_and_events(B, cfg, variant):
+    w = W.config(cfg)
+    edges = W.adapted_edges(w.dim, w.n_bins, seed=cfg)
+    g = _grid(B, w, variant, edges)
+    count = 40_000
+    for first, it in ((0, 0), ((1 << 32) - 1000, 1), ((5 << 32) + 17, 0xFFFFFFFE)):
+        gw, gb, gx, gf = g.debug_sample(first, count, w.seed, it, w.integrand_id, 64)
+        ow, ob, ox, of = O.sample(edges, w.seed, it, first, count, w.integrand_id, w.params,
+                                  variant=ORACLE_VARIANT[variant])
+        assert np.array_equal(gw, ow)                      # U53: the top 32 bits of U
+        assert np.array_equal(gb, ob)
+        np.testing.assert_allclose(gx, ox, rtol=5e-16, atol=0)
+        np.testing.assert_allclose(gf, of, rtol=1e-12, atol=0)
+    g.close()
+
+
+@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_variant_iterate_and_refine_on_oracle_grids(B, cfg, variant):
+    w = W.config(cfg).scaled(**SMALL[cfg])
+    ch = O.integrate(w.dim, w.n_bins, w.n_iter, w.n_events, w.seed, w.alpha, w.integrand_id, w.params,
+                     threads=THREADS, variant=ORACLE_VARIANT[variant])
+    g = _grid(B, w, variant)
+    assert g.get_launch(w.integrand_id, 64)["path"] == "rotated"
+    for k in range(w.n_iter):
+        g.set_edges(ch["edges_trace"][k])
+        I, s, H, st = g.iterate(w.n_events, w.seed, k, w.integrand_id, 64, chunk_events=w.chunk_events)
+        assert st == 0
+        assert I == pytest.approx(ch["per_iter"][k, 0], rel=RTOL64)
+        assert s == pytest.approx(ch["per_iter"][k, 1], rel=RTOL64)
+        np.testing.assert_allclose(H, ch["hist_trace"][k], rtol=RTOL64, atol=0)
+        assert np.all(H[ch["hist_trace"][k] == 0] == 0)
+        assert g.refine(w.alpha) == 0                       # S8 on the fp64 master grid with this histogram
+        want = ch["edges_trace"][k + 1] if k + 1 < w.n_iter else ch["edges"]
+        np.testing.assert_allclose(g.get_edges(), want, rtol=0, atol=1e-10)
+    g.close()
+
+
+@pytest.mark.parametrize("variant", [1, 2])
+def test_variant_free_running_chain_and_five_sigma(B, variant):
+    w = W.config(2).scaled(n_events=1_000_003, n_iter=5)
+    g = _grid(B, w, variant)
+    res = g.integrate(w.n_iter, w.n_events, w.seed, w.alpha, w.integrand_id, 64, n_skip=1)
+    I, sigma = res["I"], res["sigma"]
+    assert abs(I - w.closed_form) <= 5 * sigma
+    ref = O.integrate(w.dim, w.n_bins, w.n_iter, w.n_events, w.seed, w.alpha, w.integrand_id, w.params, n_skip=1,
+                      threads=THREADS, variant=ORACLE_VARIANT[variant])
+    assert I == pytest.approx(ref["I"], rel=1e-6)           # free-running chains amplify rounding (finding F2)
+    assert sigma == pytest.approx(ref["sigma"], rel=1e-4)
+    g.close()
+
+
+def test_variant_shapes_ragged_and_last_blocks(B):
+    # every last-block shape (1..4 dimensions in the last Philox block), odd bin counts, a range crossing 2^32
+    for variant in (1, 2):
+        for dim, nb, fid in ((1, 2, O.GAUSS), (2, 7, O.GAUSS), (3, 33, O.CONST), (5, 50, O.GAUSS), (6, 50, O.GENZ_PRODUCT_PEAK),
+                             (7, 128, O.GAUSS), (10, 64, O.GENZ_PRODUCT_PEAK), (17, 50, O.GAUSS), (32, 40, O.GAUSS)):
+            rng = np.random.default_rng(dim * 100 + nb)
+            params = {O.GAUSS: [0.35], O.CONST: [],
+                      O.GENZ_PRODUCT_PEAK: np.concatenate([5 + 10 * rng.random(dim), rng.random(dim)])}[fid]
+            edges = W.adapted_edges(dim, nb, seed=dim + nb)
+            g = B.VegasGrid(dim, nb)
+            g.set_params(fid, params)
+            g.set_variant(variant)
+            g.set_edges(edges)
+            n, first = 70_001, (1 << 32) - 30_000
+            g.begin_iteration()
+            g.accumulate(first, n, 9, 2, fid, 64)
+            g.reduce()
+            I, s, H, st = g.finalize(n)
+            S1, S2, Ho = O.accumulate(edges, 9, 2, first, n, fid, params, variant=ORACLE_VARIANT[variant])
+            oI, oS = O.estimate(S1, S2, n)
+            assert I == pytest.approx(oI, rel=RTOL64) and s == pytest.approx(oS, rel=RTOL64)
+            np.testing.assert_allclose(H, Ho.astype(np.float64), rtol=RTOL64, atol=0)
+            g.close()
+
+
+def test_variant_is_opt_in_and_fp64_fast_path_only(B):
+    w = W.config(1)
+    g = _grid(B, w, 0)
+    base = g.iterate(50_000, w.seed, 0, w.integrand_id, 64)
+    g.set_variant(B.VEGAS_VARIANT_Q32)
+    q32 = g.iterate(50_000, w.seed, 0, w.integrand_id, 64)
+    assert q32[0] != base[0] and q32[0] == pytest.approx(base[0], rel=1e-6)      # same sample, fp32-rounded map
+    g.set_variant(B.VEGAS_VARIANT_U53)
+    u53 = g.iterate(50_000, w.seed, 0, w.integrand_id, 64)
+    assert abs(u53[0] - base[0]) > 1e-6 * abs(base[0])                           # a different sample
+    g.set_variant(B.VEGAS_VARIANT_NONE)
+    again = g.iterate(50_000, w.seed, 0, w.integrand_id, 64)
+    assert again[0] == base[0] and again[1] == base[1] and np.array_equal(again[2], base[2])
+    # rejected: an unknown mask, fp32 with a variant, the generic kernel with a variant
+    with pytest.raises(B.VegasError):
+        g.set_variant(3)
+    g.set_variant(B.VEGAS_VARIANT_U53)
+    with pytest.raises(B.VegasError):
+        g.iterate(1000, 1, 0, w.integrand_id, 32)
+    g.set_launch(0, 0, 2, 2)                                                     # pins the generic kernel
+    with pytest.raises(B.VegasError):
+        g.iterate(1000, 1, 0, w.integrand_id, 64)
+    g.close()
+
+
+def test_q32_bias_is_within_its_bound(B):
+    # what C4' costs: the rounded bins do not tile [0,1) exactly.  On f = 1 (J alone) the estimate moves by at most
+    # dim 2^-24 relative; measured value recorded in DESIGN.md section 11
+    dim, nb = 20, 50
+    edges = W.adapted_edges(dim, nb, seed=3)
+    g = B.VegasGrid(dim, nb)
+    g.set_edges(edges)
+    n = 2_000_000
+    I0 = g.iterate(n, 5, 0, B.VEGAS_F_CONST, 64, want_hist=False)[0]
+    g.set_variant(B.VEGAS_VARIANT_Q32)
+    I1 = g.iterate(n, 5, 0, B.VEGAS_F_CONST, 64, want_hist=False)[0]
+    assert abs(I1 / I0 - 1) <= dim * 2.0**-24
+    g.close()

@@ -425,6 +425,14 @@ constexpr int kRotNamedDefaultWarps = 12;
 __host__ __device__ constexpr int rot_sections(int fid, int dim) {
     return !rot_mbar_tokens(fid, dim) ? 1 : ((dim + 3) / 4 < VEGAS_ROT_NSEC ? (dim + 3) / 4 : VEGAS_ROT_NSEC);
 }
+// Two events per token hold (template parameter PAIR of the kernel, picked at launch when warps share a histogram
+// copy): the shapes with 3 Philox blocks, whose 128 registers have room for a second set of histogram addresses and
+// whose large tables leave few copies (cfg4: 2 copies, 7 warps each).  Measured on cfg4: 5.45e10 -> 5.53e10 events/s,
+// barrier stalls per issue 3.97 -> 2.53 (profiles/r02_k1_steps.md); a kernel of its own because the second loop
+// in the same kernel cost the shapes without rings 5 %.
+__host__ __device__ constexpr bool rot_pair_hold(int fid, int dim, int var = 0) {
+    return fid != VEGAS_F_USER && fid != VEGAS_F_BW_POLY && var == 0 && dim >= 9 && dim <= 12;
+}
 __host__ __device__ constexpr int rot_section_begin(int nblk, int nsec, int s) { return (s * nblk + nsec - 1) / nsec; }
 constexpr int kRotMaxSections = 8;
 constexpr int kRotScratchWarps = 32;   // sizing of the per-warp scratch (reduction slots, tokens): any CTA has <= 32 warps
@@ -600,50 +608,67 @@ __device__ __forceinline__ double rot_event(const RotArgs& a, const RotLane<T, D
 // the warp touch pairwise different words (different rows per block; inside a row each lane has its own column), so
 // the read-modify-writes of a round are independent and pipeline.  Consecutive rounds can touch the same word from
 // different lanes, hence the __syncwarp() (shared memory is processed in order per warp).
-template <typename T, int DIM, int B0, int B1>
-__device__ __forceinline__ void rot_hist_update(const uint32_t (&haddr)[(DIM + 3) / 4][4], int gammaL, double v2) {
+template <typename T, int DIM, int B0, int B1, bool PAIR>
+__device__ __forceinline__ void rot_hist_update(const uint32_t (&haddr)[(DIM + 3) / 4][4], const uint32_t (&haddrB)[(DIM + 3) / 4][4],
+                                                int gammaL, double v2, double v2B) {
     constexpr int NBLK = RotLane<T, DIM>::NBLK, R = RotLane<T, DIM>::R;
+    const double v2AB = v2 + v2B;
+    (void)v2AB;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        double h[NBLK];
+        double h[NBLK], hB[NBLK];
+        (void)hB;
 #pragma unroll
         for (int blk = B0; blk < B1; ++blk) {
             const bool last = (blk == NBLK - 1);
             const int NSUB = last ? ((R == 3) ? 4 : R) : 4;
             const bool active = (i < NSUB) && (!(last && R == 3) || ((gammaL ^ i) < 3));
-            if (active) h[blk] = lds_f64(haddr[blk][i] + (uint32_t)(blk * 256));
+            if (active) {
+                h[blk] = lds_f64(haddr[blk][i] + (uint32_t)(blk * 256));
+                if (PAIR) hB[blk] = lds_f64(haddrB[blk][i] + (uint32_t)(blk * 256));
+            }
         }
 #pragma unroll
         for (int blk = B0; blk < B1; ++blk) {
             const bool last = (blk == NBLK - 1);
             const int NSUB = last ? ((R == 3) ? 4 : R) : 4;
             const bool active = (i < NSUB) && (!(last && R == 3) || ((gammaL ^ i) < 3));
-            if (active) sts_f64(haddr[blk][i] + (uint32_t)(blk * 256), h[blk] + v2);
+            if (active) {
+                if (PAIR) {
+                    // two events of this lane in one round: when both fall into the same word the second event's store
+                    // goes first and the first event's store, which carries both weights, lands on top of it
+                    // (one lane, program order)
+                    const bool same = haddr[blk][i] == haddrB[blk][i];
+                    sts_f64(haddrB[blk][i] + (uint32_t)(blk * 256), hB[blk] + v2B);
+                    sts_f64(haddr[blk][i] + (uint32_t)(blk * 256), h[blk] + (same ? v2AB : v2));
+                } else {
+                    sts_f64(haddr[blk][i] + (uint32_t)(blk * 256), h[blk] + v2);
+                }
+            }
         }
         __syncwarp();
     }
 }
 
-// the sections of one event's histogram update, each under its own token
-template <typename T, int DIM, int SEC, int NSEC, bool MBAR>
-__device__ __forceinline__ void rot_hist_sections(const uint32_t (&haddr)[(DIM + 3) / 4][4], int gammaL, double v2, bool ring,
+// the sections of one event's (PAIR: two events') histogram update, each under its own token
+template <typename T, int DIM, int SEC, int NSEC, bool MBAR, bool PAIR>
+__device__ __forceinline__ void rot_hist_sections(const uint32_t (&haddr)[(DIM + 3) / 4][4], const uint32_t (&haddrB)[(DIM + 3) / 4][4],
+                                                  int gammaL, double v2, double v2B, bool ring,
                                                   bool wait, uint32_t my_tok, uint32_t next_tok, uint32_t tok_stride,
-                                                  uint32_t parity, bool lane0
-                                                  ) {
+                                                  uint32_t parity, bool lane0) {
     if constexpr (SEC < NSEC) {
         constexpr int NBLK = (DIM + 3) / 4;
         if (wait) {
             if (MBAR) token_wait(my_tok + SEC * tok_stride, parity);
             else token_wait_named((int)my_tok);
         }
-        rot_hist_update<T, DIM, rot_section_begin(NBLK, NSEC, SEC), rot_section_begin(NBLK, NSEC, SEC + 1)>(haddr, gammaL, v2);
+        rot_hist_update<T, DIM, rot_section_begin(NBLK, NSEC, SEC), rot_section_begin(NBLK, NSEC, SEC + 1), PAIR>(haddr, haddrB, gammaL, v2, v2B);
         if (MBAR) {
             if (ring && lane0) token_pass(next_tok + SEC * tok_stride);     // after the __syncwarp() of the last round
         } else if (ring) {
             token_pass_named((int)next_tok);
         }
-        rot_hist_sections<T, DIM, SEC + 1, NSEC, MBAR>(haddr, gammaL, v2, ring, wait, my_tok, next_tok, tok_stride, parity, lane0
-                                                 );
+        rot_hist_sections<T, DIM, SEC + 1, NSEC, MBAR, PAIR>(haddr, haddrB, gammaL, v2, v2B, ring, wait, my_tok, next_tok, tok_stride, parity, lane0);
     }
 }
 
@@ -697,7 +722,7 @@ static __device__ __noinline__ void rot_tail(const RotArgs& a, int dim, unsigned
     }
 }
 
-template <int FID, typename T, int DIM, int VAR = 0>
+template <int FID, typename T, int DIM, int VAR = 0, bool PAIR = false>
 __global__ void __launch_bounds__(rot_max_threads(FID, DIM), 1)
 k_iterate_rot(const __grid_constant__ RotArgs a) {
     using T2 = typename RotTableEntry<T, VAR>::type;
@@ -715,6 +740,7 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     (void)obs_sh;
     constexpr int NSEC = rot_sections(FID, DIM);
     constexpr bool MBAR = rot_mbar_tokens(FID, DIM);
+    constexpr bool kPairHold = PAIR;
     const uint32_t tok_base = (uint32_t)__cvta_generic_to_shared(obs_sh + kRotMaxObsBins);   // [NSEC][warps] mbarriers
 
     // Programmatic dependent launch between the chunk launches of one accumulate call: the next chunk's CTAs may start
@@ -803,6 +829,24 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
         const uint32_t n_iter = (c_end - c0 + nthr - 1) / nthr;
         double s1 = 0.0, s2 = 0.0;
         uint32_t q = c0 + tid;
+        if (kPairHold && ring) {
+            // two events per token hold (rings only): the four dependent read-modify-write rounds of a hold and its
+            // hand-off are what a saturated ring is bound by (cfg4: 7 warps per copy); two events share them
+            for (uint32_t it = 0; it < n_iter; it += 2, q += 2 * nthr, ++tick) {
+                uint32_t haddr[NBLK][4], haddrB[NBLK][4];
+                double obs_val = 0.0;
+                const double v = rot_event<FID, T, DIM, VAR>(a, L, ctx, first_lo + q, e_hi, q < c_end, fin0, fin1, haddr, obs_val);
+                const double vB = rot_event<FID, T, DIM, VAR>(a, L, ctx, first_lo + q + nthr, e_hi, q + nthr < c_end, fin0, fin1, haddrB, obs_val);
+                const double v2 = v * v, v2B = vB * vB;
+                s1 += v;
+                s2 += v2;
+                s1 += vB;
+                s2 += v2B;
+                rot_hist_sections<T, DIM, 0, NSEC, MBAR, true>(haddr, haddrB, L.gammaL, v2, v2B, ring, !first, my_tok, next_tok, tok_stride,
+                                                                tick & 1u, lane0);
+                first = false;
+            }
+        } else
         for (uint32_t it = 0; it < n_iter; ++it, q += nthr, ++tick) {
             uint32_t haddr[NBLK][4];
             double obs_val = 0.0;
@@ -820,9 +864,8 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
 #endif
             s1 += v;
             s2 += v2;
-            rot_hist_sections<T, DIM, 0, NSEC, MBAR>(haddr, L.gammaL, v2, ring, ring && !first, my_tok, next_tok, tok_stride,
-                                               tick & 1u, lane0
-                                               );
+            rot_hist_sections<T, DIM, 0, NSEC, MBAR, false>(haddr, haddr, L.gammaL, v2, 0.0, ring, ring && !first, my_tok, next_tok, tok_stride,
+                                                            tick & 1u, lane0);
             first = false;
         }
         a1 = dd_add(a1, dd{s1, 0.0});

@@ -19,10 +19,10 @@ using RT = double;
 using RT = float;
 #endif
 
-template <int DIM>
-static cudaError_t go(const RotArgs& a, int blocks, int threads, size_t shmem, cudaStream_t st) {
-    auto kern = k_iterate_rot<ROT_FID, RT, DIM, ROT_VAR>;
-    static size_t configured_dev[kMaxDevices] = {};   // per device: the attribute is per context
+template <int DIM, bool PAIR>
+static cudaError_t go_kernel(const RotArgs& a, int blocks, int threads, size_t shmem, cudaStream_t st) {
+    auto kern = k_iterate_rot<ROT_FID, RT, DIM, ROT_VAR, PAIR>;
+    static size_t configured_dev[kMaxDevices] = {};   // per kernel and device: the attribute is per context
     int dev_ = 0;
     if (cudaGetDevice(&dev_) != cudaSuccess || dev_ < 0 || dev_ >= kMaxDevices) return cudaErrorInvalidDevice;
     size_t& configured = configured_dev[dev_];
@@ -42,6 +42,15 @@ static cudaError_t go(const RotArgs& a, int blocks, int threads, size_t shmem, c
     cfg.attrs = attr;
     cfg.numAttrs = a.pdl ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, kern, a);
+}
+
+// rings of the 3-block shapes run the two-events-per-hold kernel (rot_pair_hold)
+template <int DIM>
+static cudaError_t go(const RotArgs& a, int blocks, int threads, size_t shmem, cudaStream_t st) {
+    if constexpr (rot_pair_hold(ROT_FID, DIM, ROT_VAR)) {
+        if (a.ring > 1) return go_kernel<DIM, true>(a, blocks, threads, shmem, st);
+    }
+    return go_kernel<DIM, false>(a, blocks, threads, shmem, st);
 }
 
 template <>

@@ -189,7 +189,7 @@ bool use_rot_path(const vegas_grid* g, int fid, int precision) {
     if (g->cfg_ct > 0 || g->cfg_ch > 0) return false;
     (void)precision;
     const bool kind = fid == VEGAS_F_CONST || fid == VEGAS_F_GAUSS || fid == VEGAS_F_GENZ_PRODUCT_PEAK ||
-                      (fid == VEGAS_F_BW_POLY && g->dim <= vegas::kRotBwMaxDim);
+                      fid == VEGAS_F_BW_POLY;
     if (!kind) return false;
     return vegas::rot_shared_bytes(g->dim, g->n_bins, 1) <= g->smem_optin;
 }
@@ -247,6 +247,13 @@ void rot_constants(const vegas_grid* g, int fid, int precision, double* shift, d
         double ps = nb / scale[0];
         for (int j = 1; j < dim; ++j) { scale[j] = 1.0; ps *= nb; }
         *post_scale = ps;                                        // J = prod nb Delta_j = prod (nb/scale_j) B_j 2^32
+        if (precision == VEGAS_FP32) {
+            // fp32 (C11): n_bins^d is shared out over the four chains (IntegrandU<BW_POLY>::value)
+            const float q32 = (float)std::pow(nb, 0.25 * dim);
+            *fin1 = (double)q32;
+            *post_scale = std::exp((double)dim * std::log(nb) - 4.0 * std::log((double)q32)) / scale[0];
+        }
+        for (int k = 0; k < 5; ++k) fpar[k] = 0.0;               // row 0: the Breit-Wigner dimension has no polynomial
         for (int j = 1; j < dim; ++j)
             for (int k = 0; k < 5; ++k) fpar[5 * j + k] = d[4 + 5 * (j - 1) + k];
     }
@@ -886,7 +893,7 @@ int vegas_debug_sample(vegas_grid* g, uint64_t first_event, uint32_t count, uint
     CUDA_TRY(g, cudaSetDevice(g->device));
     const size_t per_dim = (size_t)count * g->dim;
     unsigned char* base = (unsigned char*)dev_scratch;
-    vegas::DebugArgs a;
+    vegas::DebugArgs a{};
     a.edges = g->d_edges;
     a.first_event = first_event;
     a.count = count;

@@ -52,9 +52,9 @@ template <int FID, typename T, int NBLK> struct RotCtx {
 // 15-warp CTA is tight and the extra accumulators cost more than the shorter chains give (cfg3: 3.85e10 events/s
 // with 1 chain and Horner exp, 3.76e10 with 2 chains, 3.68e10 with 4 chains and Estrin; cfg4: 4.93e10 -> 5.24e10
 // and cfg2: 8.03e10 -> 8.10e10 with 4)
-// (fp32 product peak: always 4, so that no partial product of (1 + u^2) leaves the fp32 range, see its value())
+// (fp32 product peak and fp32 BW_POLY: always 4, so that no partial product leaves the fp32 range, see their value())
 __host__ __device__ constexpr int rot_chains(int dim, int fid = -1, bool fp32 = false) {
-    return (fp32 && fid == VEGAS_F_GENZ_PRODUCT_PEAK) ? 4 : (dim > 12 ? 1 : 4);
+    return (fp32 && (fid == VEGAS_F_GENZ_PRODUCT_PEAK || fid == VEGAS_F_BW_POLY)) ? 4 : (dim > 12 ? 1 : 4);
 }
 template <int NCH, typename T> __device__ __forceinline__ T chain_sum(const T (&s)[NCH]) {
     if (NCH == 4) return (s[0] + s[NCH > 1 ? 1 : 0]) + (s[NCH > 2 ? 2 : 0] + s[NCH > 3 ? 3 : 0]);
@@ -120,9 +120,11 @@ template <typename T, int NCH> struct IntegrandU<VEGAS_F_GENZ_PRODUCT_PEAK, T, N
 // BW_POLY (BASELINE.json:configs[4], readings R11, R12): u_0 = (s(x_0) - M^2)/(M Gamma), u_j = x_j for j >= 1;
 // f = [1/(1 + u_0^2)] * [sum_j a_j0 + sum_j u_j (a_j1 + u_j (a_j2 + u_j (a_j3 + u_j a_j4)))].
 // The lane that holds dimension 0 at sub-step i of block 0 runs the quartic with zero coefficients and keeps u.
-constexpr int kRotBwMaxDim = 8;    // 4 coefficient registers pairs per dimension per lane
+constexpr int kRotBwMaxDim = 8;    // up to here a lane keeps the 4 coefficients of each of its dimensions in registers;
+                                   // beyond, it reads them from the kernel arguments (constant bank) by dimension index
 constexpr int kRotMaxObsBins = 128; // observable histogram of a user integrand (vegas_set_observable)
-constexpr int kRotParams = 64;     // doubles of integrand parameters carried in the kernel arguments (VEGAS_USER_MAX_PARAMS)
+constexpr int kRotParams = 5 * VEGAS_MAX_DIM;   // doubles of integrand parameters carried in the kernel arguments
+                                                // (BW_POLY: 5 per dimension; USER: VEGAS_USER_MAX_PARAMS = 64 of them)
 template <typename T, int NCH> struct IntegrandU<VEGAS_F_BW_POLY, T, NCH> {
     T poly[NCH], u0;
     template <class C> __device__ __forceinline__ void begin(const C& c) {
@@ -131,15 +133,25 @@ template <typename T, int NCH> struct IntegrandU<VEGAS_F_BW_POLY, T, NCH> {
         u0 = (T)0;
     }
     template <class C> __device__ __forceinline__ void dim(T u, int blk, int i, const C& c) {
-        T h = t_fma(c.a[blk][i][3], u, c.a[blk][i][2]);
-        h = t_fma(h, u, c.a[blk][i][1]);
-        h = t_fma(h, u, c.a[blk][i][0]);
+        T h = t_fma(c.coef(blk, i, 3), u, c.coef(blk, i, 2));
+        h = t_fma(h, u, c.coef(blk, i, 1));
+        h = t_fma(h, u, c.coef(blk, i, 0));
         poly[i & (NCH - 1)] = t_fma(h, u, poly[i & (NCH - 1)]);
-        if (blk == 0 && c.is0[i]) u0 = u;
+        if (blk == 0 && c.dim0(i)) u0 = u;
     }
     // reciprocal first: it depends on u_0 alone, so it runs beside the polynomial chains; one multiply follows them
     __device__ __forceinline__ T finish(T, T) const { return chain_sum<NCH, T>(poly) * ((T)1 / t_fma(u0, u0, (T)1)); }
-    __device__ __forceinline__ T value(const T (&jac)[NCH], T fin0, T fin1) const { return finish(fin0, fin1) * chain_prod<NCH, T>(jac); }
+    // fp32 (C11): prod Delta_j alone leaves the fp32 range in many dimensions (u_j = x_j: the table carries no
+    // n_bins); each of the 4 chains takes a quarter of n_bins^d first: fin1 = n_bins^(d/4), the rest is in post_scale
+    __device__ __forceinline__ T value(const T (&jac)[NCH], T fin0, T fin1) const {
+        if (sizeof(T) == 4 && NCH == 4) {
+            T r[NCH];
+#pragma unroll
+            for (int c = 0; c < NCH; ++c) r[c] = jac[c] * fin1;
+            return finish(fin0, fin1) * chain_prod<NCH, T>(r);
+        }
+        return finish(fin0, fin1) * chain_prod<NCH, T>(jac);
+    }
 };
 
 // ---- table entry and u from the low product word ---------------------------------------------------
@@ -339,16 +351,20 @@ struct RotArgs {
 };
 
 template <typename T, int NBLK> struct RotCtx<VEGAS_F_BW_POLY, T, NBLK> {
-    T a[NBLK][4][4];                // a_j1..a_j4 of the lane's dimension at (blk, i); zero for dimension 0 / no dimension
+    static constexpr bool kRegs = NBLK <= kRotBwMaxDim / 4;
+    T a[kRegs ? NBLK : 1][4][4];    // a_j1..a_j4 of the lane's dimension at (blk, i); zero for dimension 0 / no dimension
     bool is0[4];                    // the lane holds dimension 0 at sub-step i of block 0
     T poly0;                        // sum_j a_j0
-    template <class A> __device__ __forceinline__ void init(const A& r, int dim, int gamma4, int gammaL) {
-        const int nblk = (dim + 3) / 4;
+    const double* p;                // more than 8 dimensions: the coefficient rows (RotArgs::fpar; row 0 is zero)
+    int gamma4, gammaL, nblk;
+    template <class A> __device__ __forceinline__ void init(const A& r, int dim, int g4, int gL) {
+        nblk = (dim + 3) / 4;
+        gamma4 = g4; gammaL = gL; p = r.fpar;
         T c0 = (T)0;
         for (int j = 1; j < dim; ++j) c0 += (T)r.fpar[5 * j];
         poly0 = c0;
 #pragma unroll
-        for (int blk = 0; blk < NBLK; ++blk)
+        for (int blk = 0; blk < (kRegs ? NBLK : 1); ++blk)
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
                 const int j = 4 * blk + ((blk == nblk - 1 ? gammaL : gamma4) ^ i);
@@ -358,6 +374,11 @@ template <typename T, int NBLK> struct RotCtx<VEGAS_F_BW_POLY, T, NBLK> {
                 if (blk == 0) is0[i] = (j == 0);
             }
     }
+    __device__ __forceinline__ T coef(int blk, int i, int k) const {
+        if (kRegs) return a[kRegs ? blk : 0][i][k];
+        return (T)p[5 * (4 * blk + ((blk == nblk - 1 ? gammaL : gamma4) ^ i)) + 1 + k];
+    }
+    __device__ __forceinline__ bool dim0(int i) const { return is0[i]; }
 };
 
 #ifdef VEGAS_USER_INTEGRAND
@@ -410,7 +431,8 @@ template <typename T, int NCH> struct IntegrandU<VEGAS_F_USER, T, NCH> {
 #define VEGAS_ROT_WIDE_MIN_DIM 13
 #endif
 __host__ __device__ constexpr int rot_max_warps(int fid, int dim) {
-    return (fid == VEGAS_F_USER || (fid == VEGAS_F_BW_POLY && VEGAS_ROT_BW_WARPS == 12)) ? 12 : (dim >= VEGAS_ROT_WIDE_MIN_DIM ? 24 : 16);
+    return (fid == VEGAS_F_USER || (fid == VEGAS_F_BW_POLY && dim <= kRotBwMaxDim && VEGAS_ROT_BW_WARPS == 12))
+               ? 12 : (dim >= VEGAS_ROT_WIDE_MIN_DIM ? 24 : 16);
 }
 __host__ __device__ constexpr int rot_max_threads(int fid, int dim) { return 32 * rot_max_warps(fid, dim); }
 __host__ __device__ constexpr bool rot_mbar_tokens(int fid, int dim) { return rot_max_warps(fid, dim) > 16; }

@@ -84,7 +84,7 @@ __global__ void __launch_bounds__(kIterMaxThreads, kIterMinBlocks)
 k_iterate(const __grid_constant__ IterArgs a, const __grid_constant__ FParams<T> fp) {
     using T2 = typename Vec2<T>::type;
     constexpr bool AFF = (FID != VEGAS_F_BW_POLY);
-    constexpr int NCH = rot_chains(VEGAS_MAX_DIM, FID, sizeof(T) == 4);        // 1, or 4 for the fp32 product peak
+    constexpr int NCH = AFF ? rot_chains(VEGAS_MAX_DIM, FID, sizeof(T) == 4) : 1;   // 1, or 4 for the fp32 product peak
     extern __shared__ __align__(16) unsigned char smem[];
     const int dim = a.dim, nb = a.n_bins, nent = dim * nb;
     const int ct = 1 << a.log_ct, ch = 1 << a.log_ch;
@@ -324,7 +324,7 @@ __global__ void k_debug_rot(const __grid_constant__ DebugArgs a) {
     const unsigned long long e = a.first_event + q;
     const int dim = a.dim, nb = a.n_bins;
     const PhiloxKey ks = philox_key_schedule(a.key0, a.key1);
-    RotCtx<FID, T, kRotBwMaxDim / 4> ctx;      // lane 0's view: gamma = 0, dimension j at (j >> 2, j & 3)
+    RotCtx<FID, T, VEGAS_MAX_DIM / 4> ctx;     // lane 0's view: gamma = 0, dimension j at (j >> 2, j & 3)
     ctx.init(a, dim, 0, 0);
     constexpr int NCH = rot_chains(VEGAS_MAX_DIM, FID, sizeof(T) == 4);     // 1, or 4 for the fp32 product peak
     IntegrandU<FID, T, NCH> f;

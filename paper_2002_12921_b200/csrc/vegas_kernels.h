@@ -48,7 +48,7 @@ struct DebugArgs {
     // fast ("rotated") path only: the affine map and constants of vegas_iterate_rot.cuh
     double post_scale, fin0, fin1, jac_init;
     double shift[VEGAS_MAX_DIM], scale[VEGAS_MAX_DIM];
-    double fpar[64];                // RotArgs::fpar (kRotParams)
+    double fpar[5 * VEGAS_MAX_DIM]; // RotArgs::fpar (kRotParams)
     int variant;                    // VEGAS_VARIANT_* (fp64 fast path only): the sampling map of this grid
     int word_map;                   // fp64: this shape's fast-path kernel uses the word-affine table entries (rot_word_map)
 };

@@ -1,4 +1,4 @@
-// vegas_rot_inst.cu -- instantiates k_iterate_rot<ROT_FID, T, DIM, ROT_VAR> for DIM = 1..32 (BW_POLY: 2..8).
+// vegas_rot_inst.cu -- instantiates k_iterate_rot<ROT_FID, T, DIM, ROT_VAR> for DIM = 1..32 (BW_POLY: 2..32).
 // Compiled once per (ROT_FID, ROT_FP, ROT_VAR) triple by build.py so that they build in parallel
 // (ROT_VAR: 0 = the method, 1 = 53-bit uniforms, 2 = fp32-rounded table; the variants are fp64 only).
 #include "vegas_iterate_rot.cuh"
@@ -58,14 +58,13 @@ cudaError_t launch_iterate_rot<ROT_FID, RT, ROT_VAR>(int dim, const RotArgs& a, 
                                             cudaStream_t st) {
     switch (dim) {
 #define CASE(D) case D: return go<D>(a, blocks, threads, shmem, st);
-#if ROT_FID == VEGAS_F_BW_POLY
-        CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)      // kRotBwMaxDim
-#else
-        CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
+#if ROT_FID != VEGAS_F_BW_POLY
+        CASE(1)
+#endif
+        CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8)
         CASE(9) CASE(10) CASE(11) CASE(12) CASE(13) CASE(14) CASE(15) CASE(16)
         CASE(17) CASE(18) CASE(19) CASE(20) CASE(21) CASE(22) CASE(23) CASE(24)
         CASE(25) CASE(26) CASE(27) CASE(28) CASE(29) CASE(30) CASE(31) CASE(32)
-#endif
 #undef CASE
     default: return cudaErrorInvalidValue;
     }

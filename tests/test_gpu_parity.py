@@ -385,23 +385,33 @@ def test_edge_shapes(B):
 
 
 def test_bw_poly_other_dimensions(B):
-    """Every shape of the last Philox block (1..4 dimensions) on the fast path (dim <= 8), and the generic
-    kernel beyond it (dim 9, 13): the per-lane coefficient registers must follow the lane's dimension."""
-    for dim in (2, 3, 4, 5, 6, 7, 8, 9, 13):
+    """Every shape of the last Philox block (1..4 dimensions) on the fast path: the per-lane coefficient registers
+    (dim <= 8) and the constant-bank coefficient rows (dim > 8, up to the ABI's 32 dimensions) must follow the lane's
+    dimension; both precisions; and the generic kernel when the copy counts are pinned."""
+    for dim in (2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 13, 20, 32):
         p = W.bw_poly_params(dim, 77)
         edges = W.adapted_edges(dim, 40, seed=dim)
         g = B.VegasGrid(dim, 40)
         g.set_params(B.VEGAS_F_BW_POLY, p)
         g.set_edges(edges)
-        assert g.get_launch(B.VEGAS_F_BW_POLY, 64)["path"] == ("rotated" if dim <= 8 else "generic")
+        assert g.get_launch(B.VEGAS_F_BW_POLY, 64)["path"] == "rotated"
         gw, gb, gx, gf = g.debug_sample(5, 4096, 3, 2, B.VEGAS_F_BW_POLY, 64)
         ow, ob, ox, of = O.sample(edges, 3, 2, 5, 4096, O.BW_POLY, p)
         assert np.array_equal(gb, ob)
         np.testing.assert_allclose(gf, of, rtol=1e-12, atol=0)
-        I, s, H, st = g.iterate(100_001, 3, 0, B.VEGAS_F_BW_POLY, 64)
         oI, oS, oH = O.iterate(edges, 100_001, 3, 0, O.BW_POLY, p)
+        I, s, H, st = g.iterate(100_001, 3, 0, B.VEGAS_F_BW_POLY, 64)
         assert I == pytest.approx(oI, rel=RTOL64) and s == pytest.approx(oS, rel=RTOL64)
         _assert_hist(H, oH, 64)
+        I, s, H, st = g.iterate(100_001, 3, 0, B.VEGAS_F_BW_POLY, 32)
+        assert I == pytest.approx(oI, rel=RTOL32) and s == pytest.approx(oS, rel=RTOL32)
+        _assert_hist(H, oH, 32)
+        if dim in (9, 13):
+            g.set_launch(0, 0, 2, 4)
+            assert g.get_launch(B.VEGAS_F_BW_POLY, 64)["path"] == "generic"
+            I, s, H, st = g.iterate(100_001, 3, 0, B.VEGAS_F_BW_POLY, 64)
+            assert I == pytest.approx(oI, rel=RTOL64) and s == pytest.approx(oS, rel=RTOL64)
+            _assert_hist(H, oH, 64)
         g.close()
 
 

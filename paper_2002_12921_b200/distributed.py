@@ -20,17 +20,34 @@ def shard_range(n_events: int, rank: int, world: int):
     return lo, hi - lo
 
 
-def allreduce_totals(totals, group=None):
+def allreduce_totals(totals, group=None, fixed_order: bool = False):
     """Sum the per-rank totals vector in place over the process group (no-op for one process).
-    The (hi, lo) pairs of S1 and S2 are summed component-wise: each stays a valid unevaluated sum."""
+    The (hi, lo) pairs of S1 and S2 are summed component-wise: each stays a valid unevaluated sum.
+
+    fixed_order=False: one all-reduce(sum); the association of the fp64 additions is the collective library's
+    (NCCL ring/tree, gloo): every rank receives the same bits, so the grids stay in lockstep, and a run is
+    reproducible for a fixed world size and algorithm, but not bit-for-bit against another world size.
+    fixed_order=True: all-gather of the R vectors (R x <= 26 KB) and a sum in rank order 0, 1, ..., R-1 on every
+    rank: bit-reproducible whatever the collective does (SURVEY.md 8(e) "reduced in fixed rank order if bitwise
+    reproducibility is wanted")."""
+    import torch
     import torch.distributed as dist
     if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
-        dist.all_reduce(totals, op=dist.ReduceOp.SUM, group=group)
+        if fixed_order:
+            parts = [torch.empty_like(totals) for _ in range(dist.get_world_size(group))]
+            dist.all_gather(parts, totals.contiguous(), group=group)
+            acc = parts[0].clone()
+            for t in parts[1:]:
+                acc += t
+            totals.copy_(acc)
+        else:
+            dist.all_reduce(totals, op=dist.ReduceOp.SUM, group=group)
     return totals
 
 
 def iterate_sharded(grid, n_events_total: int, seed: int, iteration: int, integrand_id: int, precision: int = 64,
-                    chunk_events: int = 0, rank: int = 0, world: int = 1, want_hist: bool = False, group=None):
+                    chunk_events: int = 0, rank: int = 0, world: int = 1, want_hist: bool = False, group=None,
+                    fixed_order: bool = False):
     """One Vegas iteration of n_events_total events spread over `world` ranks; `grid` is this rank's
     binding.VegasGrid.  Returns (I, sigma, hist or None, status), identical on every rank."""
     first, count = shard_range(n_events_total, rank, world)
@@ -39,5 +56,5 @@ def iterate_sharded(grid, n_events_total: int, seed: int, iteration: int, integr
         grid.accumulate(first, count, seed, iteration, integrand_id, precision, chunk_events)
     grid.reduce()
     if world > 1:
-        allreduce_totals(grid.totals_tensor(), group)
+        allreduce_totals(grid.totals_tensor(), group, fixed_order)
     return grid.finalize(n_events_total, want_hist=want_hist)

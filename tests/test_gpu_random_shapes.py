@@ -29,8 +29,6 @@ def B():
 def _case(rng):
     fid = int(rng.integers(0, 4))
     dim = int(rng.integers(2 if fid == 3 else 1, 33))
-    if fid == 3 and dim > 20:
-        dim = int(rng.integers(2, 21))                    # BW_POLY: 4 + 5 (d-1) parameters <= VEGAS_MAX_PARAMS... d <= 32 ok, keep runs short
     nb = int(rng.choice([2, 3, 7, 16, 33, 50, 64, 100, 128, 200, 256]))
     if fid == 0:
         p = None

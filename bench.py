@@ -45,15 +45,19 @@ def n_wide(w):
 
 
 # Refined machine model from the round-2 microbenchmarks (profiles/r02_ubench_pipes.md; "refine them
-# only via the step-0 microbenchmarks"): IMAD.WIDE.U32 runs at 32 lanes/clk/SM (4 clk per warp instruction on the one
-# fma-heavy pipe of a scheduler), IMAD at 64, LOP3/IADD3/SEL at 64 (ALU pipe), one instruction issued per clock.
-# The refined bound per event is the largest of: issue slots (N_issue), fma-heavy clocks (4 N_wide + 2 N_imad) and
-# ALU clocks (2 N_alu), with N_imad = d (table address) and N_alu = 20 ceil(d/4) (XORs) + 2 ceil(d/4) + 3 d + 3.
+# only via the step-0 microbenchmarks"): one Philox round of one block -- 2 IMAD.WIDE.U32 + 2 LOP3 -- costs 9.9 scheduler
+# clocks per warp at 6 warps per scheduler (not the 4 its instruction count suggests), and instructions added to the
+# rounds cost 1.0 .. 1.9 clocks each ON TOP (DFMA, LOP3, IMAD alike): nothing hides under the wide multiplies.  The
+# refined bound charges each of the 20 ceil(d/4) Philox multiply+XOR pairs of the SURVEY count 4.95 clocks instead of 2
+# and every other instruction its one issue slot.
+PHILOX_PAIR_CLK = 4.95
+
+
 def refined_slots(w, precision):
-    d, nblk = w.dim, (w.dim + 3) // 4
-    fma_heavy = 4 * n_wide(w) + 2 * d
-    alu = 2 * (20 * nblk + 2 * nblk + 3 * d + 3)
-    return max(n_issue(w, precision), fma_heavy, alu), {"issue": n_issue(w, precision), "fma_heavy_clk": fma_heavy, "alu_clk": alu}
+    nblk = (w.dim + 3) // 4
+    ni = n_issue(w, precision)
+    extra = (PHILOX_PAIR_CLK - 2.0) * 20 * nblk
+    return ni + extra, {"issue": ni, "philox_pairs": 20 * nblk, "clk_per_pair": PHILOX_PAIR_CLK, "extra_clk": extra}
 
 
 def ncu_traffic(workload, precision):
@@ -261,11 +265,13 @@ def main():
     peaks = measured_peaks()
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
 
-    def measure(w, precision, steps, warmup, label, with_cpu_baseline=False):
+    def measure(w, precision, steps, warmup, label, with_cpu_baseline=False, variant=0):
         """Warm-up (the chain's first iterations adapt the grid), `steps` device-timed steps, the same steps with the
         library's per-launch events (K1 alone), and the same steps end to end through the C ABI with host buffers."""
         g = B.VegasGrid(w.dim, w.n_bins)
         g.set_params(w.integrand_id, w.params)
+        if variant:
+            g.set_variant(variant)
         if args.launch:
             g.set_launch(*[int(v) for v in args.launch.split(",")])
         fid = w.integrand_id
@@ -377,8 +383,9 @@ def main():
                                        "scheduler per clock confirmed by profiles/r02_ubench_pipes.md" % ("measured" if peaks else "fallback 1965 MHz"),
                         "instr_per_event": ni, "fp_instr_per_event": nf,
                         "refined": {"slots_per_event": rs, "parts": rs_parts, "frac": k1_rate * rs / peak_instr,
-                                    "why": "IMAD.WIDE.U32 occupies the scheduler's one fma-heavy pipe for 4 clk, LOP3/IADD3/SEL the ALU "
-                                           "pipe for 2 (profiles/r02_ubench_pipes.md): the bound is the busiest of issue, fma-heavy, ALU"},
+                                    "why": "a Philox round (2 IMAD.WIDE.U32 + 2 LOP3) costs 9.9 scheduler clocks per warp, and added "
+                                           "instructions cost 1.0-1.9 clk each on top of it (profiles/r02_ubench_pipes.md): each of the "
+                                           "count's Philox multiply+XOR pairs is charged 4.95 clk instead of 2 issue slots"},
                         "fp_pipe_frac": k1_rate * nf / (SM_COUNT * (FP64_LANES if precision == 64 else ISSUE_LANES) * sm_max * 1e6),
                         "kernel_events_per_s": k1_rate, "kernel_ms_per_launch": k1_s * 1e3, "kernel_launches": int(k1_launches),
                         "kernel_includes": "the whole iteration: event loop + reduce + finalize + refine run in the one launch",
@@ -407,13 +414,19 @@ def main():
     # the other workloads SURVEY.md 8(d) gates (>= 1e8 events per iteration): a few steps each, own clock window
     extra = []
     if world == 1 and not args.no_extra and args.workload == "cfg3" and args.precision == 64 and not args.n_events:
-        for cfg, prec, n_ev in ((3, 32, 0), (5, 64, 0), (4, 64, 100_000_000)):
+        # ... and the two opt-in variants of the sampling map on the headline workload: what the
+        # 32-bit draw saves against 53-bit uniforms, what an fp32-rounded grid table costs
+        for cfg, prec, n_ev, variant in ((3, 32, 0, 0), (5, 64, 0, 0), (4, 64, 100_000_000, 0), (3, 64, 0, 1), (3, 64, 0, 2)):
             we = W.config(cfg)
             if n_ev:
                 we = we.scaled(n_ev)
-            r = measure(we, prec, max(3, min(args.steps, 10)), max(args.warmup, 4), "%s/%d" % (we.name, prec))
+            vname = {0: "", 1: "/u53", 2: "/q32"}[variant]
+            r = measure(we, prec, max(3, min(args.steps, 10)), max(args.warmup, 4), "%s/%d%s" % (we.name, prec, vname), variant=variant)
             if r:
-                extra.append({"workload": r["workload"], "dtype": r["dtype"], "n_events": we.n_events, "chunk_events": we.chunk_events,
+                extra.append({"workload": r["workload"], "dtype": r["dtype"],
+                              "variant": {0: "none", 1: "u53 (53-bit uniforms, two Philox words per draw)",
+                                          2: "q32 (grid-table entries rounded to fp32)"}[variant],
+                              "n_events": we.n_events, "chunk_events": we.chunk_events,
                               "value": r["value"], "e2e": r["e2e"]["value"], "ms_per_step": r["ms_per_step"], "steps": r["steps"],
                               "kernel_ms_per_launch": r["roofline"]["kernel_ms_per_launch"],
                               "kernel_events_per_s": r["roofline"]["kernel_events_per_s"],

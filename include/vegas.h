@@ -268,15 +268,6 @@ int vegas_get_launch(vegas_grid* g, int integrand_id, int precision, int* path, 
 int vegas_set_variant(vegas_grid* g, int variant);
 int vegas_get_variant(const vegas_grid* g);
 
-/* Instrumentation for bench.py: with profiling on, every fused-kernel launch is bracketed by CUDA
- * events on its stream; vegas_kernel_time_ms() synchronises those events and returns their summed
- * duration and the number of launches since the last vegas_reset_counters().  vegas_launch_count()
- * counts ALL kernels of this library launched for the grid (no synchronisation). */
-int vegas_set_profiling(vegas_grid* g, int on);
-int vegas_kernel_time_ms(vegas_grid* g, double* iterate_kernel_ms, uint64_t* iterate_launches);
-uint64_t vegas_launch_count(const vegas_grid* g);
-int vegas_reset_counters(vegas_grid* g);
-
 const char* vegas_strerror(int code);
 /* Text of the last CUDA error seen by a call on this grid ("" if none); valid until the next call. */
 const char* vegas_last_cuda_error(const vegas_grid* g);

@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "../../include/vegas.h"
+#include "../../include/vegas_instrument.h"
 #include "vegas_kernels.h"
 #include "vegas_iterate_rot.cuh"
 #include "vegas_user.h"

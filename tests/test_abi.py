@@ -1,4 +1,4 @@
-"""The C-ABI shared library loads without a GPU and exports every symbol include/vegas.h declares;
+"""The C-ABI shared library loads without a GPU and exports every symbol include/*.h declares;
 host-only entry points behave; compute entry points fail loudly without a device (no CPU fallback)."""
 import ctypes as C
 import os
@@ -19,7 +19,7 @@ def B():
 
 
 def _declared_symbols():
-    text = open(os.path.join(ROOT, "include", "vegas.h")).read()
+    text = "".join(open(os.path.join(ROOT, "include", h)).read() for h in sorted(os.listdir(os.path.join(ROOT, "include"))) if h.endswith(".h"))
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(vegas_[a-z_0-9]+)\s*\(", text)))
 

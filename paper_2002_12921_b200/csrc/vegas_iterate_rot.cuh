@@ -798,7 +798,7 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     for (int idx = threadIdx.x; idx < NG * rows * 32; idx += blockDim.x) reinterpret_cast<double*>(hist)[idx] = 0.0;
     if (FID == VEGAS_F_USER && threadIdx.x < kRotMaxObsBins) obs_sh[threadIdx.x] = 0.0;
     if (MBAR && S > 1 && threadIdx.x < NSEC * (blockDim.x >> 5)) {
-        token_init(tok_base + 8u * threadIdx.x);
+        token_init(tok_base + 8u * (kRotScratchWarps * (threadIdx.x / (blockDim.x >> 5)) + threadIdx.x % (blockDim.x >> 5)));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -825,10 +825,17 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     const T fin0 = (T)a.fin0, fin1 = (T)a.fin1;
     RotCtx<FID, T, NBLK> ctx;
     ctx.init(a, DIM, L.gamma4, L.gammaL);
-    const uint32_t tok_stride = 8u * (blockDim.x >> 5);
+    constexpr uint32_t tok_stride = 8u * kRotScratchWarps;      // tokens [section][warp slot]: the section is an address immediate
     const int next_warp = grp * S + ((pos + 1 == S) ? 0 : pos + 1);
-    const uint32_t my_tok = MBAR ? tok_base + 8u * warp : 1u + (uint32_t)warp;              // mbarrier address / barrier id
-    const uint32_t next_tok = MBAR ? tok_base + 8u * next_warp : 1u + (uint32_t)next_warp;
+    uint32_t my_tok = MBAR ? tok_base + 8u * warp : 1u + (uint32_t)warp;              // mbarrier address / barrier id
+    uint32_t next_tok = MBAR ? tok_base + 8u * next_warp : 1u + (uint32_t)next_warp;
+    // fp64 with mbarrier tokens: kept in two registers; left to itself ptxas rebuilds both addresses from %tid and the
+    // shared-memory base at every wait and every hand-off (cfg3 4.16e10 -> 4.33e10 events/s; the named-barrier kernels
+    // and the fp32 ones, where ptxas keeps them anyway, lose 1..7 % with the same line: profiles/r02_k1_steps.md)
+    if (MBAR && sizeof(T) == 8) {
+        asm volatile("" : "+r"(my_tok), "+r"(next_tok));
+        asm volatile("" : "+r"(L.tx4[0]), "+r"(L.tx4[1]), "+r"(L.tx4[2]), "+r"(L.tx4[3]));
+    }
     const bool ring = S > 1, lane0 = lane == 0;
 
     // per-thread sums: plain fp64 inside a chunk (a few hundred terms), folded into double-double at the end of every
@@ -844,6 +851,8 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     const uint32_t chunk = (a.chunk == 0 || a.chunk > a.count) ? count : (uint32_t)a.chunk;
     const uint32_t e_hi = (uint32_t)(a.first_event >> 32), first_lo = (uint32_t)a.first_event;
     const uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x;
+    // (waiting unconditionally, with the ring heads' tokens passed once up front, takes the tests of `ring` and `first`
+    // out of the loop but measured the same in fp64 and 3 % slower in fp32: profiles/r02_k1_steps.md)
     uint32_t tick = (pos == 0) ? 1u : 0u;      // parity of the token waits: pos 0 skips the wait of its first iteration
     bool first = (pos == 0);
     for (uint32_t c0 = 0, c_end = 0; c0 < count; c0 = c_end) {

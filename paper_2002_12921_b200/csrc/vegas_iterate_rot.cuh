@@ -133,9 +133,11 @@ template <typename T, int NCH> struct IntegrandU<VEGAS_F_BW_POLY, T, NCH> {
         u0 = (T)0;
     }
     template <class C> __device__ __forceinline__ void dim(T u, int blk, int i, const C& c) {
-        T h = t_fma(c.coef(blk, i, 3), u, c.coef(blk, i, 2));
-        h = t_fma(h, u, c.coef(blk, i, 1));
-        h = t_fma(h, u, c.coef(blk, i, 0));
+        T a4[4];
+        c.coefs(blk, i, a4);
+        T h = t_fma(a4[3], u, a4[2]);
+        h = t_fma(h, u, a4[1]);
+        h = t_fma(h, u, a4[0]);
         poly[i & (NCH - 1)] = t_fma(h, u, poly[i & (NCH - 1)]);
         if (blk == 0 && c.dim0(i)) u0 = u;
     }
@@ -355,11 +357,15 @@ template <typename T, int NBLK> struct RotCtx<VEGAS_F_BW_POLY, T, NBLK> {
     T a[kRegs ? NBLK : 1][4][4];    // a_j1..a_j4 of the lane's dimension at (blk, i); zero for dimension 0 / no dimension
     bool is0[4];                    // the lane holds dimension 0 at sub-step i of block 0
     T poly0;                        // sum_j a_j0
-    const double* p;                // more than 8 dimensions: the coefficient rows (RotArgs::fpar; row 0 is zero)
+    uint32_t cbase;                 // more than 8 dimensions: shared-window address of the coefficient rows [dim][4]
+                                    // (32 bytes per dimension; the 4 lane groups of a warp read 4 consecutive rows: one
+                                    // conflict-free wavefront per LDS.128; reading them from the constant bank by a
+                                    // lane-dependent index measured 2x slower than the generic kernel's whole event)
+    const double* p;                // the same rows in the kernel arguments (RotArgs::fpar; row 0 is zero): K4's view
     int gamma4, gammaL, nblk;
     template <class A> __device__ __forceinline__ void init(const A& r, int dim, int g4, int gL) {
         nblk = (dim + 3) / 4;
-        gamma4 = g4; gammaL = gL; p = r.fpar;
+        gamma4 = g4; gammaL = gL; p = r.fpar; cbase = 0;
         T c0 = (T)0;
         for (int j = 1; j < dim; ++j) c0 += (T)r.fpar[5 * j];
         poly0 = c0;
@@ -374,9 +380,20 @@ template <typename T, int NBLK> struct RotCtx<VEGAS_F_BW_POLY, T, NBLK> {
                 if (blk == 0) is0[i] = (j == 0);
             }
     }
-    __device__ __forceinline__ T coef(int blk, int i, int k) const {
-        if (kRegs) return a[kRegs ? blk : 0][i][k];
-        return (T)p[5 * (4 * blk + ((blk == nblk - 1 ? gammaL : gamma4) ^ i)) + 1 + k];
+    __device__ __forceinline__ void coefs(int blk, int i, T (&out)[4]) const {
+        if (kRegs) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) out[k] = a[kRegs ? blk : 0][i][k];
+            return;
+        }
+        const int j = 4 * blk + ((blk == nblk - 1 ? gammaL : gamma4) ^ i);
+        if (cbase) {
+            const double2 lo = lds_entry<double2>(cbase + 32u * (uint32_t)j), hi = lds_entry<double2>(cbase + 32u * (uint32_t)j + 16u);
+            out[0] = (T)lo.x; out[1] = (T)lo.y; out[2] = (T)hi.x; out[3] = (T)hi.y;
+        } else {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) out[k] = (T)p[5 * j + 1 + k];
+        }
     }
     __device__ __forceinline__ bool dim0(int i) const { return is0[i]; }
 };
@@ -427,12 +444,15 @@ template <typename T, int NCH> struct IntegrandU<VEGAS_F_USER, T, NCH> {
 #ifndef VEGAS_ROT_BW_WARPS
 #define VEGAS_ROT_BW_WARPS 12
 #endif
+#ifndef VEGAS_ROT_WIDE_WARPS
+#define VEGAS_ROT_WIDE_WARPS 24
+#endif
 #ifndef VEGAS_ROT_WIDE_MIN_DIM
 #define VEGAS_ROT_WIDE_MIN_DIM 13
 #endif
 __host__ __device__ constexpr int rot_max_warps(int fid, int dim) {
     return (fid == VEGAS_F_USER || (fid == VEGAS_F_BW_POLY && dim <= kRotBwMaxDim && VEGAS_ROT_BW_WARPS == 12))
-               ? 12 : (dim >= VEGAS_ROT_WIDE_MIN_DIM ? 24 : 16);
+               ? 12 : (dim >= VEGAS_ROT_WIDE_MIN_DIM ? VEGAS_ROT_WIDE_WARPS : 16);
 }
 __host__ __device__ constexpr int rot_max_threads(int fid, int dim) { return 32 * rot_max_warps(fid, dim); }
 __host__ __device__ constexpr bool rot_mbar_tokens(int fid, int dim) { return rot_max_warps(fid, dim) > 16; }
@@ -763,7 +783,8 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     constexpr int NSEC = rot_sections(FID, DIM);
     constexpr bool MBAR = rot_mbar_tokens(FID, DIM);
     constexpr bool kPairHold = PAIR;
-    const uint32_t tok_base = (uint32_t)__cvta_generic_to_shared(obs_sh + kRotMaxObsBins);   // [NSEC][warps] mbarriers
+    const uint32_t tok_base = (uint32_t)__cvta_generic_to_shared(obs_sh + kRotMaxObsBins);   // [NSEC][warp slots] mbarriers
+    double* bw_coef = obs_sh + kRotMaxObsBins + kRotMaxSections * kRotScratchWarps;          // BW_POLY beyond 8 dims: [DIM][4]
 
     // Programmatic dependent launch between the chunk launches of one accumulate call: the next chunk's CTAs may start
     // (prologue, event loop) on SMs this grid has already left; they wait for this grid to complete before they touch
@@ -797,6 +818,8 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     }
     for (int idx = threadIdx.x; idx < NG * rows * 32; idx += blockDim.x) reinterpret_cast<double*>(hist)[idx] = 0.0;
     if (FID == VEGAS_F_USER && threadIdx.x < kRotMaxObsBins) obs_sh[threadIdx.x] = 0.0;
+    if (FID == VEGAS_F_BW_POLY && DIM > kRotBwMaxDim && threadIdx.x < 4 * DIM)
+        bw_coef[threadIdx.x] = a.fpar[5 * (threadIdx.x >> 2) + 1 + (threadIdx.x & 3)];
     if (MBAR && S > 1 && threadIdx.x < NSEC * (blockDim.x >> 5)) {
         token_init(tok_base + 8u * (kRotScratchWarps * (threadIdx.x / (blockDim.x >> 5)) + threadIdx.x % (blockDim.x >> 5)));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -825,6 +848,7 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
     const T fin0 = (T)a.fin0, fin1 = (T)a.fin1;
     RotCtx<FID, T, NBLK> ctx;
     ctx.init(a, DIM, L.gamma4, L.gammaL);
+    if constexpr (FID == VEGAS_F_BW_POLY && DIM > kRotBwMaxDim) ctx.cbase = (uint32_t)__cvta_generic_to_shared(bw_coef);
     constexpr uint32_t tok_stride = 8u * kRotScratchWarps;      // tokens [section][warp slot]: the section is an address immediate
     const int next_warp = grp * S + ((pos + 1 == S) ? 0 : pos + 1);
     uint32_t my_tok = MBAR ? tok_base + 8u * warp : 1u + (uint32_t)warp;              // mbarrier address / barrier id
@@ -840,6 +864,8 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
 
     // per-thread sums: plain fp64 inside a chunk (a few hundred terms), folded into double-double at the end of every
     // chunk; everything above the thread (warp, CTA, launches, CTAs) is added in double-double too
+    // (keeping them in local memory instead frees 8 registers -- 72, enough for 27 warps -- but 27 warps measured
+    // 4.20e10 events/s on cfg3 against 4.35e10 with 24, and 21 warps 3.84e10: profiles/r02_k1_steps.md)
     dd a1{0.0, 0.0}, a2{0.0, 0.0};
     // every warp runs the same number of loop iterations (the ring hands the tokens on once per iteration);
     // events past the end of a chunk contribute v = 0
@@ -994,7 +1020,8 @@ k_iterate_rot(const __grid_constant__ RotArgs a) {
 inline size_t rot_shared_bytes(int dim, int n_bins, int n_groups) {
     const size_t rows = (size_t)((dim + 3) / 4) * n_bins;
     return rows * (128 + 256 * (size_t)n_groups) + 2 * sizeof(dd) * kRotScratchWarps +
-           sizeof(double) * kRotMaxObsBins + 8 * (size_t)kRotMaxSections * kRotScratchWarps;
+           sizeof(double) * kRotMaxObsBins + 8 * (size_t)kRotMaxSections * kRotScratchWarps +
+           sizeof(double) * 4 * VEGAS_MAX_DIM;
 }
 
 // one translation unit per (FID, T, VAR) instantiates DIM = 1..32 (vegas_rot_inst.cu)

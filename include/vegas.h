@@ -74,6 +74,11 @@ extern "C" {
 /*   VEGAS_F_USER               an integrand supplied as CUDA source and compiled at run time for this grid:
  *                              see vegas_set_user_integrand() below; fp64 only, n_params <= VEGAS_USER_MAX_PARAMS */
 #define VEGAS_F_USER 4
+/*   VEGAS_F_GENZ_DISCONTINUOUS PAPER.md:67-70 Eq.(2) as printed, N = 1 (reading R19): f = 0 where any
+ *                              x_j <= a_j, exp(sum_j c_j x_j) elsewhere.  params = { c[0..d-1], a[0..d-1] }, c_j > 0.
+ *                              fp64 only: an event within rounding of a cut would be kept or dropped in a different
+ *                              precision than the fp64 oracle decides it in (VEGAS_EINVAL for precision 32). */
+#define VEGAS_F_GENZ_DISCONTINUOUS 5
 #define VEGAS_USER_MAX_PARAMS 64
 
 /* precision of the per-event arithmetic (reading C11): 64 = everything fp64; 32 = grid table, r, x,

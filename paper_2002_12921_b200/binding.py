@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libvegas_b200.so")
 
 VEGAS_OK, VEGAS_EINVAL, VEGAS_ECUDA, VEGAS_ENUMERIC = 0, -1, -2, -3
 VEGAS_F_CONST, VEGAS_F_GAUSS, VEGAS_F_GENZ_PRODUCT_PEAK, VEGAS_F_BW_POLY, VEGAS_F_USER = 0, 1, 2, 3, 4
+VEGAS_F_GENZ_DISCONTINUOUS = 5
 VEGAS_USER_MAX_PARAMS = 64
 VEGAS_FP64, VEGAS_FP32 = 64, 32
 VEGAS_VARIANT_NONE, VEGAS_VARIANT_U53, VEGAS_VARIANT_Q32 = 0, 1, 2

@@ -55,6 +55,7 @@ int expected_n_params(int fid, int dim) {
     case VEGAS_F_CONST: return 0;
     case VEGAS_F_GAUSS: return 1;
     case VEGAS_F_GENZ_PRODUCT_PEAK: return 2 * dim;
+    case VEGAS_F_GENZ_DISCONTINUOUS: return 2 * dim;
     case VEGAS_F_BW_POLY: return dim >= 2 ? 4 + 5 * (dim - 1) : -1;
     default: return -1;
     }
@@ -78,9 +79,9 @@ struct vegas_grid {
     double* d_obs = nullptr;                     // observable histogram of a user integrand: sums of v per bin
     int n_obs = 0;
     double obs_lo = 0.0, obs_hi = 1.0;
-    bool params_set[5] = {true, false, false, false, false};
-    double derived[5][VEGAS_MAX_PARAMS] = {};
-    double user[5][VEGAS_MAX_PARAMS] = {};       // the caller's arrays as given to vegas_set_params
+    bool params_set[6] = {true, false, false, false, false, false};
+    double derived[6][VEGAS_MAX_PARAMS] = {};
+    double user[6][VEGAS_MAX_PARAMS] = {};       // the caller's arrays as given to vegas_set_params
     vegas::UserKernel ukernel;                   // VEGAS_F_USER: the run-time compiled fused kernel
     int cfg_blocks = 0, cfg_threads = 0, cfg_ct = 0, cfg_ch = 0;
     int variant = 0;                // VEGAS_VARIANT_*: the sampling map of the iterate calls (vegas_set_variant)
@@ -163,15 +164,16 @@ int ilog2(int v) {
 bool use_rot_path(const vegas_grid* g, int fid, int precision);
 // the variants of the sampling map exist as fp64 fast-path kernels of the built-in integrands
 bool variant_available(const vegas_grid* g, int fid, int precision) {
-    return precision == VEGAS_FP64 && fid != VEGAS_F_USER && use_rot_path(g, fid, precision);
+    return precision == VEGAS_FP64 && fid != VEGAS_F_USER && fid != VEGAS_F_GENZ_DISCONTINUOUS && use_rot_path(g, fid, precision);
 }
 
 bool check_call(const vegas_grid* g, int fid, int precision) {
     if (!g) return false;
-    if (fid < 0 || fid > VEGAS_F_USER || !g->params_set[fid]) return false;
+    if (fid < 0 || fid > VEGAS_F_GENZ_DISCONTINUOUS || !g->params_set[fid]) return false;
     if (fid == VEGAS_F_USER) return g->ukernel.kernel != nullptr && precision == VEGAS_FP64 && g->variant == 0;
     if (expected_n_params(fid, g->dim) < 0) return false;
     if (g->variant != 0 && !variant_available(g, fid, precision)) return false;
+    if (fid == VEGAS_F_GENZ_DISCONTINUOUS) return precision == VEGAS_FP64;      // the cuts are decided in fp64 (vegas.h)
     return precision == VEGAS_FP64 || precision == VEGAS_FP32;
 }
 
@@ -190,7 +192,7 @@ bool use_rot_path(const vegas_grid* g, int fid, int precision) {
     if (g->cfg_ct > 0 || g->cfg_ch > 0) return false;
     (void)precision;
     const bool kind = fid == VEGAS_F_CONST || fid == VEGAS_F_GAUSS || fid == VEGAS_F_GENZ_PRODUCT_PEAK ||
-                      fid == VEGAS_F_BW_POLY;
+                      fid == VEGAS_F_BW_POLY || fid == VEGAS_F_GENZ_DISCONTINUOUS;
     if (!kind) return false;
     return vegas::rot_shared_bytes(g->dim, g->n_bins, 1) <= g->smem_optin;
 }
@@ -234,6 +236,17 @@ void rot_constants(const vegas_grid* g, int fid, int precision, double* shift, d
             *fin1 = (double)q32;
             *post_scale = pc * std::exp((double)dim * std::log(nb) - 4.0 * std::log((double)q32));
         }
+    } else if (fid == VEGAS_F_GENZ_DISCONTINUOUS) {
+        double ps = 1.0, k = 0.0;                                // u_j = c_j (x_j - a_j): J = prod (nb / c_j) B_j 2^32
+        for (int j = 0; j < dim; ++j) {
+            const double c = g->user[fid][j], a = g->user[fid][dim + j];
+            shift[j] = a;
+            scale[j] = c;
+            ps *= nb / c;
+            k += c * a;
+        }
+        *post_scale = ps;
+        *fin1 = k;                                               // exp(sum c_j x_j) = exp(sum u_j + sum c_j a_j)
     } else if (fid == VEGAS_F_USER) {
         double ps = 1.0;                                         // u_j = x_j; J = prod nb Delta_j = nb^d prod B_j 2^32
         for (int j = 0; j < dim; ++j) { scale[j] = 1.0; ps *= nb; }
@@ -358,6 +371,8 @@ cudaError_t launch_rot(vegas_grid* g, int fid, int precision, int dim, const veg
             return vegas::launch_iterate_rot<VEGAS_F_GENZ_PRODUCT_PEAK, double>(dim, a, s.blocks, s.threads, s.shmem, st);
         case VEGAS_F_BW_POLY:
             return vegas::launch_iterate_rot<VEGAS_F_BW_POLY, double>(dim, a, s.blocks, s.threads, s.shmem, st);
+        case VEGAS_F_GENZ_DISCONTINUOUS:
+            return vegas::launch_iterate_rot<VEGAS_F_GENZ_DISCONTINUOUS, double>(dim, a, s.blocks, s.threads, s.shmem, st);
         }
     } else {
         switch (fid) {
@@ -461,7 +476,7 @@ int vegas_set_params(vegas_grid* g, int fid, const double* p, int n_params) {
         g->params_set[fid] = true;
         return VEGAS_OK;
     }
-    if (!g || fid < 0 || fid > 3) return VEGAS_EINVAL;
+    if (!g || fid < 0 || (fid > 3 && fid != VEGAS_F_GENZ_DISCONTINUOUS)) return VEGAS_EINVAL;
     const int want = expected_n_params(fid, g->dim);
     if (want < 0 || n_params != want || want > VEGAS_MAX_PARAMS || (want > 0 && !p)) return VEGAS_EINVAL;
     for (int i = 0; i < want; ++i)
@@ -483,6 +498,10 @@ int vegas_set_params(vegas_grid* g, int fid, const double* p, int n_params) {
             d[2 * j] = 1.0 / (p[j] * p[j]);
             d[2 * j + 1] = p[dim + j];
         }
+        break;
+    case VEGAS_F_GENZ_DISCONTINUOUS:
+        for (int j = 0; j < dim; ++j)
+            if (!(p[j] > 0.0)) return VEGAS_EINVAL;                      // c_j > 0: the cut is u_j <= 0 on the fast path
         break;
     case VEGAS_F_BW_POLY: {
         const double M = p[0], G = p[1], m_min = p[2], m_max = p[3];
@@ -1005,7 +1024,7 @@ int vegas_get_variant(const vegas_grid* g) { return g ? g->variant : VEGAS_EINVA
 
 int vegas_get_launch(vegas_grid* g, int integrand_id, int precision, int* path, int* blocks, int* threads,
                      int* table_copies, int* hist_copies, size_t* shared_bytes) {
-    if (!g || (precision != VEGAS_FP64 && precision != VEGAS_FP32) || integrand_id < 0 || integrand_id > VEGAS_F_USER)
+    if (!g || (precision != VEGAS_FP64 && precision != VEGAS_FP32) || integrand_id < 0 || integrand_id > VEGAS_F_GENZ_DISCONTINUOUS)
         return VEGAS_EINVAL;
     if (use_rot_path(g, integrand_id, precision)) {
         const RotShape r = rot_shape(g, integrand_id);

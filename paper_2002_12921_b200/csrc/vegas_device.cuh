@@ -13,6 +13,9 @@ typedef unsigned long size_t;
 #define VEGAS_F_CONST 0
 #define VEGAS_F_GAUSS 1
 #define VEGAS_F_GENZ_PRODUCT_PEAK 2
+#ifndef VEGAS_F_GENZ_DISCONTINUOUS
+#define VEGAS_F_GENZ_DISCONTINUOUS 5
+#endif
 #define VEGAS_F_BW_POLY 3
 #define VEGAS_F_USER 4
 #else
@@ -172,6 +175,13 @@ struct Integrand<VEGAS_F_GENZ_PRODUCT_PEAK, T> {   // PAPER.md:74 Eq.(3), N = 1
         prod *= t_fma(t, t, fp.p[2 * j]);
     }
     __device__ __forceinline__ T finish(const FParams<T>&) const { return (T)1 / prod; }
+};
+
+template <typename T>
+struct Integrand<VEGAS_F_GENZ_DISCONTINUOUS, T> {   // served through the affine variable (IntegrandU) by both kernels
+    __device__ __forceinline__ void begin() {}
+    __device__ __forceinline__ void dim(int, T, const FParams<T>&) {}
+    __device__ __forceinline__ T finish(const FParams<T>&) const { return (T)0; }
 };
 
 template <typename T>

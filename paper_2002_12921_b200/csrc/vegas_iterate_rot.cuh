@@ -117,6 +117,25 @@ template <typename T, int NCH> struct IntegrandU<VEGAS_F_GENZ_PRODUCT_PEAK, T, N
         return finish(fin0, fin1) * chain_prod<NCH, T>(jac);
     }
 };
+// Genz discontinuous, Eq.(2) as printed (reading R19): u_j = c_j (x_j - a_j), c_j > 0, so that the cut
+// x_j <= a_j is u_j <= 0 and sum_j c_j x_j = sum_j u_j + sum_j c_j a_j (fin1).  fp64 only (include/vegas.h).
+template <typename T, int NCH> struct IntegrandU<VEGAS_F_GENZ_DISCONTINUOUS, T, NCH> {
+    T s[NCH];
+    bool cut;
+    template <class C> __device__ __forceinline__ void begin(const C&) {
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) s[c] = (T)0;
+        cut = false;
+    }
+    template <class C> __device__ __forceinline__ void dim(T u, int, int i, const C&) {
+        s[i & (NCH - 1)] += u;
+        cut = cut || !(u > (T)0);
+    }
+    __device__ __forceinline__ T finish(T, T fin1) const {
+        return cut ? (T)0 : ExpFast<T, (NCH > 1)>::f(chain_sum<NCH, T>(s) + fin1);
+    }
+    __device__ __forceinline__ T value(const T (&jac)[NCH], T fin0, T fin1) const { return finish(fin0, fin1) * chain_prod<NCH, T>(jac); }
+};
 // BW_POLY (BASELINE.json:configs[4], readings R11, R12): u_0 = (s(x_0) - M^2)/(M Gamma), u_j = x_j for j >= 1;
 // f = [1/(1 + u_0^2)] * [sum_j a_j0 + sum_j u_j (a_j1 + u_j (a_j2 + u_j (a_j3 + u_j a_j4)))].
 // The lane that holds dimension 0 at sub-step i of block 0 runs the quartic with zero coefficients and keeps u.

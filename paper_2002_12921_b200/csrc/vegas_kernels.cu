@@ -431,6 +431,8 @@ static cudaError_t launch_iterate_fid(int fid, const IterArgs& a, const FParams<
     case VEGAS_F_GENZ_PRODUCT_PEAK:
         return launch_iterate_nblk<VEGAS_F_GENZ_PRODUCT_PEAK, T>(a, fp, blocks, threads, shmem, st);
     case VEGAS_F_BW_POLY: return launch_iterate_nblk<VEGAS_F_BW_POLY, T>(a, fp, blocks, threads, shmem, st);
+    case VEGAS_F_GENZ_DISCONTINUOUS:
+        return launch_iterate_nblk<VEGAS_F_GENZ_DISCONTINUOUS, T>(a, fp, blocks, threads, shmem, st);
     default: return cudaErrorInvalidValue;
     }
 }
@@ -498,6 +500,7 @@ static cudaError_t launch_debug_rot_t(int fid, const DebugArgs& a, cudaStream_t 
     case VEGAS_F_GAUSS: k_debug_rot<VEGAS_F_GAUSS, T><<<blocks, threads, 0, st>>>(a); break;
     case VEGAS_F_GENZ_PRODUCT_PEAK: k_debug_rot<VEGAS_F_GENZ_PRODUCT_PEAK, T><<<blocks, threads, 0, st>>>(a); break;
     case VEGAS_F_BW_POLY: k_debug_rot<VEGAS_F_BW_POLY, T><<<blocks, threads, 0, st>>>(a); break;
+    case VEGAS_F_GENZ_DISCONTINUOUS: k_debug_rot<VEGAS_F_GENZ_DISCONTINUOUS, T><<<blocks, threads, 0, st>>>(a); break;
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();

@@ -655,3 +655,54 @@ def test_more_than_2_to_the_32_events_in_one_iteration(B):
     np.testing.assert_allclose(H2, H, rtol=1e-11)
     np.testing.assert_allclose(H.sum(axis=1), np.full(w.dim, H[0].sum()), rtol=1e-11)   # every dimension sums to S2
     g.close()
+
+
+@pytest.mark.parametrize("path", ["auto", "generic"])
+@pytest.mark.parametrize("dim,nb,pseed", [(16, 50, 9), (2, 8, 2), (7, 33, 5), (20, 50, 11)])
+def test_genz_discontinuous_built_in(B, dim, nb, pseed, path):
+    """PAPER.md:67-70 Eq.(2) as printed (reading R19), at the paper's 16 dimensions and odd shapes, as a
+    built-in fast-path integrand (VEGAS_F_GENZ_DISCONTINUOUS; the oracle's id for it is 4): events, teacher-forced
+    iterations and refinement against the oracle; fp64 only."""
+    fid = B.VEGAS_F_GENZ_DISCONTINUOUS
+    p = W.genz_discontinuous_params(dim, pseed)
+    n, n_iter = 200_003, 3
+    ch = O.integrate(dim, nb, n_iter, n, pseed, 1.5, O.GENZ_DISCONTINUOUS, p, threads=THREADS)
+    g = B.VegasGrid(dim, nb)
+    g.set_params(fid, p)
+    if path == "generic":
+        g.set_launch(0, 0, 2, 4)
+    assert g.get_launch(fid, 64)["path"] == ("generic" if path == "generic" else "rotated")
+    for k in range(n_iter):
+        g.set_edges(ch["edges_trace"][k])
+        if k == 1:
+            gw, gb, gx, gf = g.debug_sample(7, 20_000, pseed, k, fid, 64)
+            ow, ob, ox, of = O.sample(ch["edges_trace"][k], pseed, k, 7, 20_000, O.GENZ_DISCONTINUOUS, p)
+            assert np.array_equal(gw, ow) and np.array_equal(gb, ob)
+            assert np.array_equal(gf == 0, of == 0)                 # the same events fall on the zero side of a cut
+            np.testing.assert_allclose(gf, of, rtol=1e-12, atol=0)
+        I, s, H, st = g.iterate(n, pseed, k, fid, 64)
+        assert st == 0
+        assert I == pytest.approx(ch["per_iter"][k, 0], rel=RTOL64)
+        assert s == pytest.approx(ch["per_iter"][k, 1], rel=RTOL64)
+        _assert_hist(H, ch["hist_trace"][k], 64)
+        assert g.refine(1.5) == 0
+        want = ch["edges_trace"][k + 1] if k + 1 < n_iter else ch["edges"]
+        np.testing.assert_allclose(g.get_edges(), want, rtol=0, atol=1e-10)
+    # fp32 is refused (the cuts are decided in fp64); so are non-positive c_j
+    with pytest.raises(B.VegasError):
+        g.iterate(1000, 1, 0, fid, 32)
+    bad = np.array(p, dtype=float)
+    bad[0] = -bad[0]
+    with pytest.raises(B.VegasError):
+        g.set_params(fid, bad)
+    g.close()
+
+
+def test_genz_discontinuous_chain_within_5_sigma_at_16_dimensions(B):
+    p = W.genz_discontinuous_params(16, 9)
+    g = B.VegasGrid(16, 50)
+    g.set_params(B.VEGAS_F_GENZ_DISCONTINUOUS, p)
+    r = g.integrate(8, 2_000_000, 9, 1.5, B.VEGAS_F_GENZ_DISCONTINUOUS, 64, n_skip=3)
+    exact = W.closed_form(W.GENZ_DISCONTINUOUS, 16, p)
+    assert r["status"] == 0 and abs(r["I"] - exact) <= 5 * r["sigma"] and r["sigma"] < 0.01 * exact
+    g.close()

@@ -45,12 +45,12 @@ def n_wide(w):
 
 
 # Refined machine model from the round-2 microbenchmarks (profiles/r02_ubench_pipes.md; "refine them
-# only via the step-0 microbenchmarks"): one Philox round of one block -- 2 IMAD.WIDE.U32 + 2 LOP3 -- costs 9.9 scheduler
-# clocks per warp at 6 warps per scheduler (not the 4 its instruction count suggests), and instructions added to the
-# rounds cost 1.0 .. 1.9 clocks each ON TOP (DFMA, LOP3, IMAD alike): nothing hides under the wide multiplies.  The
-# refined bound charges each of the 20 ceil(d/4) Philox multiply+XOR pairs of the SURVEY count 4.95 clocks instead of 2
-# and every other instruction its one issue slot.
-PHILOX_PAIR_CLK = 4.95
+# only via the step-0 microbenchmarks"): one Philox round of one block -- 2 IMAD.WIDE.U32 + 2 LOP3 -- costs 8.8 scheduler
+# clocks per warp (9.9 measured with the one register move the benchmark loop carries per round), not the 4 its
+# instruction count suggests, and instructions added to the rounds cost 1.0 .. 1.9 clocks each ON TOP (DFMA, LOP3, IMAD
+# alike): nothing hides under the wide multiplies.  The refined bound charges each of the 20 ceil(d/4) Philox
+# multiply+XOR pairs of the SURVEY count 4.4 clocks instead of 2 and every other instruction its one issue slot.
+PHILOX_PAIR_CLK = 4.4
 
 
 def refined_slots(w, precision):
@@ -383,9 +383,9 @@ def main():
                                        "scheduler per clock confirmed by profiles/r02_ubench_pipes.md" % ("measured" if peaks else "fallback 1965 MHz"),
                         "instr_per_event": ni, "fp_instr_per_event": nf,
                         "refined": {"slots_per_event": rs, "parts": rs_parts, "frac": k1_rate * rs / peak_instr,
-                                    "why": "a Philox round (2 IMAD.WIDE.U32 + 2 LOP3) costs 9.9 scheduler clocks per warp, and added "
+                                    "why": "a Philox round (2 IMAD.WIDE.U32 + 2 LOP3) costs 8.8 scheduler clocks per warp, and added "
                                            "instructions cost 1.0-1.9 clk each on top of it (profiles/r02_ubench_pipes.md): each of the "
-                                           "count's Philox multiply+XOR pairs is charged 4.95 clk instead of 2 issue slots"},
+                                           "count's Philox multiply+XOR pairs is charged 4.4 clk instead of 2 issue slots"},
                         "fp_pipe_frac": k1_rate * nf / (SM_COUNT * (FP64_LANES if precision == 64 else ISSUE_LANES) * sm_max * 1e6),
                         "kernel_events_per_s": k1_rate, "kernel_ms_per_launch": k1_s * 1e3, "kernel_launches": int(k1_launches),
                         "kernel_includes": "the whole iteration: event loop + reduce + finalize + refine run in the one launch",

@@ -229,6 +229,30 @@ __global__ void k_ring(Stamp* out, int work, double a) {
     BENCH_EPILOG(__double2loint(x))
 }
 
+// the same ring with one mbarrier (arrival count 1) per warp: the waiting warp spins on try_wait.parity, the
+// signalling warp's lane 0 arrives (K1's tokens for CTAs of more than 15 warps)
+__global__ void k_ring_mbar(Stamp* out, int work, double a) {
+    __shared__ __align__(8) unsigned long long bars[32];
+    const int warp = threadIdx.x >> 5, W = blockDim.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t base = (uint32_t)__cvta_generic_to_shared(bars);
+    if (threadIdx.x < W) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(base + 8u * threadIdx.x) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    double x = threadIdx.x;
+    BENCH_PROLOG
+    uint32_t tick = (warp == 0) ? 1u : 0u;
+    for (int i = 0; i < SM_ITER; ++i, ++tick) {
+        if (!(warp == 0 && i == 0))
+            asm volatile("{\n.reg .pred p;\nW_%=:\nmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@!p bra W_%=;\n}"
+                         ::"r"(base + 8u * warp), "r"(tick & 1u) : "memory");
+        for (int k = 0; k < work; ++k) x = fma(x, a, 1.0);
+        __syncwarp();
+        if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(base + 8u * ((warp + 1) % W)) : "memory");
+    }
+    BENCH_EPILOG(__double2loint(x))
+}
+
 static Stamp* d_out;
 static int n_sm;
 static void philox_section();
@@ -404,6 +428,19 @@ int main(int argc, char** argv) {
             char nm[128];
             k_ring<<<n_sm, W * 32>>>(d_out, work, 1.0000001);
             snprintf(nm, sizeof nm, "ring of %d warps, %d dependent DFMA inside", W, work);
+            Stamp h[1024];
+            CHECK(cudaDeviceSynchronize());
+            CHECK(cudaMemcpy(h, d_out, sizeof(Stamp) * n_sm, cudaMemcpyDeviceToHost));
+            double cyc = 0; for (int i = 0; i < n_sm; ++i) cyc += (double)h[i].cycles; cyc /= n_sm;
+            printf("%-58s %7.1f clk per hand-off\n", nm, cyc / ((double)SM_ITER * W));
+        }
+    }
+    printf("# mbarrier token ring (try_wait.parity spin / arrive by one lane)\n");
+    for (int W : {2, 4, 8, 24}) {
+        for (int work : {0, 32}) {
+            char nm[128];
+            k_ring_mbar<<<n_sm, W * 32>>>(d_out, work, 1.0000001);
+            snprintf(nm, sizeof nm, "mbarrier ring of %d warps, %d dependent DFMA inside", W, work);
             Stamp h[1024];
             CHECK(cudaDeviceSynchronize());
             CHECK(cudaMemcpy(h, d_out, sizeof(Stamp) * n_sm, cudaMemcpyDeviceToHost));

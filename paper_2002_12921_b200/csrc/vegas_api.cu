@@ -84,6 +84,8 @@ struct vegas_grid {
     double user[6][VEGAS_MAX_PARAMS] = {};       // the caller's arrays as given to vegas_set_params
     vegas::UserKernel ukernel;                   // VEGAS_F_USER: the run-time compiled fused kernel
     int cfg_blocks = 0, cfg_threads = 0, cfg_ct = 0, cfg_ch = 0;
+    double* h_pinned = nullptr;     // page-locked HOST staging for the per-iteration results of vegas_integrate (a copy to
+                                    // pageable memory costs ~10 us more per call); host memory, owned by the library
     int variant = 0;                // VEGAS_VARIANT_*: the sampling map of the iterate calls (vegas_set_variant)
     int active_blocks = 0;          // CTAs whose partial slots the current iteration uses
     bool profiling = false;
@@ -460,6 +462,7 @@ int vegas_create(int dim, int n_bins, void* dev_workspace, size_t bytes, vegas_g
 int vegas_destroy(vegas_grid* g) {
     if (!g) return VEGAS_EINVAL;
     for (cudaEvent_t ev : g->events) cudaEventDestroy(ev);
+    if (g->h_pinned) cudaFreeHost(g->h_pinned);
     vegas::user_unload(&g->ukernel);
     delete g;
     return VEGAS_OK;
@@ -881,11 +884,13 @@ int vegas_integrate_from(vegas_grid* g, uint32_t first_iteration, int n_iter, in
                                          alpha >= 0.0 ? alpha : -1.0, g->d_result + (size_t)kResultStride * k);
         if (rc) return rc;
     }
-    std::vector<double> res((size_t)kResultStride * n_iter);
-    int status = 0;
-    CUDA_TRY(g, cudaMemcpyAsync(res.data(), g->d_result, sizeof(double) * res.size(), cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(g, cudaMemcpyAsync(&status, g->d_status, sizeof(int), cudaMemcpyDeviceToHost, st));
+    if (!g->h_pinned) CUDA_TRY(g, cudaHostAlloc((void**)&g->h_pinned, sizeof(double) * ((size_t)kResultStride * kMaxIter + 1), cudaHostAllocDefault));
+    double* res = g->h_pinned;
+    int* status_p = reinterpret_cast<int*>(g->h_pinned + (size_t)kResultStride * kMaxIter);
+    CUDA_TRY(g, cudaMemcpyAsync(res, g->d_result, sizeof(double) * (size_t)kResultStride * n_iter, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(g, cudaMemcpyAsync(status_p, g->d_status, sizeof(int), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(g, cudaStreamSynchronize(st));
+    const int status = *status_p;
     std::vector<double> Ik(n_iter), sk(n_iter);
     int rc = status == 0 ? VEGAS_OK : VEGAS_ENUMERIC;
     for (int k = 0; k < n_iter; ++k) {

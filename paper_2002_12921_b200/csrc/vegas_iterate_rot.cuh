@@ -314,13 +314,15 @@ __device__ __forceinline__ void sts_f64(uint32_t addr, double v) {
 // Token passing between the warps that share a histogram copy: one mbarrier (arrival count 1) per warp and section
 // in shared memory.  The holder's predecessor arrives (release), the waiting warp spins on try_wait (acquire; the
 // hardware suspends the warp for a bounded time per attempt, so a waiting warp takes no issue slots to speak of).
-// Measured on B200 (profiles/r02_ubench_tokens.md): 78 clk per hand-off against 42 for bar.sync/bar.arrive, but the
-// 16 named barriers of a CTA cap a ring scheme at 15 warps, and more warps are worth more than the 36 clk.
+// Measured on B200 (profiles/r02_ubench_pipes.md, token rings): 113..124 clk per hand-off against 42 for
+// bar.sync/bar.arrive, but the 16 named barriers of a CTA cap a ring scheme at 15 warps, and more warps are worth more
+// than the 70 clk (cfg3: 24 warps 4.35e10 events/s, 21 warps 3.84e10; the ring itself is not what cfg3 waits for:
+// with a private copy per warp and no tokens at all it runs 4.31e10).
 __device__ __forceinline__ void token_init(uint32_t bar) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar) : "memory");
 }
 // try_wait returns after ~12 clk on sm_100a whether or not the phase has completed (a suspend-time hint, nanosleep
-// between attempts, or an L2 round trip between attempts all measured the same or slower: profiles/r02_k1_steps.md),
+// between attempts, or an L2 round trip between attempts all measured the same or slower, round-2 experiments),
 // so this is a spin; a waiting warp issues ~3 instructions per 12 clk.
 __device__ __forceinline__ void token_wait(uint32_t bar, uint32_t parity) {
     asm volatile(

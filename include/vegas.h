@@ -150,9 +150,11 @@ int vegas_get_observable_hist(vegas_grid* g, double* obs_hist_host, void* cuda_s
  * x [n][dim] (row-major fp64) to the host, calls fn(x, n, dim, f, user) -- which must fill f[0..n-1] -- copies f back
  * and accumulates S1, S2 and the histogram on the device (S5-S6).  Same sample, same sums as a device integrand with
  * the same f; fp64; this is a convenience path bound by the host function and the PCIe copies, not the hot path.
- * dev_scratch: device memory, 256-byte aligned, at least vegas_callback_scratch_bytes(dim, batch_events) bytes
- * (caller-owned; about batch_events * (20 dim + 16) bytes).  The callback runs on the calling thread, between stream
- * synchronisations; it must not call into this grid.
+ * dev_scratch: device memory, 256-byte aligned, caller-owned.  vegas_callback_scratch_bytes(dim, batch_events) bytes
+ * (about batch_events * (40 dim + 32)) hold TWO batches: the device samples batch k+1 and copies its points to the host
+ * while the host evaluates batch k (one stream; the host waits on events, not on the stream); with half of that the
+ * batches are processed strictly one after the other.  The callback runs on the calling thread; it must not call
+ * into this grid.  Host staging is page-locked memory owned by the library (2 x batch_events x (dim + 1) doubles).
  * Errors: VEGAS_EINVAL (NULL fn / scratch, n_events < 2, batch_events = 0, scratch too small or misaligned),
  * VEGAS_ECUDA, VEGAS_ENUMERIC (a non-finite f makes the sums non-finite; I, sigma are still written). */
 typedef void (*vegas_host_integrand)(const double* x, uint64_t n, int dim, double* f, void* user);

@@ -224,12 +224,15 @@ class VegasGrid:
                                precision, _stream(stream), C.byref(I), C.byref(s), _ptr(h))
         return I.value, s.value, h, self._check(rc, allow_numeric=True)
 
-    def iterate_callback(self, fn, n_events, seed, iteration, batch_events=1 << 18, want_hist=True, stream=None):
+    def iterate_callback(self, fn, n_events, seed, iteration, batch_events=1 << 18, want_hist=True, stream=None,
+                         overlap=True):
         """One iteration with a HOST integrand: fn(x) takes a float64 array [n, dim] and returns n values.
+        overlap: scratch for two batches (the device samples batch k+1 while fn evaluates batch k); False hands the
+        library half of it, which processes the batches strictly one after the other.
         -> (I, sigma, hist or None, status)"""
         import torch
         n_batch = int(min(batch_events, n_events))
-        nbytes = lib.vegas_callback_scratch_bytes(self.dim, n_batch)
+        nbytes = lib.vegas_callback_scratch_bytes(self.dim, n_batch) // (1 if overlap else 2)
         scratch = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
         ptr = (scratch.data_ptr() + 255) // 256 * 256
         dim = self.dim

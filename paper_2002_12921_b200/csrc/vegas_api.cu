@@ -84,6 +84,9 @@ struct vegas_grid {
     double user[6][VEGAS_MAX_PARAMS] = {};       // the caller's arrays as given to vegas_set_params
     vegas::UserKernel ukernel;                   // VEGAS_F_USER: the run-time compiled fused kernel
     int cfg_blocks = 0, cfg_threads = 0, cfg_ct = 0, cfg_ch = 0;
+    double* h_cb = nullptr;         // page-locked HOST staging of the host-callback path (x and f of two batches)
+    size_t h_cb_doubles = 0;
+    cudaEvent_t cb_ev[4] = {nullptr, nullptr, nullptr, nullptr};     // its "x arrived" / "f consumed" events, per slot
     double* h_pinned = nullptr;     // page-locked HOST staging for the per-iteration results of vegas_integrate (a copy to
                                     // pageable memory costs ~10 us more per call); host memory, owned by the library
     int variant = 0;                // VEGAS_VARIANT_*: the sampling map of the iterate calls (vegas_set_variant)
@@ -463,6 +466,9 @@ int vegas_destroy(vegas_grid* g) {
     if (!g) return VEGAS_EINVAL;
     for (cudaEvent_t ev : g->events) cudaEventDestroy(ev);
     if (g->h_pinned) cudaFreeHost(g->h_pinned);
+    if (g->h_cb) cudaFreeHost(g->h_cb);
+    for (cudaEvent_t ev : g->cb_ev)
+        if (ev) cudaEventDestroy(ev);
     vegas::user_unload(&g->ukernel);
     delete g;
     return VEGAS_OK;
@@ -947,9 +953,14 @@ int vegas_debug_sample(vegas_grid* g, uint64_t first_event, uint32_t count, uint
     return VEGAS_OK;
 }
 
+static size_t callback_slot_bytes(int dim, uint32_t batch_events) {
+    return vegas_debug_scratch_bytes(dim, batch_events) + align_up((size_t)batch_events * 8);
+}
+
+// two slots: the device samples batch k+1 (and copies its points to the host) while the host evaluates batch k
 size_t vegas_callback_scratch_bytes(int dim, uint32_t batch_events) {
     if (dim < 1 || dim > VEGAS_MAX_DIM || batch_events == 0) return 0;
-    return vegas_debug_scratch_bytes(dim, batch_events) + align_up((size_t)batch_events * 8);
+    return 2 * callback_slot_bytes(dim, batch_events);
 }
 
 int vegas_iterate_callback(vegas_grid* g, uint64_t n_events, uint32_t batch_events, uint64_t seed, uint32_t iteration,
@@ -957,42 +968,86 @@ int vegas_iterate_callback(vegas_grid* g, uint64_t n_events, uint32_t batch_even
                            void* cuda_stream, double* I, double* sigma, double* hist_host) {
     if (!g || !fn || !dev_scratch || n_events < 2 || batch_events == 0) return VEGAS_EINVAL;
     if (((uintptr_t)dev_scratch) % kAlign) return VEGAS_EINVAL;
-    if (scratch_bytes < vegas_callback_scratch_bytes(g->dim, batch_events)) return VEGAS_EINVAL;
+    const size_t slot_bytes = callback_slot_bytes(g->dim, batch_events);
+    if (scratch_bytes < slot_bytes) return VEGAS_EINVAL;
+    const int n_slots = scratch_bytes >= 2 * slot_bytes ? 2 : 1;      // one slot: the strictly serial form
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int rc = vegas_begin_iteration(g, cuda_stream);
     if (rc) return rc;
     const int dim = g->dim;
     const size_t per_dim = (size_t)batch_events * dim;
-    unsigned char* base = (unsigned char*)dev_scratch;
-    vegas::DebugArgs a{};
-    a.edges = g->d_edges;
-    a.key0 = (uint32_t)(seed & 0xFFFFFFFFu);
-    a.key1 = (uint32_t)(seed >> 32);
-    a.iteration = iteration;
-    a.dim = dim;
-    a.n_bins = g->n_bins;
-    a.jac_scale = jac_scale_for(g, VEGAS_FP64);
-    a.words = (uint32_t*)base;                 base += align_up(per_dim * 4);
-    a.bins = (int32_t*)base;                   base += align_up(per_dim * 4);
-    a.x = (double*)base;                       base += align_up(per_dim * 8);
-    a.fJ = (double*)base;                      base += align_up((size_t)batch_events * 8);
-    double* d_f = (double*)base;
-    std::vector<double> x_host(per_dim), f_host(batch_events);
+    // page-locked host staging (x and f per slot), kept with the grid and grown on demand; four events
+    const size_t need = 2 * (per_dim + batch_events);
+    if (g->h_cb_doubles < need) {
+        if (g->h_cb) cudaFreeHost(g->h_cb);
+        g->h_cb = nullptr;
+        g->h_cb_doubles = 0;
+        CUDA_TRY(g, cudaHostAlloc((void**)&g->h_cb, sizeof(double) * need, cudaHostAllocDefault));
+        g->h_cb_doubles = need;
+    }
+    for (cudaEvent_t& ev : g->cb_ev)
+        if (!ev) CUDA_TRY(g, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+    vegas::DebugArgs a[2];
+    double* d_f[2];
+    double* x_host[2];
+    double* f_host[2];
+    for (int s = 0; s < 2; ++s) {
+        unsigned char* base = (unsigned char*)dev_scratch + (s < n_slots ? (size_t)s * slot_bytes : 0);
+        a[s] = vegas::DebugArgs{};
+        a[s].edges = g->d_edges;
+        a[s].key0 = (uint32_t)(seed & 0xFFFFFFFFu);
+        a[s].key1 = (uint32_t)(seed >> 32);
+        a[s].iteration = iteration;
+        a[s].dim = dim;
+        a[s].n_bins = g->n_bins;
+        a[s].jac_scale = jac_scale_for(g, VEGAS_FP64);
+        a[s].words = (uint32_t*)base;                 base += align_up(per_dim * 4);
+        a[s].bins = (int32_t*)base;                   base += align_up(per_dim * 4);
+        a[s].x = (double*)base;                       base += align_up(per_dim * 8);
+        a[s].fJ = (double*)base;                      base += align_up((size_t)batch_events * 8);
+        d_f[s] = (double*)base;
+        x_host[s] = g->h_cb + (size_t)s * (per_dim + batch_events);
+        f_host[s] = x_host[s] + per_dim;
+    }
     const int blocks = g->active_blocks < g->sm_count ? g->active_blocks : g->sm_count;
-    for (uint64_t done = 0; done < n_events; done += batch_events) {
-        const uint32_t n = (uint32_t)((n_events - done < batch_events) ? n_events - done : batch_events);
-        a.first_event = done;
-        a.count = n;
-        // S1-S3 for the batch with f = 1: x, bins and J = prod n_bins Delta go to the scratch (the only place in the
-        // library where per-event arrays exist)
-        CUDA_TRY(g, vegas::launch_debug(VEGAS_F_CONST, VEGAS_FP64, false, a, g->derived[VEGAS_F_CONST], st));
-        CUDA_TRY(g, cudaMemcpyAsync(x_host.data(), a.x, sizeof(double) * (size_t)n * dim, cudaMemcpyDeviceToHost, st));
-        CUDA_TRY(g, cudaStreamSynchronize(st));
-        fn(x_host.data(), (uint64_t)n, dim, f_host.data(), user);                    // S4 on the host
-        CUDA_TRY(g, cudaMemcpyAsync(d_f, f_host.data(), sizeof(double) * n, cudaMemcpyHostToDevice, st));
-        CUDA_TRY(g, vegas::launch_accumulate_batch(d_f, a.fJ, a.bins, n, dim, g->n_bins, g->d_partials, blocks, st));
-        CUDA_TRY(g, cudaStreamSynchronize(st));                                       // f_host is reused by the next batch
-        g->launches += 2;
+    const uint64_t n_batches = (n_events + batch_events - 1) / batch_events;
+    auto batch_size = [&](uint64_t k) {
+        const uint64_t done = k * (uint64_t)batch_events;
+        return (uint32_t)((n_events - done < batch_events) ? n_events - done : batch_events);
+    };
+    // S1-S3 for batch k with f = 1: x, bins and J = prod n_bins Delta go to the slot's scratch (the only place in the
+    // library where per-event arrays exist), x on to the host
+    auto enqueue_sample = [&](uint64_t k, int s) -> int {
+        a[s].first_event = k * (uint64_t)batch_events;
+        a[s].count = batch_size(k);
+        CUDA_TRY(g, vegas::launch_debug(VEGAS_F_CONST, VEGAS_FP64, false, a[s], g->derived[VEGAS_F_CONST], st));
+        CUDA_TRY(g, cudaMemcpyAsync(x_host[s], a[s].x, sizeof(double) * (size_t)a[s].count * dim, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(g, cudaEventRecord(g->cb_ev[s], st));
+        g->launches++;
+        return VEGAS_OK;
+    };
+    rc = enqueue_sample(0, 0);
+    if (rc) return rc;
+    bool f_in_flight[2] = {false, false};
+    for (uint64_t k = 0; k < n_batches; ++k) {
+        const int s = n_slots == 2 ? (int)(k & 1) : 0;
+        const uint32_t n = batch_size(k);
+        if (n_slots == 2 && k + 1 < n_batches) {           // the device goes on with batch k+1 while the host evaluates batch k
+            rc = enqueue_sample(k + 1, s ^ 1);
+            if (rc) return rc;
+        }
+        CUDA_TRY(g, cudaEventSynchronize(g->cb_ev[s]));                               // x of batch k is on the host
+        if (f_in_flight[s]) CUDA_TRY(g, cudaEventSynchronize(g->cb_ev[2 + s]));       // f of batch k-2 has left f_host[s]
+        fn(x_host[s], (uint64_t)n, dim, f_host[s], user);                             // S4 on the host
+        CUDA_TRY(g, cudaMemcpyAsync(d_f[s], f_host[s], sizeof(double) * n, cudaMemcpyHostToDevice, st));
+        CUDA_TRY(g, cudaEventRecord(g->cb_ev[2 + s], st));
+        f_in_flight[s] = true;
+        CUDA_TRY(g, vegas::launch_accumulate_batch(d_f[s], a[s].fJ, a[s].bins, n, dim, g->n_bins, g->d_partials, blocks, st));
+        g->launches++;
+        if (n_slots == 1 && k + 1 < n_batches) {           // one slot: the next sample overwrites what accumulate reads -- stream order
+            rc = enqueue_sample(k + 1, 0);
+            if (rc) return rc;
+        }
     }
     rc = vegas_reduce(g, cuda_stream);
     if (rc) return rc;

@@ -165,6 +165,42 @@ def test_host_callback_integrand_matches_the_oracle(B):
     g.close()
 
 
+def test_host_callback_overlapped_and_serial_batches_agree(B):
+    """The two-slot form (device samples batch k+1 while the host evaluates batch k) and the one-slot serial form see the
+    same batches in the same order and give the same sums; many batches, ragged tail, a slow callback."""
+    import time
+    dim, nb, n, seed = 5, 30, 123_457, 77
+    edges = W.adapted_edges(dim, nb, seed=8)
+    g = B.VegasGrid(dim, nb)
+    g.set_edges(edges)
+    seen = {True: [], False: []}
+
+    def make(mode):
+        def f_host(x):
+            seen[mode].append((x.shape[0], float(x[0, 0]), float(x[-1, -1])))
+            if len(seen[mode]) % 3 == 0:
+                time.sleep(0.002)                      # the device is ahead of the host here
+            return np.exp(-np.sum((x - 0.4) ** 2, axis=1) / 0.09)
+        return f_host
+
+    res = {}
+    for mode in (True, False):
+        res[mode] = g.iterate_callback(make(mode), n, seed, 1, batch_events=10_000, overlap=mode)
+        assert res[mode][3] == 0
+    assert seen[True] == seen[False] and len(seen[True]) == 13 and seen[True][-1][0] == 3_457
+    assert res[True][0] == res[False][0] and res[True][1] == res[False][1]
+    np.testing.assert_allclose(res[True][2], res[False][2], rtol=1e-13)     # the batch kernel's adds are unordered
+    # against the oracle's sample: same x, f evaluated here, sums in numpy
+    _, bins, x, fJ = O.sample(edges, seed, 1, 0, n, O.CONST)
+    v = np.exp(-np.sum((x - 0.4) ** 2, axis=1) / 0.09) * fJ
+    assert res[True][0] == pytest.approx(v.mean(), rel=1e-12)
+    Hb = np.zeros((dim, nb))
+    for j in range(dim):
+        np.add.at(Hb[j], bins[:, j], v * v)
+    np.testing.assert_allclose(res[True][2], Hb, rtol=1e-10)
+    g.close()
+
+
 def test_user_integrand_shape_limits_and_no_parameters(B):
     # a shape whose table plus one histogram copy exceed the 227 KB of shared memory has no fast path: refused
     g = B.VegasGrid(32, 256)

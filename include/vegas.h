@@ -72,7 +72,7 @@ extern "C" {
 #define VEGAS_F_GENZ_PRODUCT_PEAK 2
 #define VEGAS_F_BW_POLY 3
 /*   VEGAS_F_USER               an integrand supplied as CUDA source and compiled at run time for this grid:
- *                              see vegas_set_user_integrand() below; fp64 only, n_params <= VEGAS_USER_MAX_PARAMS */
+ *                              see vegas_set_user_integrand() below; n_params <= VEGAS_USER_MAX_PARAMS */
 #define VEGAS_F_USER 4
 /*   VEGAS_F_GENZ_DISCONTINUOUS PAPER.md:67-70 Eq.(2) as printed, N = 1 (reading R19): f = 0 where any
  *                              x_j <= a_j, exp(sum_j c_j x_j) elsewhere.  params = { c[0..d-1], a[0..d-1] }, c_j > 0.
@@ -122,8 +122,10 @@ int vegas_set_params(vegas_grid* g, int integrand_id, const double* params_host,
  * (any members, helper functions and constants it needs; no #include of host headers; p points to the
  * n_params doubles given here, read-only).  The library compiles it with NVRTC for sm_100a into the SAME fused
  * iterate kernel the built-in integrands use (streaming form: x is consumed dimension by dimension, nothing per
- * event is stored) for this grid's dim, and selects it with integrand_id = VEGAS_F_USER, precision VEGAS_FP64,
- * in vegas_iterate / vegas_accumulate / vegas_integrate.  vegas_set_params(g, VEGAS_F_USER, ...) replaces the
+ * event is stored) for this grid's dim, in both precisions, and selects it with integrand_id = VEGAS_F_USER in
+ * vegas_iterate / vegas_accumulate / vegas_integrate.  With precision VEGAS_FP32 the sampling map, the Jacobian and
+ * v = f*J are fp32 (C11) around the same user code: dim() receives the fp32 x widened to double, finish()'s value is
+ * rounded to fp32 (it must then lie in the fp32 range).  vegas_set_params(g, VEGAS_F_USER, ...) replaces the
  * parameters without recompiling.  log (host, may be NULL) receives the NUL-terminated compiler log, truncated
  * to log_bytes.  Needs libnvrtc.so.12 at run time (loaded on first use).
  * Errors: VEGAS_EINVAL (NULL source, n_params out of range, compile error -> see log; dim * n_bins too large for

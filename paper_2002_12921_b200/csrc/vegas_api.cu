@@ -175,7 +175,7 @@ bool variant_available(const vegas_grid* g, int fid, int precision) {
 bool check_call(const vegas_grid* g, int fid, int precision) {
     if (!g) return false;
     if (fid < 0 || fid > VEGAS_F_GENZ_DISCONTINUOUS || !g->params_set[fid]) return false;
-    if (fid == VEGAS_F_USER) return g->ukernel.kernel != nullptr && precision == VEGAS_FP64 && g->variant == 0;
+    if (fid == VEGAS_F_USER) return g->ukernel.kernel != nullptr && (precision == VEGAS_FP64 || precision == VEGAS_FP32) && g->variant == 0;
     if (expected_n_params(fid, g->dim) < 0) return false;
     if (g->variant != 0 && !variant_available(g, fid, precision)) return false;
     if (fid == VEGAS_F_GENZ_DISCONTINUOUS) return precision == VEGAS_FP64;      // the cuts are decided in fp64 (vegas.h)
@@ -256,6 +256,12 @@ void rot_constants(const vegas_grid* g, int fid, int precision, double* shift, d
         double ps = 1.0;                                         // u_j = x_j; J = prod nb Delta_j = nb^d prod B_j 2^32
         for (int j = 0; j < dim; ++j) { scale[j] = 1.0; ps *= nb; }
         *post_scale = ps;
+        if (precision == VEGAS_FP32) {
+            // fp32 (C11): n_bins^d is shared out over the four chains (IntegrandU<USER>::value)
+            const float q32 = (float)std::pow(nb, 0.25 * dim);
+            *fin1 = (double)q32;
+            *post_scale = std::exp((double)dim * std::log(nb) - 4.0 * std::log((double)q32));
+        }
         for (int k = 0; k < vegas::kRotParams; ++k) fpar[k] = g->user[fid][k];
     } else if (fid == VEGAS_F_BW_POLY) {
         // u_0 = (s - M^2)/(M Gamma) with s = s_min + x_0 ds (C5): the Breit-Wigner is 1/(1 + u_0^2); u_j = x_j, j >= 1
@@ -352,7 +358,7 @@ RotShape rot_shape(const vegas_grid* g, int fid) {
 
 cudaError_t launch_rot(vegas_grid* g, int fid, int precision, int dim, const vegas::RotArgs& a, const RotShape& s,
                        cudaStream_t st) {
-    if (fid == VEGAS_F_USER) return vegas::user_launch(&g->ukernel, a, s.blocks, s.threads, s.shmem, st);
+    if (fid == VEGAS_F_USER) return vegas::user_launch(&g->ukernel, precision == VEGAS_FP32, a, s.blocks, s.threads, s.shmem, st);
     if (precision == VEGAS_FP64 && g->variant != 0) {
 #define VEGAS_VAR_CASE(F)                                                                                              \
     case F:                                                                                                            \

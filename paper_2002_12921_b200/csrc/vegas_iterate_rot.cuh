@@ -54,7 +54,7 @@ template <int FID, typename T, int NBLK> struct RotCtx {
 // and cfg2: 8.03e10 -> 8.10e10 with 4)
 // (fp32 product peak and fp32 BW_POLY: always 4, so that no partial product leaves the fp32 range, see their value())
 __host__ __device__ constexpr int rot_chains(int dim, int fid = -1, bool fp32 = false) {
-    return (fp32 && (fid == VEGAS_F_GENZ_PRODUCT_PEAK || fid == VEGAS_F_BW_POLY)) ? 4 : (dim > 12 ? 1 : 4);
+    return (fp32 && (fid == VEGAS_F_GENZ_PRODUCT_PEAK || fid == VEGAS_F_BW_POLY || fid == VEGAS_F_USER)) ? 4 : (dim > 12 ? 1 : 4);
 }
 template <int NCH, typename T> __device__ __forceinline__ T chain_sum(const T (&s)[NCH]) {
     if (NCH == 4) return (s[0] + s[NCH > 1 ? 1 : 0]) + (s[NCH > 2 ? 2 : 0] + s[NCH > 3 ? 3 : 0]);
@@ -448,7 +448,17 @@ template <typename T, int NCH> struct IntegrandU<VEGAS_F_USER, T, NCH> {
         f.dim(4 * blk + ((blk == c.nblk - 1 ? c.gammaL : c.gamma4) ^ i), (double)u, p);
     }
     __device__ __forceinline__ T finish(T, T) { return (T)f.finish(p); }
-    __device__ __forceinline__ T value(const T (&jac)[NCH], T fin0, T fin1) { return finish(fin0, fin1) * chain_prod<NCH, T>(jac); }
+    // fp32 (C11): the sampling map, J and v = f J in fp32 around the user's f (evaluated in the user's own types from
+    // x widened to double, then rounded to fp32); the four partial Jacobian chains take a quarter of n_bins^d each
+    __device__ __forceinline__ T value(const T (&jac)[NCH], T fin0, T fin1) {
+        if (sizeof(T) == 4 && NCH == 4) {
+            T r[NCH];
+#pragma unroll
+            for (int c = 0; c < NCH; ++c) r[c] = jac[c] * fin1;
+            return finish(fin0, fin1) * chain_prod<NCH, T>(r);
+        }
+        return finish(fin0, fin1) * chain_prod<NCH, T>(jac);
+    }
 };
 #endif
 

@@ -96,7 +96,7 @@ def test_user_integrand_parameters_and_errors(B):
         g.set_user_integrand(U.GENZ_DISCONTINUOUS, np.zeros(B.VEGAS_USER_MAX_PARAMS + 1))
     g.set_user_integrand(U.GENZ_DISCONTINUOUS, p)
     with pytest.raises(B.VegasError):
-        g.iterate(1000, 1, 0, B.VEGAS_F_USER, 32)                 # fp64 only
+        g.iterate(1000, 1, 0, B.VEGAS_F_USER, 16)                 # precision is 64 or 32
     with pytest.raises(B.VegasError):
         g.debug_sample(0, 16, 1, 0, B.VEGAS_F_USER, 64)
     edges = W.adapted_edges(6, 50, seed=6)
@@ -162,6 +162,28 @@ def test_host_callback_integrand_matches_the_oracle(B):
     # a non-finite f is reported, not hidden
     I2, s2, _, st2 = g.iterate_callback(lambda x: np.full(x.shape[0], np.inf), 1000, seed, 0, batch_events=512)
     assert st2 == B.VEGAS_ENUMERIC
+    g.close()
+
+
+@pytest.mark.parametrize("name,fid,dim,nb,a", [("GAUSS", O.GAUSS, 6, 50, 0.2), ("GAUSS", O.GAUSS, 20, 50, 0.35),
+                                                ("GENZ_PRODUCT_PEAK", O.GENZ_PRODUCT_PEAK, 12, 64, None)])
+def test_user_integrand_in_fp32(B, name, fid, dim, nb, a):
+    """VEGAS_F_USER with precision 32: the fp32 sampling map (C11) around the user's source, against the fp64 oracle at
+    north_star's 1e-5 on I, sigma and H (per-dimension max-norm, reading F3); the fp64 run of the same source beside it."""
+    p = W.gauss_params(a) if fid == O.GAUSS else W.genz_params(dim, 4)
+    edges = W.adapted_edges(dim, nb, seed=dim)
+    g = B.VegasGrid(dim, nb)
+    g.set_user_integrand(getattr(U, name), p)
+    g.set_edges(edges)
+    n = 300_007
+    oI, oS, oH = O.iterate(edges, n, 21, 3, fid, p, threads=THREADS)
+    I, s, H, st = g.iterate(n, 21, 3, B.VEGAS_F_USER, 32)
+    assert st == 0
+    assert I == pytest.approx(oI, rel=1e-5) and s == pytest.approx(oS, rel=1e-5)
+    assert np.all(np.abs(H - oH) <= 1e-5 * oH.max(axis=1, keepdims=True))
+    assert np.any(H != oH)                                   # it really is the fp32 map
+    I64, s64, H64, _ = g.iterate(n, 21, 3, B.VEGAS_F_USER, 64)
+    assert I64 == pytest.approx(oI, rel=RTOL64) and s64 == pytest.approx(oS, rel=RTOL64)
     g.close()
 
 

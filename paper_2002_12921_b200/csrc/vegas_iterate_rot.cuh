@@ -499,12 +499,16 @@ __host__ __device__ constexpr int rot_sections(int fid, int dim) {
     return !rot_mbar_tokens(fid, dim) ? 1 : ((dim + 3) / 4 < VEGAS_ROT_NSEC ? (dim + 3) / 4 : VEGAS_ROT_NSEC);
 }
 // Two events per token hold (template parameter PAIR of the kernel, picked at launch when warps share a histogram
-// copy): the shapes with 3 Philox blocks, whose 128 registers have room for a second set of histogram addresses and
-// whose large tables leave few copies (cfg4: 2 copies, 7 warps each).  Measured on cfg4: 5.45e10 -> 5.53e10 events/s,
-// barrier stalls per issue 3.97 -> 2.53 (profiles/r02_k1_steps.md); a kernel of its own because the second loop
-// in the same kernel cost the shapes without rings 5 %.
+// copy): every shape of up to 3 Philox blocks, whose register budget has room for a second set of histogram
+// addresses.  It pays most where large tables leave few copies (cfg4: 2 copies, 7 warps each: 5.45e10 -> 5.53e10
+// events/s, barrier stalls per issue 3.97 -> 2.53) and 1..2 % on the short rings of the small shapes (cfg2, cfg5:
+// two independent events in flight per thread); profiles/r02_k1_steps.md.  A kernel of its own because the second
+// loop in the same kernel cost the shapes without rings 5 %.
+#ifndef VEGAS_ROT_PAIR_MIN_DIM
+#define VEGAS_ROT_PAIR_MIN_DIM 2
+#endif
 __host__ __device__ constexpr bool rot_pair_hold(int fid, int dim, int var = 0) {
-    return fid != VEGAS_F_USER && fid != VEGAS_F_BW_POLY && var == 0 && dim >= 9 && dim <= 12;
+    return fid != VEGAS_F_USER && var == 0 && dim >= VEGAS_ROT_PAIR_MIN_DIM && dim <= 12;
 }
 __host__ __device__ constexpr int rot_section_begin(int nblk, int nsec, int s) { return (s * nblk + nsec - 1) / nsec; }
 constexpr int kRotMaxSections = 8;

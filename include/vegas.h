@@ -246,7 +246,7 @@ int vegas_debug_sample(vegas_grid* g, uint64_t first_event, uint32_t count, uint
 /* Launch shape of the fused kernel.  0 = automatic for any field.  blocks: CTAs per launch (default:
  * one per SM); threads: per CTA (multiple of 32, <= 512).  The library has two fused kernels
  * (DESIGN.md "Kernels"): the fast path (path 1: compile-time dimension, affine pre-composed table, bank
- * rotation, exclusive-owner histograms; every built-in integrand in both precisions -- BW_POLY up to 8 dimensions --
+ * rotation, exclusive-owner histograms; every built-in integrand at every dimension -- Genz discontinuous in fp64 only --
  * and user integrands, when the table plus one histogram copy fit the shared memory)
  * and the generic path (path 0: every built-in integrand, any shape).  table_copies / hist_copies are the
  * bank-interleaved replicas of the grid table / histogram of the GENERIC kernel (powers of two, <= 32);
@@ -268,8 +268,9 @@ int vegas_get_launch(vegas_grid* g, int integrand_id, int precision, int* path, 
  *                       to fp32 (half the table read); x = X~_b + Delta~_b * r and J = prod n_bins * Delta~_b in fp64.
  *                       The master grid, the histogram and the refinement stay fp64.  The rounded bins do not tile [0,1)
  *                       exactly: a relative bias of up to dim * 2^-24 on I (measured: DESIGN.md section 11).
- * Both are fp64 modes of the built-in integrands on the fast path: with a variant set, a call with precision 32, with
- * VEGAS_F_USER, or for a shape that only the generic kernel serves returns VEGAS_EINVAL.  vegas_debug_sample reports
+ * Both are fp64 modes of CONST, GAUSS, GENZ_PRODUCT_PEAK and BW_POLY on the fast path: with a variant set, a call with
+ * precision 32, with VEGAS_F_USER or VEGAS_F_GENZ_DISCONTINUOUS, or for a shape that only the generic kernel serves
+ * returns VEGAS_EINVAL.  vegas_debug_sample reports
  * the top 32 bits of U in `words` under VEGAS_VARIANT_U53. */
 #define VEGAS_VARIANT_NONE 0
 #define VEGAS_VARIANT_U53 1

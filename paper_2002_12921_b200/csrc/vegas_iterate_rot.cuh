@@ -2,23 +2,26 @@
 //
 // Same computation as the generic k_iterate (vegas_kernels.cu), for integrands whose dependence on
 // x_j goes through a per-dimension affine variable u_j = scale_j (x_j - shift_j)
-// (CONST, GAUSS: u = n_bins (x - 1/2); GENZ product peak: u = c_j (x - w_j)).  Design points, each
-// driven by a counter in profiles/ (r01_s2_baseline.md, r01_s2_ubench_hist.md, r01_s7_ubench_pipes.md):
+// (CONST, GAUSS: u = n_bins (x - 1/2); GENZ product peak: u = c_j (x - w_j); Genz discontinuous: u = c_j (x - a_j);
+// BW_POLY: u_0 = (s - M^2)/(M Gamma), u_j = x_j; user integrands: u_j = x_j).  Design points, each driven by a counter
+// in profiles/ (r01_s2_baseline.md, r01_s2_ubench_hist.md, r02_ubench_pipes.md, r02_k1_steps.md, r02_k1_final.md):
 //
 //  1. DIM is a compile-time constant: no per-dimension guards, fully unrolled, bins packed one byte
 //     per dimension in registers.
 //  2. Affine pre-composition: the shared-memory table holds, per (dimension, bin), the pair
 //     (A, B) with u = A + B w, where w is the low product word of the split (C3) converted by one
-//     I2F (fp64: exact; u = scale (x - shift) with r = (w + 1/2) 2^-32 folded into A and B) or the
-//     top 23 bits put into a float mantissa (fp32).  One FMA gives u; x_j itself is never formed,
+//     I2F (fp64: exact; u = scale (x - shift) with r = (w + 1/2) 2^-32 folded into A and B), the whole
+//     Philox word (fp64, more than 8 dimensions: RotSplit<double, true>, no wide multiply in the split) or the
+//     top 23 bits of the low product word put into a float mantissa (fp32).  One FMA gives u; x_j itself is never formed,
 //     and B is the Jacobian factor up to a per-dimension constant folded into post_scale.
 //     No integrand parameter is read inside the event loop.
 //  3. Bank rotation.  A Philox block serves 4 dimensions.  The 32 lanes of a warp are split into 4
 //     groups gamma = (lane>>1)&3; at sub-step i group gamma works on dimension 4 blk + (gamma ^ i)
 //     (its four Philox words are permuted accordingly, 8 SELs per block).  So the lanes of one
 //     shared-memory wavefront always touch different dimensions, and the rows
-//         table [blk*n_bins + bin] : 128 B = 4 dim-slots x 2 copies x 16 B   (fp32: 4 x 4 x 8 B)
-//         hist  [blk*n_bins + bin] : 256 B = 2 half-warps x 4 dim-slots x 4 copies x 8 B
+//         table [bin*NBLK + blk] : 128 B = 4 dim-slots x 2 copies x 16 B   (fp32: 4 x 4 x 8 B)
+//         hist  [bin*NBLK + blk] : 256 B = 2 half-warps x 4 dim-slots x 4 copies x 8 B
+//     (ordered [bin][block]: the block enters every address as a compile-time immediate)
 //     are conflict-free whatever bins the lanes drew, with 2 table copies and 8 histogram copies
 //     instead of 8 and 32, and no two lanes of a warp ever touch the same histogram word in one
 //     instruction.  A last block with 2 (1) dimensions uses 2 (1) groups and 4 (8) table copies in
@@ -27,12 +30,13 @@
 //     64-bit integer) shared-memory atomic: atomicAdd(double) is an LDS + DADD + ATOMS.CAST.SPIN + BRA
 //     loop that costs 6.4 shared wavefronts and serialises the 20 updates of an event.  Here the CTA
 //     (one per SM, sharing one table) holds n_groups histogram copies; the `ring` warps of a group
-//     pass a token round a ring of named barriers (bar.sync / bar.arrive on 64 threads, 42 clk per
-//     hand-off) and only the token holder updates the group's histogram, with plain LDS.64 / DADD /
-//     STS.64 (4 wavefronts), the updates of the independent Philox blocks pipelined.  The critical
-//     section is ~10 % of a warp's loop iteration, so a ring of 4..6 warps rarely waits.  When the
-//     shared memory holds one histogram per warp (small dim * n_bins) the ring has length 1 and there
-//     is no synchronisation at all.
+//     pass a token round a ring (named barriers, bar.sync / bar.arrive on 64 threads, 42 clk per hand-off, for
+//     CTAs of up to 16 warps; mbarriers, one per warp and histogram section, for the 24-warp kernels) and only
+//     the token holder updates the group's histogram, with plain LDS.64 / DADD / STS.64 (4 wavefronts), the
+//     updates of the independent Philox blocks pipelined.  When the shared memory holds one histogram per warp
+//     (small dim * n_bins) the ring has length 1 and there is no synchronisation at all.
+//  5. One launch per iteration: the chunk loop runs inside the kernel, and the last CTAs to finish reduce the
+//     partial rows in K2's fixed association, finalise (S7) and refine the grid (S8): rot_tail.
 #pragma once
 #include "vegas_device.cuh"
 #ifndef __CUDACC_RTC__

@@ -416,12 +416,15 @@ def main():
     if world == 1 and not args.no_extra and args.workload == "cfg3" and args.precision == 64 and not args.n_events:
         # ... and the two opt-in variants of the sampling map on the headline workload: what the
         # 32-bit draw saves against 53-bit uniforms, what an fp32-rounded grid table costs
-        for cfg, prec, n_ev, variant in ((3, 32, 0, 0), (5, 64, 0, 0), (4, 64, 100_000_000, 0), (3, 64, 0, 1), (3, 64, 0, 2)):
+        # ... and cfg1 / cfg2 at their OWN sizes (1e5 / 1e7 events per iteration), which SURVEY.md 8(d) lists as reported:
+        # launch- and latency-bound, one launch per iteration
+        for cfg, prec, n_ev, variant in ((3, 32, 0, 0), (5, 64, 0, 0), (4, 64, 100_000_000, 0), (3, 64, 0, 1), (3, 64, 0, 2),
+                                         (1, 64, 0, 0), (2, 64, 0, 0)):
             we = W.config(cfg)
             if n_ev:
                 we = we.scaled(n_ev)
             vname = {0: "", 1: "/u53", 2: "/q32"}[variant]
-            r = measure(we, prec, max(3, min(args.steps, 10)), max(args.warmup, 4), "%s/%d%s" % (we.name, prec, vname), variant=variant)
+            r = measure(we, prec, max(3, min(args.steps, 10 if cfg > 2 else 100)), max(args.warmup, 4), "%s/%d%s" % (we.name, prec, vname), variant=variant)
             if r:
                 extra.append({"workload": r["workload"], "dtype": r["dtype"],
                               "variant": {0: "none", 1: "u53 (53-bit uniforms, two Philox words per draw)",

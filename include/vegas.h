@@ -53,6 +53,9 @@ extern "C" {
                                smoothed histogram has no finite positive sum (that dimension's grid
                                is left unchanged, the others are refined)                           */
 
+#define VEGAS_ELIMIT (-4)   /* vegas_iterate_static() only: dim * n_bins is larger than VEGAS_STATIC_MAX_ENTRIES, the
+                               shape its fixed built-in scratch was sized for; nothing was launched              */
+
 #define VEGAS_MAX_DIM 32
 #define VEGAS_MAX_BINS 256
 #define VEGAS_MAX_PARAMS 160
@@ -201,6 +204,52 @@ int vegas_finalize(vegas_grid* g, uint64_t n_events_total, void* cuda_stream, do
  * H[dim][n_bins] } that vegas_reduce() writes and vegas_finalize() / vegas_refine() read. */
 void* vegas_totals_device(vegas_grid* g);
 size_t vegas_totals_count(const vegas_grid* g);
+
+/* One iteration for callers that have no device memory to give beyond the data itself (steps S1-S7 as vegas_iterate).
+ *
+ * Who this is for.  Every other compute call needs a vegas_grid, and a vegas_grid needs a device workspace that the caller
+ * allocates.  Some callers cannot do that.  The typical one is code running as an op or callback inside a framework that
+ * owns the GPU's memory -- a TensorFlow custom op (the paper's library lives on TensorFlow) or a PyTorch
+ * extension that gets handed its input and output buffers and nothing else: the framework's pool has usually claimed most
+ * of the card already, so a cudaMalloc from inside the op fails or eats into someone else's budget, and it stalls every
+ * stream on the device while it runs.  Others are a service loop that must not see that device-wide stall on its latency
+ * path, and a process that was given a fixed slice of device memory at start-up with no headroom for a workspace whose
+ * size depends on the grid shape.  For them this call needs only what they already hold: the grid edges going in, the
+ * result and the histogram coming out.  It calls no cudaMalloc / cudaFree / cudaMallocHost and no library routine that
+ * allocates; the per-CTA partial sums and the reduced totals that the kernels need as working memory live in an array
+ * compiled into the library.
+ *
+ * The price of that array.  It is 2 642 976 bytes (161 rows of 4 + VEGAS_STATIC_MAX_ENTRIES doubles), it exists once per
+ * GPU in every process that loads this library, from the moment the library's device code is loaded on that GPU until the
+ * process exits, whether or not this call is ever used.  Shapes with dim * n_bins > VEGAS_STATIC_MAX_ENTRIES (2048: e.g.
+ * 20 x 100, 16 x 128, 8 x 256; all five BASELINE.json configs fit) are refused with VEGAS_ELIMIT before anything is
+ * launched -- use a vegas_grid for those.
+ *
+ * Arguments.  edges_dev: DEVICE, [dim][n_bins+1] fp64, every row increasing from 0 to 1 (read only; not checked -- it is
+ * on the device).  params_host / n_params: HOST, the integrand's parameter array exactly as vegas_set_params() takes it
+ * (VEGAS_F_USER is not served: compiling one allocates).  result_dev: DEVICE, 3 doubles, receives { I, sigma, status }
+ * with status 0.0 or -3.0 (VEGAS_ENUMERIC: the sums came out non-finite).  hist_dev: DEVICE, [dim][n_bins] fp64, receives
+ * the histogram of v^2 (C6); may be NULL.  Both outputs are caller-owned and fully overwritten.  The call runs on the
+ * CURRENT device and only enqueues work on `cuda_stream`: the outputs are valid once the stream has reached that point.
+ * Same sample as vegas_iterate with the same (seed, iteration) (C2); it runs the library's generic fused kernel in one
+ * launch plus the fixed-order reduction, so I, sigma and H agree with vegas_iterate to rounding (summation order), and
+ * repeated calls with the same arguments give the same bits.
+ *
+ * First call on each GPU.  It looks up the device address of the built-in array and the device's limits and keeps them
+ * for later calls (guarded by a lock).  Make that first call at start-up, outside of any stream capture.
+ *
+ * Sharing.  All calls on one GPU -- from any thread, on any stream -- use the SAME array, and it still holds whatever
+ * the previous call left there.  Each call therefore zeroes, in stream order, the rows it is about to use before its
+ * kernels run.  Two calls that can execute at the same time on the GPU (different streams without an event between them,
+ * or two host threads) overwrite each other's partial sums and both results are garbage: keep all calls on one stream, or
+ * order them with events.  Calls that follow each other on one stream are safe; no host synchronisation is needed.
+ *
+ * Errors: VEGAS_EINVAL (NULL edges_dev / result_dev, n_events < 2, bad shape, id, precision or parameters -- the same
+ * rules as vegas_set_params / vegas_iterate), VEGAS_ELIMIT (see above), VEGAS_ECUDA (no device, launch failure). */
+#define VEGAS_STATIC_MAX_ENTRIES 2048
+int vegas_iterate_static(const double* edges_dev, int dim, int n_bins, uint64_t n_events, uint64_t seed,
+                         uint32_t iteration, int integrand_id, const double* params_host, int n_params, int precision,
+                         void* cuda_stream, double* result_dev, double* hist_dev);
 
 /* Refine the grid (step S8, reading C8: smooth, normalise, compress with damping alpha, rebin), per
  * dimension, fp64.  hist_host NULL = use the histogram the last iteration left on the device;

@@ -15,7 +15,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libvegas_b200.so")
 
-VEGAS_OK, VEGAS_EINVAL, VEGAS_ECUDA, VEGAS_ENUMERIC = 0, -1, -2, -3
+VEGAS_OK, VEGAS_EINVAL, VEGAS_ECUDA, VEGAS_ENUMERIC, VEGAS_ELIMIT = 0, -1, -2, -3, -4
+VEGAS_STATIC_MAX_ENTRIES = 2048
 VEGAS_F_CONST, VEGAS_F_GAUSS, VEGAS_F_GENZ_PRODUCT_PEAK, VEGAS_F_BW_POLY, VEGAS_F_USER = 0, 1, 2, 3, 4
 VEGAS_F_GENZ_DISCONTINUOUS = 5
 VEGAS_USER_MAX_PARAMS = 64
@@ -49,6 +50,8 @@ SIGNATURES = {
     "vegas_get_edges": (C.c_int, [_vp, _f64p, _vp]),
     "vegas_get_hist": (C.c_int, [_vp, _f64p, _vp]),
     "vegas_iterate": (C.c_int, [_vp, _u64, _u64, _u64, C.c_uint32, C.c_int, C.c_int, _vp, _f64p, _f64p, _f64p]),
+    "vegas_iterate_static": (C.c_int, [_vp, C.c_int, C.c_int, _u64, _u64, C.c_uint32, C.c_int, _f64p, C.c_int, C.c_int,
+                                       _vp, _vp, _vp]),
     "vegas_begin_iteration": (C.c_int, [_vp, _vp]),
     "vegas_accumulate": (C.c_int, [_vp, _u64, _u64, _u64, _u64, C.c_uint32, C.c_int, C.c_int, _vp]),
     "vegas_reduce": (C.c_int, [_vp, _vp]),
@@ -126,6 +129,34 @@ def vegas_combine(I_k, sigma_k, n_skip=0):
     if rc:
         raise VegasError(rc)
     return I.value, s.value, c.value
+
+
+def vegas_iterate_static(edges, n_events, seed, iteration, integrand_id, params, result, hist=None,
+                         precision=VEGAS_FP64, stream=None):
+    """One iteration without a grid handle and without any device workspace (include/vegas.h: vegas_iterate_static).
+
+    For code that only holds the buffers it was given -- an op inside a framework that owns the GPU memory pool, a
+    latency-bound loop, a process on a fixed memory budget -- and so cannot allocate the workspace a VegasGrid needs.
+    edges [dim, n_bins+1], result [>=3] and hist [dim, n_bins] (optional) are CUDA float64 torch tensors owned by the
+    caller, contiguous, on the current device; params is a host array as for set_params.  Only enqueues work on the
+    stream: result = {I, sigma, status} and hist are valid once the stream gets there (torch.cuda.synchronize() or
+    an event).  Shapes with dim * n_bins > VEGAS_STATIC_MAX_ENTRIES raise VegasError(VEGAS_ELIMIT).  All calls on a
+    GPU share one built-in scratch array: issue them on one stream, or order them with events."""
+    import torch
+    for t, what in ((edges, "edges"), (result, "result"), (hist, "hist")):
+        if t is None and what == "hist":
+            continue
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+            raise VegasError(VEGAS_EINVAL, "%s must be a contiguous CUDA float64 tensor" % what)
+    dim, n_bins = int(edges.shape[0]), int(edges.shape[1]) - 1
+    if result.numel() < 3 or (hist is not None and tuple(hist.shape) != (dim, n_bins)):
+        raise VegasError(VEGAS_EINVAL, "result needs 3 elements, hist the shape [dim, n_bins]")
+    p = np.ascontiguousarray(np.atleast_1d(np.asarray(params if params is not None else [], dtype=np.float64)))
+    rc = lib.vegas_iterate_static(_vp(edges.data_ptr()), dim, n_bins, int(n_events), int(seed), int(iteration),
+                                  integrand_id, _ptr(p) if p.size else None, p.size, precision, _stream(stream),
+                                  _vp(result.data_ptr()), _vp(hist.data_ptr()) if hist is not None else None)
+    if rc:
+        raise VegasError(rc)
 
 
 class VegasGrid:

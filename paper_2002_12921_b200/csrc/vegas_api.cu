@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1145,12 +1146,135 @@ int vegas_reset_counters(vegas_grid* g) {
     return VEGAS_OK;
 }
 
+}  // extern "C"
+#pragma GCC visibility pop
+
+// =============================================================================================
+// vegas_iterate_static: one iteration for a caller that cannot give the library any device memory beyond its inputs
+// and outputs (include/vegas.h says who that is).  The working memory of the generic fused kernel K1 and of the
+// reduction K2 -- one row { S1 hi, S1 lo, S2 hi, S2 lo, H[dim][n_bins] } per CTA, then one row of totals -- lives in
+// the array below instead of a caller workspace.  Nothing in this path allocates: no cudaMalloc / cudaFree /
+// cudaMallocHost, no vegas_grid with a workspace; the kernels and their launchers are the ones vegas_iterate uses
+// with pinned copy counts, given pointers into this array.
+//
+// The array is device memory that the CUDA runtime reserves on every GPU where this translation unit's device code
+// gets loaded, until the process exits (kStaticDoubles * 8 = 2 642 976 bytes).  On the host the name
+// g_static_scratch is only a handle for the runtime's symbol table, NOT an address a kernel can use: the device
+// address is asked for once per device with cudaGetSymbolAddress (static_setup) and that pointer is what the
+// kernels get.
+// =============================================================================================
+namespace {
+constexpr int kStaticMaxBlocks = 160;                                        // >= one CTA per SM of a B200 (148)
+constexpr size_t kStaticRow = 4 + (size_t)VEGAS_STATIC_MAX_ENTRIES;          // doubles per CTA row / totals row
+constexpr size_t kStaticDoubles = kStaticRow * (kStaticMaxBlocks + 1);       // CTA rows, then the totals row
+}  // namespace
+
+static __device__ __align__(256) double g_static_scratch[kStaticDoubles];
+
+namespace {
+
+struct StaticDevice {
+    bool ready = false;
+    double* scratch = nullptr;      // DEVICE address of g_static_scratch on this GPU
+    int sm_count = 0;
+    size_t smem_optin = 0;
+};
+StaticDevice g_static_dev[vegas::kMaxDevices];
+std::mutex g_static_mutex;
+
+// Once per device, with that device current: the array's device address and the limits the launch shape needs.
+cudaError_t static_setup(int dev, StaticDevice* out) {
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticDevice& d = g_static_dev[dev];
+    if (!d.ready) {
+        void* ptr = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&ptr, g_static_scratch);
+        if (e != cudaSuccess) return e;
+        int sms = 0, optin = 0;
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+        e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+        if (e != cudaSuccess) return e;
+        d.scratch = static_cast<double*>(ptr);
+        d.sm_count = sms;
+        d.smem_optin = (size_t)optin;
+        d.ready = true;
+    }
+    *out = d;
+    return cudaSuccess;
+}
+
+}  // namespace
+
+#pragma GCC visibility push(default)
+extern "C" {
+
+int vegas_iterate_static(const double* edges_dev, int dim, int n_bins, uint64_t n_events, uint64_t seed,
+                         uint32_t iteration, int fid, const double* params_host, int n_params, int precision,
+                         void* cuda_stream, double* result_dev, double* hist_dev) {
+    if (!edges_dev || !result_dev || n_events < 2 || !valid_shape(dim, n_bins)) return VEGAS_EINVAL;
+    if ((size_t)dim * n_bins > (size_t)VEGAS_STATIC_MAX_ENTRIES) return VEGAS_ELIMIT;      // before anything is launched
+    if (fid == VEGAS_F_USER) return VEGAS_EINVAL;
+
+    // a host-only grid object: it carries the shape and the derived integrand parameters through the same
+    // validation and derivation as vegas_set_params / vegas_accumulate; it has no workspace and owns nothing
+    vegas_grid host;
+    host.dim = dim;
+    host.n_bins = n_bins;
+    int rc = vegas_set_params(&host, fid, params_host, n_params);
+    if (rc) return rc;
+    if (!check_call(&host, fid, precision)) return VEGAS_EINVAL;
+
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= vegas::kMaxDevices) return VEGAS_ECUDA;
+    StaticDevice sd;
+    if (static_setup(dev, &sd) != cudaSuccess) return VEGAS_ECUDA;
+    host.device = dev;
+    host.sm_count = sd.sm_count;
+    host.smem_optin = sd.smem_optin;
+    host.cfg_blocks = sd.sm_count < kStaticMaxBlocks ? sd.sm_count : kStaticMaxBlocks;     // one CTA per SM, rows permitting
+    LaunchShape s;
+    if (resolve_launch(&host, precision, &s)) return VEGAS_EINVAL;
+
+    const size_t nent = (size_t)dim * n_bins, ntot = 4 + nent;
+    double* partials = sd.scratch;                            // [s.blocks][ntot]
+    double* totals = sd.scratch + (size_t)kStaticMaxBlocks * kStaticRow;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+
+    vegas::IterArgs a{};
+    a.edges = edges_dev;
+    a.partials = partials;
+    a.first_event = 0;
+    a.count = n_events;
+    a.key0 = (uint32_t)(seed & 0xFFFFFFFFu);
+    a.key1 = (uint32_t)(seed >> 32);
+    a.iteration = iteration;
+    a.dim = dim;
+    a.n_bins = n_bins;
+    a.log_ct = ilog2(s.ct);
+    a.log_ch = ilog2(s.ch);
+    a.jac_scale = jac_scale_for(&host, precision);
+    if (fid != VEGAS_F_BW_POLY) {
+        double fpar_unused[vegas::kRotParams];
+        rot_constants(&host, fid, precision, a.shift, a.scale, &a.post_scale, &a.fin0, &a.fin1, &a.jac_init, fpar_unused, false);
+    }
+    // the CTA rows are accumulated into (K1 adds to its row): the previous call's sums must go first, in stream order
+    CUDA_TRY(nullptr, cudaMemsetAsync(partials, 0, sizeof(double) * ntot * s.blocks, st));
+    CUDA_TRY(nullptr, vegas::launch_iterate(fid, precision, a, host.derived[fid], s.blocks, s.threads, s.shmem, st));
+    CUDA_TRY(nullptr, vegas::launch_reduce(partials, s.blocks, (int)ntot, totals, st));     // writes every total
+    CUDA_TRY(nullptr, vegas::launch_finalize(totals, (double)n_events, result_dev, st));
+    if (hist_dev)
+        CUDA_TRY(nullptr, cudaMemcpyAsync(hist_dev, totals + 4, sizeof(double) * nent, cudaMemcpyDeviceToDevice, st));
+    return VEGAS_OK;
+}
+
 const char* vegas_strerror(int code) {
     switch (code) {
     case VEGAS_OK: return "ok";
     case VEGAS_EINVAL: return "invalid argument";
     case VEGAS_ECUDA: return "CUDA runtime or launch failure (see vegas_last_cuda_error)";
     case VEGAS_ENUMERIC: return "non-finite sums, or a histogram row without a finite positive sum in refine";
+    case VEGAS_ELIMIT: return "vegas_iterate_static: dim * n_bins exceeds VEGAS_STATIC_MAX_ENTRIES (2048), the shape its built-in scratch holds; use a vegas_grid";
     default: return "unknown error code";
     }
 }

@@ -19,8 +19,10 @@
  *
  * Conventions for every entry point
  *   - Return value: 0 (VEGAS_OK) or a negative VEGAS_E* code; vegas_strerror() explains it.  No C++
- *     exception crosses this boundary.  There is no global state; calls on ONE vegas_grid are not
- *     thread-safe, different grids are independent.
+ *     exception crosses this boundary.  Calls on ONE vegas_grid are not thread-safe; different grids are
+ *     independent and may be used from different host threads.  The only process-wide state is internal and
+ *     lock-protected: per kernel and device, the shared-memory size already configured for it, and the built-in
+ *     scratch array of vegas_iterate_static().
  *   - "host" pointers are ordinary host memory owned by the caller (pageable or pinned), row-major,
  *     fp64 unless stated.  "device" pointers are CUDA device memory owned by the caller.
  *   - The library never allocates device memory and never creates streams: the caller provides one
@@ -292,8 +294,12 @@ int vegas_debug_sample(vegas_grid* g, uint64_t first_event, uint32_t count, uint
                        uint32_t iteration, int integrand_id, int precision, void* dev_scratch,
                        void* cuda_stream, uint32_t* words, int32_t* bins, double* x, double* fJ);
 
-/* Launch shape of the fused kernel.  0 = automatic for any field.  blocks: CTAs per launch (default:
- * one per SM); threads: per CTA (multiple of 32, <= 512).  The library has two fused kernels
+/* Launch shape of the fused kernel.  0 = automatic for any field.  blocks: CTAs per launch (default: one per SM, at
+ * most 1024); threads: per CTA, a multiple of 32 up to 1024 -- a REQUEST that each kernel clamps to its own launch bound:
+ * the generic kernel runs at most 512 threads, a fast-path kernel at most 12, 16 or 24 warps (384 / 512 / 768 threads)
+ * depending on integrand and dimension (automatic = that maximum, or the warp count below it that gives the most
+ * histogram copies), and a user integrand's kernel 12 warps.  vegas_get_launch reports the EFFECTIVE shape, which is the
+ * only way to know what a call will run with.  The library has two fused kernels
  * (DESIGN.md "Kernels"): the fast path (path 1: compile-time dimension, affine pre-composed table, bank
  * rotation, exclusive-owner histograms; every built-in integrand at every dimension -- Genz discontinuous in fp64 only --
  * and user integrands, when the table plus one histogram copy fit the shared memory)

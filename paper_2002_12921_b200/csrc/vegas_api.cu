@@ -892,6 +892,9 @@ int vegas_integrate_from(vegas_grid* g, uint32_t first_iteration, int n_iter, in
     cudaStream_t st = (cudaStream_t)cuda_stream;
     CUDA_TRY(g, cudaSetDevice(g->device));
     CUDA_TRY(g, cudaMemsetAsync(g->d_status, 0, sizeof(int), st));
+    // the CTAs-done tickets of the one-launch iteration reset themselves in the tail; a launch that aborted would
+    // leave them counting, and only vegas_create zeroes them otherwise
+    CUDA_TRY(g, cudaMemsetAsync(g->d_counter, 0, sizeof(unsigned int) * (vegas::kReduceSlices + 1), st));
     for (int k = 0; k < n_iter; ++k) {
         const int rc = enqueue_iteration(g, n_events, chunk_events, seed, first_iteration + (uint32_t)k, fid, precision, st,
                                          alpha >= 0.0 ? alpha : -1.0, g->d_result + (size_t)kResultStride * k);
@@ -1033,7 +1036,10 @@ int vegas_iterate_callback(vegas_grid* g, uint64_t n_events, uint32_t batch_even
         g->launches++;
         return VEGAS_OK;
     };
-    rc = enqueue_sample(0, 0);
+    // the two-slot pipeline; on any error the caller's stream is drained before returning (below): copies into the
+    // page-locked staging and kernels on the scratch slots may still be in flight, and the next call may free both
+    auto pipeline = [&]() -> int {
+    int rc = enqueue_sample(0, 0);
     if (rc) return rc;
     bool f_in_flight[2] = {false, false};
     for (uint64_t k = 0; k < n_batches; ++k) {
@@ -1056,8 +1062,13 @@ int vegas_iterate_callback(vegas_grid* g, uint64_t n_events, uint32_t batch_even
             if (rc) return rc;
         }
     }
-    rc = vegas_reduce(g, cuda_stream);
-    if (rc) return rc;
+    return vegas_reduce(g, cuda_stream);
+    };
+    rc = pipeline();
+    if (rc) {
+        cudaStreamSynchronize(st);                          // nothing of this call is left in flight
+        return rc;
+    }
     return finish_iteration(g, n_events, st, I, sigma, hist_host);
 }
 

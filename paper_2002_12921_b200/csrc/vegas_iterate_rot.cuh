@@ -797,9 +797,13 @@ static __device__ __noinline__ void rot_tail(const RotArgs& a, int dim, unsigned
         int conc = (int)((size_t)a.tail_smem_doubles / (size_t)per);
         if (conc > nwarps) conc = nwarps;
         if (warp < conc)
-            for (int j = warp; j < DIM; j += conc)
+            for (int j = warp; j < DIM; j += conc) {
                 refine_dimension(const_cast<double*>(a.edges) + (size_t)j * (nb + 1), a.totals + 4 + (size_t)j * nb, nb,
                                  a.tail_alpha, a.status, scratch + (size_t)warp * per, lane, 32, SyncWarp{});
+                // refine_dimension ends in a walk of data-dependent length that still reads X[], m[], cum[] of this
+                // warp's scratch: every lane must be out of it before the next dimension overwrites them
+                __syncwarp();
+            }
     }
 }
 

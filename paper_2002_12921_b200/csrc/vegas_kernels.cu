@@ -7,6 +7,8 @@
 // Step names S1..S9 are SURVEY.md 8(a); readings C1..C11 are DESIGN.md.
 #include "vegas_kernels.h"
 
+#include <mutex>
+
 #include "vegas_device.cuh"
 #include "vegas_iterate_rot.cuh"
 
@@ -396,11 +398,16 @@ static cudaError_t launch_iterate_t(const IterArgs& a, const FParams<T>& fp, int
     static size_t configured_dev[kMaxDevices] = {};   // per instantiation and device: the attribute is per context
     int dev_ = 0;
     if (cudaGetDevice(&dev_) != cudaSuccess || dev_ < 0 || dev_ >= kMaxDevices) return cudaErrorInvalidDevice;
-    size_t& configured = configured_dev[dev_];
-    if (shmem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem);
-        if (e != cudaSuccess) return e;
-        configured = shmem;
+    {
+        // grids on different host threads may launch the same kernel: the cache and the attribute change together
+        static std::mutex configured_mutex;
+        std::lock_guard<std::mutex> lock(configured_mutex);
+        size_t& configured = configured_dev[dev_];
+        if (shmem > configured) {
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem);
+            if (e != cudaSuccess) return e;
+            configured = shmem;
+        }
     }
     kern<<<blocks, threads, shmem, st>>>(a, fp);
     return cudaGetLastError();
@@ -512,11 +519,16 @@ cudaError_t launch_accumulate_batch(const double* f, const double* J, const int3
     static size_t configured_dev[kMaxDevices] = {};   // per device: the attribute is per context
     int dev_ = 0;
     if (cudaGetDevice(&dev_) != cudaSuccess || dev_ < 0 || dev_ >= kMaxDevices) return cudaErrorInvalidDevice;
-    size_t& configured = configured_dev[dev_];
-    if (shmem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(k_accumulate_batch, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem);
-        if (e != cudaSuccess) return e;
-        configured = shmem;
+    {
+        // grids on different host threads may launch the same kernel: the cache and the attribute change together
+        static std::mutex configured_mutex;
+        std::lock_guard<std::mutex> lock(configured_mutex);
+        size_t& configured = configured_dev[dev_];
+        if (shmem > configured) {
+            cudaError_t e = cudaFuncSetAttribute(k_accumulate_batch, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem);
+            if (e != cudaSuccess) return e;
+            configured = shmem;
+        }
     }
     k_accumulate_batch<<<blocks, 256, shmem, st>>>(f, J, bins, count, dim, n_bins, partials);
     return cudaGetLastError();

@@ -3,6 +3,8 @@
 // (ROT_VAR: 0 = the method, 1 = 53-bit uniforms, 2 = fp32-rounded table; the variants are fp64 only).
 #include "vegas_iterate_rot.cuh"
 
+#include <mutex>
+
 #ifndef ROT_FID
 #error "compile with -DROT_FID=<integrand id> -DROT_FP=<64|32>"
 #endif
@@ -25,11 +27,16 @@ static cudaError_t go_kernel(const RotArgs& a, int blocks, int threads, size_t s
     static size_t configured_dev[kMaxDevices] = {};   // per kernel and device: the attribute is per context
     int dev_ = 0;
     if (cudaGetDevice(&dev_) != cudaSuccess || dev_ < 0 || dev_ >= kMaxDevices) return cudaErrorInvalidDevice;
-    size_t& configured = configured_dev[dev_];
-    if (shmem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem);
-        if (e != cudaSuccess) return e;
-        configured = shmem;
+    {
+        // grids on different host threads may launch the same kernel: the cache and the attribute change together
+        static std::mutex configured_mutex;
+        std::lock_guard<std::mutex> lock(configured_mutex);
+        size_t& configured = configured_dev[dev_];
+        if (shmem > configured) {
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem);
+            if (e != cudaSuccess) return e;
+            configured = shmem;
+        }
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(blocks);

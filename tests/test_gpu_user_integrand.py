@@ -253,6 +253,36 @@ def test_user_integrand_shape_limits_and_no_parameters(B):
     g.close(); g2.close(); g3.close()
 
 
+def test_one_launch_refinement_of_more_dimensions_than_warps_equals_the_stand_alone_kernel(B):
+    """The one-launch iteration refines one dimension per warp and, beyond the kernel's warp count, several in turn
+    through the same shared scratch (a user kernel has 12 warps: dim 32 makes three rounds; the 24-warp built-in kernels
+    two from dim 25 on).  The stand-alone refinement (K3, one CTA per dimension) never reuses scratch: same edges, bit
+    for bit."""
+    n, seed, alpha = 200_003, 5, 1.5
+    for dim, nb, user in ((32, 50, True), (32, 37, True), (28, 50, False), (32, 64, False)):
+        edges = []
+        for one_launch in (True, False):
+            g = B.VegasGrid(dim, nb)
+            if user:
+                g.set_user_integrand(U.GAUSS, [0.4])
+                fid = B.VEGAS_F_USER
+            else:
+                g.set_params(B.VEGAS_F_GAUSS, [0.4])
+                fid = B.VEGAS_F_GAUSS
+            assert g.get_launch(fid, 64)["path"] == "rotated"
+            g.set_edges(W.adapted_edges(dim, nb, seed=77))
+            if one_launch:
+                r = g.integrate(1, n, seed, alpha, fid, 64)
+                assert r["status"] == 0
+            else:
+                assert g.iterate(n, seed, 0, fid, 64)[3] == 0
+                assert g.refine(alpha) == 0
+            edges.append(g.get_edges())
+            g.close()
+        assert np.array_equal(edges[0], edges[1]), (dim, nb, user, float(np.max(np.abs(edges[0] - edges[1]))))
+        assert not np.array_equal(edges[0], W.adapted_edges(dim, nb, seed=77))
+
+
 def test_observable_buffer_is_zero_before_any_iteration(B):
     g = B.VegasGrid(3, 20)
     g.set_user_integrand(U.GENZ_PRODUCT_PEAK_WITH_OBSERVABLE, W.genz_params(3, 8))

@@ -32,11 +32,18 @@ INTEGRAND_DIM_FP = {0: 0, 1: 2, 2: 3, 3: 4}                # SURVEY.md 8(d) coun
 INTEGRAND_EVENT_FP = {0: {64: 0, 32: 0}, 1: {64: 19, 32: 5}, 2: {64: 8, 32: 8}, 3: {64: 12, 32: 12}}
 
 
-def n_issue(w, precision):
-    """Algorithmic thread-level instructions per event (SURVEY.md 8(d) counting rule)."""
+def philox_blocks(w, variant=0):
+    """Philox4x32-10 blocks per event: one per 4 dimensions (C2); the u53 variant (C3') draws two words per dimension."""
+    return (w.dim + 1) // 2 if variant == 1 else (w.dim + 3) // 4
+
+
+def n_issue(w, precision, variant=0):
+    """Algorithmic thread-level instructions per event (SURVEY.md 8(d) counting rule).  variant 1 (u53): the
+    same rule with ceil(d/2) Philox blocks (its 53-bit split is counted like the 32-bit one: a lower bound); variant 2
+    (q32) runs the same instruction stream as the method."""
     d = w.dim
     per_dim_fp = INTEGRAND_DIM_FP[w.integrand_id] * (d - 1 if w.integrand_id == 3 else d)
-    return 42 * ((d + 3) // 4) + d * (4 + 1 + 2 + 3) + per_dim_fp + 3 + 4 + INTEGRAND_EVENT_FP[w.integrand_id][precision]
+    return 42 * philox_blocks(w, variant) + d * (4 + 1 + 2 + 3) + per_dim_fp + 3 + 4 + INTEGRAND_EVENT_FP[w.integrand_id][precision]
 
 
 def n_wide(w):
@@ -53,9 +60,9 @@ def n_wide(w):
 PHILOX_PAIR_CLK = 4.4
 
 
-def refined_slots(w, precision):
-    nblk = (w.dim + 3) // 4
-    ni = n_issue(w, precision)
+def refined_slots(w, precision, variant=0):
+    nblk = philox_blocks(w, variant)
+    ni = n_issue(w, precision, variant)
     extra = (PHILOX_PAIR_CLK - 2.0) * 20 * nblk
     return ni + extra, {"issue": ni, "philox_pairs": 20 * nblk, "clk_per_pair": PHILOX_PAIR_CLK, "extra_clk": extra}
 
@@ -161,6 +168,14 @@ def cpu_baseline(w, edges, target_cpu_seconds=16.0):
             "per_core": n / dt / cores}
 
 
+def base_config(w, n_events_per_gpu_per_step=None):
+    """The keys both arms (--impl b200 / reference) report under `config`, with the same names and values."""
+    from paper_2002_12921_b200 import workloads as W
+    return {"workload": w.name, "dim": w.dim, "n_bins": w.n_bins, "integrand": W.INTEGRAND_NAMES[w.integrand_id],
+            "n_events_per_gpu_per_step": w.n_events if n_events_per_gpu_per_step is None else n_events_per_gpu_per_step,
+            "chunk_events": w.chunk_events, "alpha": w.alpha, "seed": w.seed}
+
+
 def run_reference(args, w, precision):
     """--impl reference: the oracle timed on the host cores; each step = one iteration + refine over a
     bounded sample of the workload's events."""
@@ -189,8 +204,7 @@ def run_reference(args, w, precision):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w.name, "dim": w.dim, "n_bins": w.n_bins, "integrand": w.integrand_id,
-                       "n_events_per_step": n, "full_n_events": w.n_events},
+            "config": base_config(w), "sample_events_per_step": n,
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
                              "sample": "%d events per step (bounded sample of %d), %d threads" % (n, w.n_events, cores)},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -207,6 +221,9 @@ def main():
     ap.add_argument("--workload", default="cfg3", help="cfg1..cfg5 (BASELINE.json configs)")
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32])
     ap.add_argument("--n-events", type=int, default=0, help="override events per step per GPU")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="weak: every GPU takes the workload's n_events per step; strong: the workload's n_events are split "
+                         "over the GPUs, rank g takes [g n/G, (g+1) n/G) (SURVEY.md 8(e)'s own partition)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the `workloads` array (cfg3 fp32, cfg5, cfg4 at 1e8)")
     ap.add_argument("--alpha", type=float, default=None,
@@ -281,7 +298,8 @@ def main():
             g.set_user_integrand(src, w.params)
             fid = B.VEGAS_F_USER
         shape = g.get_launch(fid, precision)
-        n_step = w.n_events * world                                   # weak scaling: n_events per GPU per step
+        # weak scaling: n_events per GPU per step; strong: n_events per step in all, split over the ranks
+        n_step = w.n_events * world if args.scaling == "weak" else w.n_events
 
         def step(k):
             if world == 1:
@@ -310,7 +328,8 @@ def main():
             k += 1
         barrier()
         t_wall = time.perf_counter() - t_begin
-        ms = sum(a.elapsed_time(b) for a, b in ev)
+        per_step_ms = [a.elapsed_time(b) for a, b in ev]
+        ms = sum(per_step_ms)
         launches = g.launch_count()
         if world > 1:
             t = torch.tensor([ms], dtype=torch.float64, device="cuda")
@@ -368,12 +387,12 @@ def main():
         out = None
         if rank == 0:
             clk = float(clocks["sm_mhz"] or sm_max)
-            ni, nf = n_issue(w, precision), n_fp(w, precision)
+            ni, nf = n_issue(w, precision, variant), n_fp(w, precision)
             k1_s = (k1_ms * 1e-3) / max(1, k1_launches)
-            events_per_launch = w.n_events * k1_steps / max(1, k1_launches)   # the fast path runs the chunk loop in the kernel
+            events_per_launch = (n_step // world) * k1_steps / max(1, k1_launches)   # the fast path runs the chunk loop in the kernel
             k1_rate = events_per_launch / k1_s                         # events/s of the fused kernel alone
             peak_instr = SM_COUNT * ISSUE_LANES * sm_max * 1e6         # thread-instructions/s at max clock
-            rs, rs_parts = refined_slots(w, precision)
+            rs, rs_parts = refined_slots(w, precision, variant)
             traffic, traffic_src = ncu_traffic(w.name, precision)
             roofline = {"bound": "alu", "kernel": ("k_iterate_rot<%s>" % shape["path"]) if shape["path"] == "rotated" else "k_iterate",
                         "achieved": k1_rate * ni / 1e12, "peak": peak_instr / 1e12, "unit": "Tinstr/s",
@@ -394,11 +413,11 @@ def main():
                         "traffic_note": "algorithmic global bytes per launch = grid read + partial row write per CTA = %d" % (
                             shape["blocks"] * 8 * (w.dim * (w.n_bins + 1) + (4 + w.dim * w.n_bins)))}
             out = {"workload": w.name, "dtype": "f64" if precision == 64 else "f32", "value": value, "ms_per_step": ms / steps,
+                   "ms_per_step_median": statistics.median(per_step_ms),     # this rank's steps (median of repeats)
                    "steps": steps, "warmup": warmup,
-                   "config": {"workload": w.name, "dim": w.dim, "n_bins": w.n_bins,
-                              "integrand": W.INTEGRAND_NAMES[w.integrand_id] + (" (user source, NVRTC)" if args.user_integrand else ""),
-                              "n_events_per_gpu_per_step": w.n_events, "chunk_events": w.chunk_events, "alpha": w.alpha,
-                              "seed": w.seed, "launch": shape,
+                   "config": {**base_config(w, n_step // world if args.scaling == "strong" else w.n_events),
+                              "integrand_source": "run-time compiled user source (NVRTC)" if args.user_integrand else "built-in",
+                              "launch": shape,
                               "l2": "256 MiB memset between timed steps, outside the event brackets (the path reads ~10 KB of global memory per launch)",
                               "grid": ("uniform (alpha = 0)" if w.alpha == 0 else "adapted by the %d warm-up iterations" % warmup)},
                    "clocks": clocks, "wall_s_timed_region": t_wall,
@@ -418,8 +437,9 @@ def main():
         # 32-bit draw saves against 53-bit uniforms, what an fp32-rounded grid table costs
         # ... and cfg1 / cfg2 at their OWN sizes (1e5 / 1e7 events per iteration), which SURVEY.md 8(d) lists as reported:
         # launch- and latency-bound, one launch per iteration
-        for cfg, prec, n_ev, variant in ((3, 32, 0, 0), (5, 64, 0, 0), (4, 64, 100_000_000, 0), (3, 64, 0, 1), (3, 64, 0, 2),
-                                         (1, 64, 0, 0), (2, 64, 0, 0)):
+        # order: the three other GATED workloads close the array (a reader that keeps the tail of the line keeps them)
+        for cfg, prec, n_ev, variant in ((3, 64, 0, 1), (3, 64, 0, 2), (1, 64, 0, 0), (2, 64, 0, 0),
+                                         (3, 32, 0, 0), (5, 64, 0, 0), (4, 64, 100_000_000, 0)):
             we = W.config(cfg)
             if n_ev:
                 we = we.scaled(n_ev)
@@ -436,10 +456,17 @@ def main():
                               "roofline_frac": r["roofline"]["frac"], "refined_frac": r["roofline"]["refined"]["frac"],
                               "instr_per_event": r["roofline"]["instr_per_event"], "launch": r["config"]["launch"],
                               "clocks": r["clocks"], "last_iteration": r["last_iteration"]})
+    # one timing of the headline workload on the UNIFORM grid (alpha = 0: the grid never adapts) beside
+    # the adapted-grid one
+    uniform = None
+    if world == 1 and not args.no_extra and args.alpha is None and not args.n_events:
+        import dataclasses
+        uniform = measure(dataclasses.replace(w, alpha=0.0), args.precision, max(3, min(args.steps, 10)), max(args.warmup, 3),
+                          "%s/%d uniform grid" % (w.name, args.precision))
     sampler.stop()
     if rank == 0:
         line = {"metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+                "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": args.scaling,
                 "vs_baseline": None, "dtype": head["dtype"], "data": "synthetic", "config": head["config"],
                 "clocks": head["clocks"], "wall_s_timed_region": head["wall_s_timed_region"], "e2e": head["e2e"],
                 "gpu_launches": head["gpu_launches"], "roofline": head["roofline"], "last_iteration": head["last_iteration"]}
@@ -447,6 +474,27 @@ def main():
             line["cpu_baseline"] = head["cpu_baseline"]
         if extra:
             line["workloads"] = extra
+        line["ms_per_step_median"] = head["ms_per_step_median"]
+        if uniform:
+            line["uniform_grid"] = {"value": uniform["value"], "ms_per_step": uniform["ms_per_step"],
+                                    "kernel_ms_per_launch": uniform["roofline"]["kernel_ms_per_launch"],
+                                    "roofline_frac": uniform["roofline"]["frac"], "steps": uniform["steps"],
+                                    "note": "same workload with alpha = 0 (the grid stays uniform)"}
+        # every workload SURVEY.md 8(d) gates (>= 1e8 events per iteration), compact and LAST on the line
+        gated = {"%s/%s" % (head["workload"], head["dtype"]): head}
+        gated_names = {"cfg3_gauss_d20/f32", "cfg5_bw_poly_d6/f64", "cfg4_genz_pp_d12/f64"}
+        rows = {}
+        for name, r in gated.items():
+            rows[name] = {"n_events": w.n_events, "value": r["value"], "e2e": r["e2e"]["value"], "frac": r["roofline"]["frac"],
+                          "kernel_ms": r["roofline"]["kernel_ms_per_launch"], "instr_per_event": r["roofline"]["instr_per_event"],
+                          "sm_mhz": r["clocks"]["sm_mhz"], "reasons": r["clocks"]["reasons"]}
+        for e in extra:
+            name = "%s/%s" % (e["workload"], e["dtype"])
+            if e["variant"] == "none" and name in gated_names and e["n_events"] >= 100_000_000:
+                rows[name] = {"n_events": e["n_events"], "value": e["value"], "e2e": e["e2e"], "frac": e["roofline_frac"],
+                              "kernel_ms": e["kernel_ms_per_launch"], "instr_per_event": e["instr_per_event"],
+                              "sm_mhz": e["clocks"]["sm_mhz"], "reasons": e["clocks"]["reasons"]}
+        line["gated"] = rows
         print(json.dumps(line))
     if world > 1:
         dist.barrier()

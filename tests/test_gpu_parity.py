@@ -350,9 +350,14 @@ def test_p7_constant_control_and_fixed_point(B):
 
 @pytest.mark.parametrize("cfg", [1, 2, 4, 5])
 def test_p7_five_sigma_rule(B, cfg):
-    w = _small(cfg).scaled(n_events=SMALL[cfg]["n_events"], n_iter=8)
+    if cfg == 1:
+        # cfg1 at its own size and length: SURVEY.md F1 gates every I_k from k = 0 and the average over all of them
+        w, n_skip = W.config(1), 0
+    else:
+        # reduced-size chains of the large configs (their first iterations under-estimate sigma at these sizes, F1);
+        # at full size they are gated from k = 0 in test_full_size_chains_match_the_survey_probe
+        w, n_skip = _small(cfg).scaled(n_events=SMALL[cfg]["n_events"], n_iter=8), 2
     g = _grid(B, w)
-    n_skip = 2                       # reduced-size chains: the first iterations under-estimate sigma (F1)
     r = g.integrate(w.n_iter, w.n_events, w.seed, w.alpha, w.integrand_id, 64, n_skip=n_skip)
     exact = w.closed_form
     assert abs(r["I"] - exact) < 5 * r["sigma"]
@@ -609,7 +614,13 @@ def test_full_size_chains_match_the_survey_probe(B, probe, cfg):
         for k in range(3, 10):
             assert abs(r["per_iter"][k, 0] - w.closed_form) < 5 * r["per_iter"][k, 1]
     else:
+        # SURVEY.md F1 (value +- error lands on the closed form): n_skip = 0 for cfg2, 4, 5 -- every
+        # I_k from the first, un-adapted iteration on, and the average over all of them; the survey's probe saw
+        # largest pulls of 2.50, 2.95 and 2.65
         assert abs(r["I"] - w.closed_form) < 5 * r["sigma"]
+        pulls = np.abs(r["per_iter"][:, 0] - w.closed_form) / r["per_iter"][:, 1]
+        assert np.all(pulls < 5.0), pulls
+        assert pulls.max() == pytest.approx({2: 2.50, 4: 2.95, 5: 2.65}[cfg], abs=0.02)
     g.close()
 
 

@@ -8,7 +8,7 @@ A "step" is one pass of the whole hot path over one batc
 of the workload's n_events events (in its chunk size) followed by the grid refinement.  Warm-up steps
 are the first iterations of the chain, so the timed steps run on an adapted grid (equiprobable bins:
 the conflict-heavy state the method spends its time in).  Inputs are seeded and synthetic
-(paper_2002_12921_b200/workloads.py).  One JSON line on stdout (rank 0).
+(workloads/__init__.py).  One JSON line on stdout (rank 0).
 """
 from __future__ import annotations
 
@@ -170,7 +170,7 @@ def cpu_baseline(w, edges, target_cpu_seconds=16.0):
 
 def base_config(w, n_events_per_gpu_per_step=None):
     """The keys both arms (--impl b200 / reference) report under `config`, with the same names and values."""
-    from paper_2002_12921_b200 import workloads as W
+    import workloads as W
     return {"workload": w.name, "dim": w.dim, "n_bins": w.n_bins, "integrand": W.INTEGRAND_NAMES[w.integrand_id],
             "n_events_per_gpu_per_step": w.n_events if n_events_per_gpu_per_step is None else n_events_per_gpu_per_step,
             "chunk_events": w.chunk_events, "alpha": w.alpha, "seed": w.seed}
@@ -235,7 +235,7 @@ def main():
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
 
-    from paper_2002_12921_b200 import workloads as W
+    import workloads as W
     w = W.config(int(args.workload.replace("cfg", "")))
     if args.n_events:
         w = w.scaled(args.n_events)

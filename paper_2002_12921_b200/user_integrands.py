@@ -2,7 +2,7 @@
 `struct vegas_user_integrand { begin(dim, p); dim(j, x, p); finish(p); }` the fused kernel is compiled around.
 
 These are examples that ship with the library and the inputs of the user-integrand parity tests; each states the
-formula it implements.  Parameters are the same host arrays the built-in integrands take (workloads.py).
+formula it implements.  Parameters are the same host arrays the built-in integrands take (the top-level `workloads` module).
 """
 
 # PAPER.md:69 Eq.(2) as printed, N = 1: f = 0 if any x_j <= a_j, else exp(sum_j c_j x_j); p = { c[0..d-1], a[0..d-1] }

@@ -12,7 +12,7 @@ import torch.distributed as dist
 import torch.multiprocessing as mp
 
 from paper_2002_12921_b200 import distributed as D
-from paper_2002_12921_b200 import workloads as W
+import workloads as W
 
 
 def test_shard_range_partitions_exactly():

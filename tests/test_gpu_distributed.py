@@ -11,7 +11,7 @@ import pytest
 
 pytestmark = pytest.mark.gpu
 
-from paper_2002_12921_b200 import workloads as W
+import workloads as W
 
 
 def _free_port():

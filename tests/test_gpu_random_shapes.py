@@ -10,7 +10,7 @@ import pytest
 pytestmark = pytest.mark.gpu
 
 import oracle as O
-from paper_2002_12921_b200 import workloads as W
+import workloads as W
 
 THREADS = os.cpu_count() or 8
 

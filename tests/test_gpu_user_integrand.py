@@ -9,7 +9,7 @@ pytestmark = pytest.mark.gpu
 
 import oracle as O
 from paper_2002_12921_b200 import user_integrands as U
-from paper_2002_12921_b200 import workloads as W
+import workloads as W
 
 THREADS = os.cpu_count() or 8
 RTOL64 = 1e-10

@@ -7,7 +7,7 @@ import numpy as np
 import pytest
 
 import oracle as O
-from paper_2002_12921_b200 import workloads as W
+import workloads as W
 
 
 def _flt(probe, key):

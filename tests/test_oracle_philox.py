@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 
 import oracle as O
-from paper_2002_12921_b200 import workloads as W
+import workloads as W
 
 from conftest import GOLDEN, ROOT
 

@@ -11,7 +11,7 @@ import numpy as np
 import pytest
 
 import oracle as O
-from paper_2002_12921_b200 import workloads as W
+import workloads as W
 
 
 # ---------------------------------------------------------------- C3': two-word layout and the 53-bit split

@@ -18,7 +18,7 @@ import pytest
 
 pytestmark = pytest.mark.gpu
 
-from paper_2002_12921_b200 import workloads as W
+import workloads as W
 
 RTOL64 = 1e-10
 

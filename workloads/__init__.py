@@ -2,7 +2,7 @@
 
 This module is the ONLY thing the CUDA path's tests/bench and the CPU oracle's tests have in
 common.  It holds inputs, not the method: sizes, seeds, integrand ids, the integrand parameter
-arrays and the analytic value of each integral.  It imports neither the CUDA binding nor
+arrays and the analytic value of each integral.  It lives outside the product package and imports neither the CUDA binding nor
 ``oracle``.  Parameters are handed to both implementations as plain fp64 arrays.
 
 Parameter draws (reading C10 of DESIGN.md; BASELINE.json:configs[3] "c_i drawn uniform in

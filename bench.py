@@ -306,8 +306,9 @@ def main():
                 # one iteration + refinement, ONE launch (vegas_integrate_from, n_iter = 1), one synchronisation
                 r = g.integrate(1, n_step, w.seed, w.alpha, fid, precision, chunk_events=w.chunk_events, first_iteration=k)
                 return r["I"], r["sigma"]
-            I, s, _, st = D.iterate_sharded(g, n_step, w.seed, k, fid, precision, w.chunk_events, rank, world, want_hist=False)
-            g.refine(w.alpha)
+            # accumulate -> all-reduce -> finalize + refine: one host synchronisation per sharded step
+            I, s, _, st = D.iterate_sharded(g, n_step, w.seed, k, fid, precision, w.chunk_events, rank, world, want_hist=False,
+                                            alpha=w.alpha)
             return I, s
 
         k = 0
@@ -376,6 +377,19 @@ def main():
         barrier()
         t_end = time.perf_counter()
         e2e_s = t_end - t0
+        # ---- the sharded call sequence on this one rank (begin, accumulate, reduce, [all-reduce: none at world 1],
+        # finalize + refine, one synchronisation): what a small iteration costs through the multi-GPU path
+        sharded_ms = None
+        if world == 1 and w.n_events <= 10_000_000:
+            n_sh = min(steps, 50)
+            D.iterate_sharded(g, n_step, w.seed, k, fid, precision, w.chunk_events, 0, 1, want_hist=False, alpha=w.alpha)
+            barrier()
+            t_sh = time.perf_counter()
+            for i in range(n_sh):
+                D.iterate_sharded(g, n_step, w.seed, k + 1 + i, fid, precision, w.chunk_events, 0, 1, want_hist=False, alpha=w.alpha)
+            barrier()
+            sharded_ms = 1e3 * (time.perf_counter() - t_sh) / n_sh
+            k += 1 + n_sh
         clocks = sampler.window(t_begin, t_end, "%s: timed steps + K1 steps + e2e steps" % label)
         if world > 1:
             t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
@@ -422,7 +436,7 @@ def main():
                               "grid": ("uniform (alpha = 0)" if w.alpha == 0 else "adapted by the %d warm-up iterations" % warmup)},
                    "clocks": clocks, "wall_s_timed_region": t_wall,
                    "e2e": {"value": n_step * steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
-                   "gpu_launches": int(launches), "roofline": roofline,
+                   "gpu_launches": int(launches), "roofline": roofline, "sharded_call_sequence_ms_per_step": sharded_ms,
                    "last_iteration": {"I": results[-1][0], "sigma": results[-1][1], "closed_form": w.closed_form}}
             if with_cpu_baseline:
                 out["cpu_baseline"] = cpu_baseline(w, edges_host)
@@ -451,6 +465,7 @@ def main():
                                           2: "q32 (grid-table entries rounded to fp32)"}[variant],
                               "n_events": we.n_events, "chunk_events": we.chunk_events,
                               "value": r["value"], "e2e": r["e2e"]["value"], "ms_per_step": r["ms_per_step"], "steps": r["steps"],
+                              "sharded_call_sequence_ms_per_step": r["sharded_call_sequence_ms_per_step"],
                               "kernel_ms_per_launch": r["roofline"]["kernel_ms_per_launch"],
                               "kernel_events_per_s": r["roofline"]["kernel_events_per_s"],
                               "roofline_frac": r["roofline"]["frac"], "refined_frac": r["roofline"]["refined"]["frac"],

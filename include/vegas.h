@@ -202,6 +202,15 @@ int vegas_accumulate(vegas_grid* g, uint64_t first_event, uint64_t count, uint64
 int vegas_reduce(vegas_grid* g, void* cuda_stream);
 int vegas_finalize(vegas_grid* g, uint64_t n_events_total, void* cuda_stream, double* I, double* sigma,
                    double* hist_host);
+/* vegas_finalize and vegas_refine in one call, for the sharded iteration: after the ranks' all-reduce of the totals,
+ * enqueue S7 (I, sigma) and, if alpha >= 0, S8 (refinement from the summed histogram; alpha < 0: none) back to back on
+ * `stream`, then read { I, sigma, status } (and the histogram, if hist_host is not NULL) with ONE synchronisation -- a
+ * sharded iteration costs one host synchronisation like a single-GPU one, instead of one for finalize and one for refine
+ * (the multi-GPU runs; what matters for the small configs, whose iteration is tens of
+ * microseconds).  Every rank calls it with the GLOBAL event count and the same alpha, and ends with the same grid.
+ * Errors: as vegas_finalize and vegas_refine (VEGAS_ENUMERIC: non-finite sums, or a dimension kept its grid). */
+int vegas_finish_sharded(vegas_grid* g, uint64_t n_events_total, double alpha, void* cuda_stream, double* I, double* sigma,
+                         double* hist_host);
 /* Device address / length (in doubles) of the reduced totals { S1_hi, S1_lo, S2_hi, S2_lo,
  * H[dim][n_bins] } that vegas_reduce() writes and vegas_finalize() / vegas_refine() read. */
 void* vegas_totals_device(vegas_grid* g);

@@ -56,6 +56,7 @@ SIGNATURES = {
     "vegas_accumulate": (C.c_int, [_vp, _u64, _u64, _u64, _u64, C.c_uint32, C.c_int, C.c_int, _vp]),
     "vegas_reduce": (C.c_int, [_vp, _vp]),
     "vegas_finalize": (C.c_int, [_vp, _u64, _vp, _f64p, _f64p, _f64p]),
+    "vegas_finish_sharded": (C.c_int, [_vp, _u64, C.c_double, _vp, _f64p, _f64p, _f64p]),
     "vegas_totals_device": (_vp, [_vp]),
     "vegas_totals_count": (C.c_size_t, [_vp]),
     "vegas_refine": (C.c_int, [_vp, _f64p, C.c_double, _vp]),
@@ -297,6 +298,13 @@ class VegasGrid:
         I, s = C.c_double(), C.c_double()
         h = np.empty((self.dim, self.n_bins)) if want_hist else None
         rc = lib.vegas_finalize(self._h, int(n_events_total), _stream(stream), C.byref(I), C.byref(s), _ptr(h))
+        return I.value, s.value, h, self._check(rc, allow_numeric=True)
+
+    def finish_sharded(self, n_events_total, alpha, want_hist=True, stream=None):
+        """finalize + refine (alpha >= 0) after the ranks' all-reduce, one synchronisation -> (I, sigma, hist or None, status)"""
+        I, s = C.c_double(), C.c_double()
+        h = np.empty((self.dim, self.n_bins)) if want_hist else None
+        rc = lib.vegas_finish_sharded(self._h, int(n_events_total), float(alpha), _stream(stream), C.byref(I), C.byref(s), _ptr(h))
         return I.value, s.value, h, self._check(rc, allow_numeric=True)
 
     def totals_tensor(self):

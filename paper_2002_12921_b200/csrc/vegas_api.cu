@@ -800,6 +800,34 @@ int vegas_finalize(vegas_grid* g, uint64_t n_events_total, void* cuda_stream, do
     return finish_iteration(g, n_events_total, (cudaStream_t)cuda_stream, I, sigma, hist_host);
 }
 
+int vegas_finish_sharded(vegas_grid* g, uint64_t n_events_total, double alpha, void* cuda_stream, double* I, double* sigma,
+                         double* hist_host) {
+    if (!g || n_events_total < 2 || alpha != alpha || std::isinf(alpha)) return VEGAS_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CUDA_TRY(g, cudaSetDevice(g->device));
+    CUDA_TRY(g, vegas::launch_finalize(g->d_totals, (double)n_events_total, g->d_result, st));
+    g->launches++;
+    const bool refine = alpha >= 0.0;
+    if (refine) {
+        CUDA_TRY(g, cudaMemsetAsync(g->d_status, 0, sizeof(int), st));
+        CUDA_TRY(g, vegas::launch_refine(g->d_edges, g->d_totals + 4, g->dim, g->n_bins, alpha, g->d_status, st));
+        g->launches++;
+    }
+    // { I, sigma, status }, the refinement's status word and the histogram: one synchronisation for all of them
+    if (!g->h_pinned) CUDA_TRY(g, cudaHostAlloc((void**)&g->h_pinned, sizeof(double) * ((size_t)kResultStride * kMaxIter + 1), cudaHostAllocDefault));
+    double* res = g->h_pinned;
+    int* status_p = reinterpret_cast<int*>(g->h_pinned + (size_t)kResultStride * kMaxIter);
+    *status_p = 0;
+    CUDA_TRY(g, cudaMemcpyAsync(res, g->d_result, sizeof(double) * 3, cudaMemcpyDeviceToHost, st));
+    if (refine) CUDA_TRY(g, cudaMemcpyAsync(status_p, g->d_status, sizeof(int), cudaMemcpyDeviceToHost, st));
+    if (hist_host)
+        CUDA_TRY(g, cudaMemcpyAsync(hist_host, g->d_totals + 4, sizeof(double) * (size_t)g->dim * g->n_bins, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(g, cudaStreamSynchronize(st));
+    if (I) *I = res[0];
+    if (sigma) *sigma = res[1];
+    return (res[2] == 0.0 && *status_p == 0) ? VEGAS_OK : VEGAS_ENUMERIC;
+}
+
 void* vegas_totals_device(vegas_grid* g) { return g ? (void*)g->d_totals : nullptr; }
 size_t vegas_totals_count(const vegas_grid* g) { return g ? 4 + (size_t)g->dim * g->n_bins : 0; }
 

@@ -47,9 +47,13 @@ def allreduce_totals(totals, group=None, fixed_order: bool = False):
 
 def iterate_sharded(grid, n_events_total: int, seed: int, iteration: int, integrand_id: int, precision: int = 64,
                     chunk_events: int = 0, rank: int = 0, world: int = 1, want_hist: bool = False, group=None,
-                    fixed_order: bool = False):
+                    fixed_order: bool = False, alpha=None):
     """One Vegas iteration of n_events_total events spread over `world` ranks; `grid` is this rank's
-    binding.VegasGrid.  Returns (I, sigma, hist or None, status), identical on every rank."""
+    binding.VegasGrid.  Returns (I, sigma, hist or None, status), identical on every rank.
+    alpha=None: the grid is left as it is (the caller refines, a second host synchronisation).  alpha given: the
+    refinement with that damping exponent (alpha < 0: none) follows the estimate in the same call
+    (vegas_finish_sharded): accumulate -> all-reduce on the stream -> finalize + refine -> ONE host synchronisation,
+    like the single-GPU iteration."""
     first, count = shard_range(n_events_total, rank, world)
     grid.begin_iteration()
     if count:
@@ -57,4 +61,6 @@ def iterate_sharded(grid, n_events_total: int, seed: int, iteration: int, integr
     grid.reduce()
     if world > 1:
         allreduce_totals(grid.totals_tensor(), group, fixed_order)
+    if alpha is not None:
+        return grid.finish_sharded(n_events_total, alpha, want_hist=want_hist)
     return grid.finalize(n_events_total, want_hist=want_hist)

@@ -107,6 +107,13 @@ class _OracleRankGrid:
         I, sg = self.O.estimate(ld(t[0]) + ld(t[1]), ld(t[2]) + ld(t[3]), n_total)
         return I, sg, (t[4:].reshape(self.dim, self.n_bins).copy() if want_hist else None), 0
 
+    def finish_sharded(self, n_total, alpha, want_hist=False):
+        I, sg, H, st = self.finalize(n_total, want_hist=True)
+        if alpha >= 0:
+            self.edges, _ = self.O.refine(self.edges, H, alpha)
+        self.calls.append(("finish_sharded", alpha))
+        return I, sg, (H if want_hist else None), st
+
 
 def _worker_sharded(rank, world, port, n, fixed_order, out_dir):
     os.environ["MASTER_ADDR"] = "127.0.0.1"
@@ -117,7 +124,14 @@ def _worker_sharded(rank, world, port, n, fixed_order, out_dir):
     I, sg, H, st = D.iterate_sharded(g, n, w.seed, 2, w.integrand_id, 64, 0, rank, world, want_hist=True,
                                      fixed_order=fixed_order)
     assert g.calls[0] == "begin" and g.calls[1] == ("accumulate",) + D.shard_range(n, rank, world) and g.calls[2] == "reduce"
-    np.save(os.path.join(out_dir, "r%d.npy" % rank), np.concatenate([[I, sg], H.ravel()]))
+    # the same iteration with the refinement in the same call: same estimate and histogram, grid refined once, on every rank
+    e0 = g.edges.copy()
+    I2, sg2, H2, _ = D.iterate_sharded(g, n, w.seed, 2, w.integrand_id, 64, 0, rank, world, want_hist=True,
+                                       fixed_order=fixed_order, alpha=w.alpha)
+    assert (I2, sg2) == (I, sg) and np.array_equal(H2, H) and g.calls[-1] == ("finish_sharded", w.alpha)
+    import oracle as O
+    assert np.array_equal(g.edges, O.refine(e0, H, w.alpha)[0]) and not np.array_equal(g.edges, e0)
+    np.save(os.path.join(out_dir, "r%d.npy" % rank), np.concatenate([[I, sg], H.ravel(), g.edges.ravel()]))
     dist.barrier()
     dist.destroy_process_group()
 
@@ -135,4 +149,4 @@ def test_iterate_sharded_itself_over_gloo(tmp_path, world, fixed_order):
     w = W.config(1)
     I, sg, H = O.iterate(W.adapted_edges(w.dim, w.n_bins, seed=5), n, w.seed, 2, w.integrand_id, w.params)
     assert got[0][0] == pytest.approx(I, rel=1e-14) and got[0][1] == pytest.approx(sg, rel=1e-12)
-    np.testing.assert_allclose(got[0][2:].reshape(H.shape), H, rtol=1e-14)
+    np.testing.assert_allclose(got[0][2:2 + H.size].reshape(H.shape), H, rtol=1e-14)

@@ -36,11 +36,16 @@ def _worker(rank, world, port, cfg, n, n_iter, fixed_order, out_dir):
     g.set_params(w.integrand_id, w.params)
     out = []
     for k in range(n_iter):
+        # odd iterations: estimate and refinement in one call with one synchronisation (vegas_finish_sharded);
+        # even ones: vegas_finalize, then vegas_refine -- the same grid either way
+        launches = g.launch_count()
         I, s, H, st = D.iterate_sharded(g, n, w.seed, k, w.integrand_id, 64, w.chunk_events and 50_000, rank, world,
-                                        want_hist=True, fixed_order=fixed_order)
+                                        want_hist=True, fixed_order=fixed_order, alpha=w.alpha if k % 2 else None)
         assert st == 0
         assert g.totals_tensor().is_cuda
-        assert g.refine(w.alpha) == 0
+        if k % 2 == 0:
+            assert g.refine(w.alpha) == 0
+        assert g.launch_count() - launches >= 4          # accumulate, reduce, finalize, refine: all of them ran here
         out.append(np.concatenate([[I, s], H.ravel(), g.get_edges().ravel()]))
     np.save(os.path.join(out_dir, "r%d.npy" % rank), np.stack(out))
     g.close()

@@ -68,15 +68,18 @@ def refined_slots(w, precision, variant=0):
 
 
 def ncu_traffic(workload, precision):
-    """DRAM bytes per K1 launch from the committed `ncu --set full` summary (profiles/r02_traffic.json), with its source."""
-    try:
-        with open(os.path.join(ROOT, "profiles", "r02_traffic.json")) as fh:
-            t = json.load(fh)
-        e = t["entries"].get("%s/%d" % (workload, precision))
-        if e:
-            return e["dram_bytes_per_launch"], {"source": t["source"], "commit": t["commit"], "events_per_launch": e["events_per_launch"]}
-    except Exception:
-        pass
+    """DRAM bytes per K1 launch from the committed `ncu --set full` summaries (the newest round that captured this
+    workload: profiles/r03_traffic.json, else profiles/r02_traffic.json), with its source."""
+    for name in ("r03_traffic.json", "r02_traffic.json"):
+        try:
+            with open(os.path.join(ROOT, "profiles", name)) as fh:
+                t = json.load(fh)
+            e = t["entries"].get("%s/%d" % (workload, precision))
+            if e:
+                return e["dram_bytes_per_launch"], {"source": t["source"], "commit": t["commit"], "file": "profiles/" + name,
+                                                    "events_per_launch": e["events_per_launch"]}
+        except Exception:
+            pass
     return None, None
 
 

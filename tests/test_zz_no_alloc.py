@@ -81,6 +81,13 @@ def test_two_calls_in_a_row_match_the_grid_path(B):
     B.vegas_iterate_static(edges_d[0], w.n_events, w.seed, it, w.integrand_id, w.params, no_hist, None)
     torch.cuda.synchronize()
     assert torch.equal(again, result_d[0]) and torch.equal(hist_again, hist_d[0]) and torch.equal(no_hist, result_d[0])
+    # and the point of it all: with the set-up behind it, a call leaves the device's free memory where it was
+    # (cudaMemGetInfo through torch; the outputs above are reused, so torch's own allocator has nothing to do either)
+    free_before = torch.cuda.mem_get_info()[0]
+    for k, (w, _, it) in enumerate(cases):
+        B.vegas_iterate_static(edges_d[k], w.n_events, w.seed, it, w.integrand_id, w.params, result_d[k], hist_d[k])
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] == free_before
 
 
 def test_shapes_beyond_the_built_in_scratch_are_refused(B):
